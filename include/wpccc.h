@@ -1,0 +1,180 @@
+/* wpccc.h -- C ABI of the B200-native WP-CCC hot path (arXiv 2403.04252).
+ *
+ * The library evaluates, at every projectile position R(t) = (b, 0, v t) of many straight-line
+ * trajectories, the coupling matrix elements of the two-centre close-coupling equations
+ * (eq. (1)) and advances the amplitudes by classical RK4 (Algorithm 1,
+ * PAPER.md L69-104).  Citations "P:Lnnn" are lines of /root/reference/PAPER.md; "A<n>" are the
+ * readings of the paper listed in DESIGN.md (section "Readings").
+ *
+ * Conventions common to every entry point
+ *   - Plain pointers and sizes only.  Each pointer argument is marked [host] or [device].
+ *   - The library NEVER allocates device memory for data: the caller owns the basis arena, the
+ *     workspace and every output buffer.  A pointer is borrowed for the duration of the call,
+ *     except the arena, which the basis handle keeps using until wpccc_free_basis().
+ *   - All device work is enqueued on the caller's CUDA stream (`stream` is a cudaStream_t passed
+ *     as void*; NULL = legacy default stream).  wpccc_propagate additionally forks onto one
+ *     internal stream and joins back before it returns control to `stream` order.
+ *     Calls are asynchronous with respect to the host unless stated otherwise.
+ *   - Complex numbers are interleaved double[2] = (re, im).  All arithmetic is IEEE fp64.
+ *   - Return value: 0 on success, a negative WPCCC_E* code otherwise; wpccc_last_error() gives a
+ *     thread-local message.  There is no CPU fallback: without a CUDA device every compute call
+ *     returns WPCCC_ECUDA.
+ *   - State ordering (binding): centre T then centre P; inside a centre the radial functions in
+ *     caller order; each radial function expands to m = -l .. +l ascending.
+ *   - Geometry (A.1): target nucleus at the origin, projectile at (b, 0, z), velocity v along +z,
+ *     b >= 0.  Atomic units.
+ */
+#ifndef WPCCC_H
+#define WPCCC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WPCCC_OK          0
+#define WPCCC_EINVAL     (-1)  /* bad argument (message says which)                               */
+#define WPCCC_ENOMEM     (-2)  /* arena or workspace too small                                     */
+#define WPCCC_ECUDA      (-3)  /* CUDA runtime error / no device                                   */
+#define WPCCC_ESINGULAR  (-4)  /* zero pivot in the overlap solve, or |S_PT| >= 1 (see propagate)  */
+
+typedef struct wpccc_basis wpccc_basis; /* opaque */
+
+/* One expansion centre: bound eigenstates plus wave-packet pseudostates tabulated on the
+ * uniform radial grid r_k = k h, k = 0..Nr ("precomputed and stored"; A7).  All arrays [host]. */
+typedef struct {
+    double        Z;      /* nuclear charge of this centre (H: 1, He2+: 2)                         */
+    int           n_rad;  /* number of radial functions                                            */
+    const int    *l;      /* [n_rad] orbital angular momentum                                      */
+    const double *eps;    /* [n_rad] energies eps_a (a.u.), used in the phases e^{i(eps'-eps)z/v}  */
+    const int    *kind;   /* [n_rad] 0 = bound eigenstate, 1 = wave packet (labels for classes)    */
+    const int    *nq;     /* [n_rad] principal quantum number or bin index (labels only)           */
+    const double *u;      /* [n_rad][Nr+1] reduced radial function u_a(r_k) = r f_a(r), u(0) = 0   */
+    const double *g;      /* [n_rad][Nr+1] residual (H_c - eps_a) u_a (A5); NULL = all zero        */
+} wpccc_centre;
+
+/* Fixed Gauss-Legendre product rule for the two-centre integrals in body-frame cylindrical
+ * coordinates (rho', phi', z') (BASELINE.json configs[1], [3]; A10):
+ *   rho' one panel on [0, rho_max] (n_rho nodes); phi' one panel on [0, 2 pi] (n_phi nodes);
+ *   z' three panels [-z_pad, 0], [0, R], [R, R + z_pad] with n_z/4, n_z/2, n_z/4 nodes.
+ * n_z must be a multiple of 16, n_rho >= 1, n_phi >= 1.
+ * phi_rule 0: the discrete n_phi-node sum.  phi_rule 1: the continuum azimuthal integral
+ * (-+i)^Delta J_Delta(x) of eq. (9), evaluated by a 512-node periodic trapezoid rule
+ * (exact to rounding for x + |Delta| < 400). */
+typedef struct {
+    int    n_rho, n_phi, n_z;
+    double rho_max, z_pad;
+    int    phi_rule;
+} wpccc_quad;
+
+/* ---- a0: staging ("stored in the GPU global memory") ------------ */
+
+/* Bytes of device arena wpccc_setup_basis needs for this problem (0 on invalid arguments). */
+size_t wpccc_basis_bytes(int n_centres, const wpccc_centre *centres /*[host]*/, int Nr, int lambda_max,
+                         const wpccc_quad *quad /*[host] or NULL*/);
+
+/* Copies the host tables, builds the position-independent tables (angular coefficients of eq. (6),
+ * pair-product matrix w_k u_a'(r_k) u_a(r_k) for eq. (7), interpolation tables, Gauss-Legendre
+ * nodes) into `dev_arena` [device, arena_bytes, 256-byte aligned] and returns a handle.
+ *   n_centres 1: target centre only (eq. (5): S = I, H = D^T);  2: target then projectile.
+ *   Z_proj: charge seen by target-centred states; with two centres it must equal centres[1].Z.
+ *   h, w[Nr+1] [host]: grid step and quadrature weights of the radial grid (A7, A8); w[0] ignored.
+ *   lambda_max: largest multipole in eq. (6).
+ * Host arrays are copied before return (the call synchronises `stream`).  The handle itself is
+ * host memory owned by the library; free it with wpccc_free_basis (the arena stays the caller's). */
+int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_centre *centres /*[host]*/,
+                      double Z_proj, int Nr, double h, const double *w /*[host]*/, int lambda_max,
+                      const wpccc_quad *quad /*[host]; NULL iff n_centres == 1*/,
+                      void *dev_arena /*[device]*/, size_t arena_bytes, void *stream);
+void wpccc_free_basis(wpccc_basis *basis);
+
+/* Sizes the caller needs to allocate outputs: total number of states N_tot, states on centre c,
+ * radial functions on centre c, number of radial entries E_c = allowed (a' <= a, lambda) of centre c. */
+int wpccc_n_states(const wpccc_basis *basis);
+int wpccc_n_states_centre(const wpccc_basis *basis, int c);
+int wpccc_n_rad_centre(const wpccc_basis *basis, int c);
+int wpccc_n_radial_entries(const wpccc_basis *basis, int c);
+/* Describes radial entry e of centre c: (a', a, lambda) with a' <= a.  Returns 0 or WPCCC_EINVAL. */
+int wpccc_radial_entry(const wpccc_basis *basis, int c, int e, int *a_prime, int *a, int *lambda);
+
+/* Workspace bytes.  what = 0: wpccc_matrix_elements for n_traj positions (n_steps ignored);
+ * what = 1: wpccc_propagate of n_traj trajectories with n_steps RK4 steps (a size that lets the
+ * pipeline keep its preferred window; any size >= the value for what = 2 works, with shorter
+ * windows); what = 2: the minimum wpccc_propagate accepts. */
+size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, int what);
+
+/* ---- a1-a6: matrix elements at given positions ------------------------------------------------
+ * For each position p (b[p], z[p], v[p]) [host arrays] computes
+ *   S = [[I, S_PT^H], [S_PT, I]],  H = [[D^T, H_TP], [H_PT, D^P]]            (eq. (1); A1)
+ *   D^T, D^P   direct elements, eq. (6)-(7), radial integral as the grid sum over r_k
+ *              evaluated at the exact R (A9), by an FP64 tensor-core GEMM over the radial grid;
+ *   S_PT, H_PT, H_TP  two-centre overlap and electron-transfer elements with the translation
+ *              factor e^{-+ i v z_m} (eq. (8)-(9) structure; A4, A5, A10) by the fixed
+ *              product rule of wpccc_quad.
+ * flags bit 0: multiply every element by e^{i (eps_row - eps_col) z / v} (interaction picture, A2).
+ * flags bit 1: also return the radial entries F^c_lambda(a', a; R) in dF.
+ * Outputs [device]: dS, dH [n_pos][N_tot][N_tot] complex, row-major (either may be NULL);
+ *   dF [n_pos][E_T (+ E_P)] doubles (centre T entries then centre P), or NULL.
+ * With one centre S is the identity and H = D^T. */
+int wpccc_matrix_elements(const wpccc_basis *basis, int n_pos, const double *b /*[host]*/,
+                          const double *z /*[host]*/, const double *v /*[host]*/, int flags,
+                          double *dS /*[device]*/, double *dH /*[device]*/, double *dF /*[device]*/,
+                          void *ws /*[device]*/, size_t ws_bytes, void *stream);
+
+/* ---- a1-a8: propagation ------------------------------------------------------------------------
+ * Integrates i S dc/dt = H c, i.e. dc/dz = -(i/v) S^{-1} H c (eq. (2)-(4)), for n_traj
+ * straight-line trajectories (b[t], v[t]) [host arrays] concurrently, with classical RK4
+ * (Algorithm 1) on the uniform grid z_i = z_min + i (z_max - z_min)/n_steps (A13).
+ * The 2 n_steps + 1 evaluations of (S, H) per path are computed in windows for all
+ * trajectories at once; the overlap system is factorised by Gaussian elimination with partial
+ * pivoting (the role of ZGESV) and solved once per RK4 stage (A14).
+ * Initial condition c = delta_{j, init_state}.
+ * Outputs [device]: dC [n_traj][N_tot] complex amplitudes at z_max;
+ *   d_norm_drift [n_traj] max over steps of |c^H S c - 1| (A17), or NULL.
+ * Errors: WPCCC_ENOMEM if ws_bytes < wpccc_workspace_bytes(.., 2).  A zero pivot, or an overlap
+ * element with |S_PT| >= 1 (which would invalidate the pivot order the factorisation relies on,
+ * DESIGN.md "a7"), is detected on the device; the call then synchronises and returns
+ * WPCCC_ESINGULAR.  The call synchronises `stream` before returning (it reads that status). */
+int wpccc_propagate(const wpccc_basis *basis, int n_traj, const double *b /*[host]*/,
+                    const double *v /*[host]*/, double z_min, double z_max, int n_steps, int init_state,
+                    double *dC /*[device]*/, double *d_norm_drift /*[device] or NULL*/,
+                    void *ws /*[device]*/, size_t ws_bytes, void *stream);
+
+/* ---- a9: observables ------------------------------------------------------------------
+ * From amplitudes dC [device, n_traj][N_tot] complex:
+ *   P_state [n_traj][N_tot]       |c_j|^2
+ *   P_nl    [n_traj][n_rad_tot]   sum over m for each radial function (centre T functions, then P)
+ *   P_class [n_traj][5]           elastic (radial function of init_state), target excitation (bound),
+ *                                 target continuum (wave packets), capture bound, capture continuum
+ *   sigma_nl [n_vgroups][n_rad_tot], sigma_class [n_vgroups][5]
+ *                                 2 pi Int b P(b) db by the trapezoid rule in ln b over the
+ *                                 trajectories of each velocity group, sorted by b (units a0^2).
+ * b [host][n_traj], vgroup [host][n_traj] in 0..n_vgroups-1.  All outputs [device]; any may be NULL
+ * (sigma_* need b and vgroup). */
+int wpccc_probabilities(const wpccc_basis *basis, int n_traj, const double *dC /*[device]*/,
+                        const double *b /*[host]*/, const int *vgroup /*[host]*/, int n_vgroups,
+                        int init_state, double *P_state, double *P_nl, double *P_class,
+                        double *sigma_nl, double *sigma_class, void *stream);
+
+/* ---- diagnostics ----------------------------------------------------------------------------- */
+
+/* Per-family device time of the last wpccc_propagate / wpccc_matrix_elements call on this handle,
+ * in milliseconds, measured with CUDA events on the streams the kernels ran on, and launch counts.
+ * ms[k], launches[k], k: 0 direct GEMM (a2), 1 direct assembly (a3), 2 transfer node tables (a4),
+ * 3 transfer contraction (a5), 4 rotation/assembly (a6), 5 factorisation (a7), 6 RK4 sweep (a8),
+ * 7 other.  Synchronises the device.  Returns the number of families (8). */
+int wpccc_last_timing(const wpccc_basis *basis, double *ms /*[host][8]*/, long long *launches /*[host][8]*/);
+
+/* Measures the device's FP64 peak with a register-resident micro-benchmark on `stream`:
+ * kind 0 = DFMA (plain FP64 FMA pipe), kind 1 = DMMA (mma.sync.m8n8k4.f64).  Returns TFLOP/s
+ * (negative WPCCC_E* as a double on error).  Used by bench.py for the roofline denominator. */
+double wpccc_fp64_peak(int kind, void *stream);
+
+const char *wpccc_last_error(void);
+const char *wpccc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WPCCC_H */

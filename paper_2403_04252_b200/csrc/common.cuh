@@ -1,0 +1,110 @@
+// Internal declarations shared by the translation units of libwpccc.so (not part of the C ABI).
+// Notation follows the paper (arXiv 2403.04252) and DESIGN.md: centres T, P; radial functions a, a';
+// states alpha = (a, m); multipole lambda; F^c_lambda(a',a;R) radial entries of eq. (7); D^T, D^P of eq. (6);
+// body-frame two-centre integrals of eq. (9) rotated by Wigner d(Theta) as in eq. (8).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "wpccc.h"
+
+#define WP_MAX_L 6        // largest orbital momentum supported per centre
+#define WP_MAX_LAMBDA 12  // largest multipole (2 * WP_MAX_L)
+#define WP_NFAM 8         // timing families (wpccc_last_timing)
+
+enum { FAM_GEMM = 0, FAM_DASM = 1, FAM_TTAB = 2, FAM_TCON = 3, FAM_ROT = 4, FAM_FACT = 5, FAM_SWEEP = 6, FAM_OTHER = 7 };
+
+void wp_set_error(const char *fmt, ...);
+#define WP_FAIL(code, ...) do { wp_set_error(__VA_ARGS__); return (code); } while (0)
+#define WP_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    wp_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); return WPCCC_ECUDA; } } while (0)
+
+// One n-tile of the grouped direct GEMM: columns [n0, n0+cnt) of multipole `lam` of centre `c`.
+struct GemmTile { int c, lam, n0, cnt; };
+
+// Column of the transfer node tables: radial function `rad` with body-frame projection q >= 0.
+struct CentreTab {
+    double Z = 0;
+    int n_rad = 0, n_states = 0, l_max = 0;
+    std::vector<int> l, kind, nq;
+    std::vector<double> eps;
+    std::vector<int> st_rad, st_l, st_m, rad_first;
+    // direct: entries e = (a' <= a, lambda), grouped by lambda
+    int n_pairs = 0, E = 0;
+    std::vector<int> lam_off, ent_a1, ent_a, ent_lam, ent_pair;
+    // transfer: columns (a, q >= 0), grouped by q
+    int nqc = 0, nqc_pad = 0;
+    std::vector<int> col_rad, col_q, q_off;
+    // device tables (inside the caller's arena)
+    double *d_PP = nullptr;        // [n_pairs][Kpad]  w_k u_a'(r_k) u_a(r_k), k = 1..Nr (index k-1), zero padded
+    int    *d_ent_pair = nullptr;  // [E]              pair row of entry e
+    int    *d_ent_lookup = nullptr;// [lambda_max+1][n_rad][n_rad]  entry index of (lambda, a', a), -1 if not allowed
+    double *d_G = nullptr;         // [(Lc+1)^2][(Lc+1)^2][lambda_max+1]  G^lambda_{(l'm'),(lm)} of eq. (6)
+    double *d_Ut = nullptr;        // [Nr+1][nf_pad]   row k: u_a(r_k) (a = 0..n_rad-1) then g_a(r_k)
+    int    *d_st_rad = nullptr, *d_st_l = nullptr, *d_st_m = nullptr;   // [n_states]
+    double *d_eps = nullptr;       // [n_rad]
+    int    *d_l = nullptr;         // [n_rad]
+    int    *d_col_rad = nullptr, *d_col_q = nullptr;                    // [nqc_pad] (-1 padding)
+    int    *d_rad_first = nullptr; // [n_rad]
+    int nf_pad = 0;
+};
+
+struct wpccc_basis {
+    int n_centres = 0, Nr = 0, Kpad = 0, lambda_max = 0, n_tot = 0;
+    double h = 0, Z_proj = 0;
+    wpccc_quad quad{};
+    bool has_quad = false;
+    CentreTab c[2];
+    int E_tot = 0;
+    std::vector<GemmTile> tiles;
+    // shared device tables
+    double *d_rp = nullptr;    // [lambda_max+1][Kpad] r_k^lambda
+    double *d_rm = nullptr;    // [lambda_max+1][Kpad] r_k^-(lambda+1)
+    double *d_rk = nullptr;    // [Kpad] r_k (0 in the padding)
+    GemmTile *d_tiles = nullptr;
+    double *d_gl_rho = nullptr, *d_gl_phi = nullptr, *d_gl_zq = nullptr, *d_gl_zh = nullptr;  // GL x,w on [-1,1]: [2][n]
+    int    *d_status = nullptr; // [4] device status word (0 ok; 1 zero pivot; 2 |S_PT| >= 1), position index
+    char *arena = nullptr; size_t arena_bytes = 0;
+    // timing
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    std::vector<cudaEvent_t> ev_pool;
+    struct Span { int fam; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+    size_t ev_used = 0;
+    double last_ms[WP_NFAM] = {0};
+    long long last_launches[WP_NFAM] = {0};
+    long long launches[WP_NFAM] = {0};
+    long long groups[WP_NFAM] = {0};
+    int cur_fam = 0; bool cur_sampled = false;
+};
+
+// timing helpers (api.cu)
+void wp_span_begin(wpccc_basis *B, int fam, cudaStream_t s);
+void wp_span_end(wpccc_basis *B, cudaStream_t s, int n_launches);
+void wp_timing_reset(wpccc_basis *B);
+
+// ---- direct.cu ----
+// F[p][off_c + e] for all entries of all centres; R = |R_p|.
+int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s);
+// Real direct blocks without time phase: Dre[p][N_c][N_c] = -charge * sum_lambda sgn^lambda G P_lambda^mu(cos) F.
+int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, const double *d_F, int ldF,
+                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s);
+
+// ---- transfer.cu ----
+size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk);
+int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes);
+// Lab-frame S_PT -> d_K [p][N_P][N_T]; H_PT -> d_H rows N_T.., cols 0..; H_TP -> d_H rows 0.., cols N_T..  (no time phases).
+// `chunk` positions are processed per launch group (node tables of a chunk should stay L2-resident).
+int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
+                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s);
+int wp_transfer_default_chunk(const wpccc_basis *B);
+
+// ---- sweep.cu ----
+int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_LU, int *d_piv, cudaStream_t s);
+
+// ---- device helpers ----
+__host__ __device__ inline int lm_index(int l, int m) { return l * l + l + m; }

@@ -1,0 +1,249 @@
+// Direct (one-centre) couplings: eq. (6)-(7) of the paper.
+//
+// a2  radial contraction  F^c_lambda(a',a;R_p) = sum_k V_lambda(r_k,R_p) * PP[(a',a)][k],
+//     PP[(a',a)][k] = w_k u_a'(r_k) u_a(r_k),  V_lambda(r,R) = min(r,R)^lambda / max(r,R)^(lambda+1)
+//     as a grouped FP64 tensor-core GEMM (mma.sync m8n8k4 = SASS DMMA.8x8x4): one group per multipole lambda,
+//     M = positions, N = pairs allowed for lambda, K = radial grid.  The M operand V is generated on the fly
+//     from the r^lambda / r^-(lambda+1) tables; the N operand streams from the pair-product matrix in HBM/L2
+//     with cp.async double buffering.
+// a3  assembly  D_{alpha' alpha} = -Z sum_lambda (+-1)^lambda G^lambda_{alpha' alpha} P_lambda^{m'-m}(cos Theta) F_lambda
+#include "common.cuh"
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 32, LDS_ = BK + 4;   // row stride 36 doubles: conflict-free fragment reads
+constexpr int GEMM_THREADS = 256;
+
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+struct GemmArgs {
+    const GemmTile *tiles;
+    const double *PP[2];
+    const int *ent_pair[2];
+    int lam_off[2][WP_MAX_LAMBDA + 2];
+    int cen_off[2];
+    const double *rp, *rm, *rk;
+    const double *R;
+    double *F;
+    int ldF, n_pos, Kpad;
+};
+
+// grid: (m tiles, n tiles).  256 threads = 8 warps as 2 (M) x 4 (N); warp tile 64 x 32 -> 32 DMMA per k4 step.
+__global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs a) {
+    extern __shared__ __align__(16) double smem[];
+    double *As = smem;                         // [2][BM][LDS_]
+    double *Bs = smem + 2 * BM * LDS_;         // [2][BN][LDS_]
+    __shared__ double sR[BM], sRp[BM], sRm[BM];
+    __shared__ int sPair[BN];
+
+    const GemmTile t = a.tiles[blockIdx.y];
+    const int m0 = blockIdx.x * BM;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lam = t.lam;
+
+    if (tid < BM) {
+        int p = m0 + tid;
+        double R = (p < a.n_pos) ? a.R[p] : 1.0;
+        double Rp = 1.0;
+        for (int i = 0; i < lam; ++i) Rp *= R;
+        sR[tid] = R; sRp[tid] = Rp; sRm[tid] = 1.0 / (Rp * R);
+    }
+    if (tid < BN) {
+        int n = t.n0 + tid;
+        sPair[tid] = (tid < t.cnt) ? a.ent_pair[t.c][a.lam_off[t.c][lam] + n] : -1;
+    }
+    __syncthreads();
+
+    const double *PP = a.PP[t.c];
+    const double *rp = a.rp + (size_t)lam * a.Kpad, *rm = a.rm + (size_t)lam * a.Kpad;
+    const int nk = a.Kpad / BK;
+
+    auto load_B = [&](int buf, int kc) {
+        double *dst = Bs + buf * BN * LDS_;
+        #pragma unroll
+        for (int j = 0; j < (BN * BK / 2) / GEMM_THREADS; ++j) {
+            int c = tid + GEMM_THREADS * j, row = c >> 4, part = c & 15;
+            int pr = sPair[row];
+            double *d = dst + row * LDS_ + part * 2;
+            if (pr >= 0) cp_async16(d, PP + (size_t)pr * a.Kpad + kc * BK + part * 2);
+            else { d[0] = 0.0; d[1] = 0.0; }
+        }
+    };
+    auto gen_A = [&](int buf, int kc) {
+        double *dst = As + buf * BM * LDS_;
+        const int k = tid & 31, r0 = tid >> 5;
+        const double rkk = a.rk[kc * BK + k], rpk = rp[kc * BK + k], rmk = rm[kc * BK + k];
+        #pragma unroll
+        for (int j = 0; j < BM / 8; ++j) {
+            int row = r0 + 8 * j;
+            dst[row * LDS_ + k] = (rkk < sR[row]) ? rpk * sRm[row] : rmk * sRp[row];
+        }
+    };
+
+    double acc[8][4][2];
+    #pragma unroll
+    for (int i = 0; i < 8; ++i)
+        #pragma unroll
+        for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+
+    const int wm = (warp >> 2) * 64, wn = (warp & 3) * 32;
+    const bool warp_active = (wn < t.cnt);
+    const int fr = lane >> 2, fk = lane & 3;
+
+    load_B(0, 0); cp_async_commit();
+    gen_A(0, 0);
+    for (int kc = 0; kc < nk; ++kc) {
+        const int buf = kc & 1;
+        if (kc + 1 < nk) { load_B(buf ^ 1, kc + 1); cp_async_commit(); gen_A(buf ^ 1, kc + 1); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        if (warp_active) {
+            const double *Ab = As + buf * BM * LDS_ + (wm + fr) * LDS_ + fk;
+            const double *Bb = Bs + buf * BN * LDS_ + (wn + fr) * LDS_ + fk;
+            #pragma unroll
+            for (int ks = 0; ks < BK / 4; ++ks) {
+                double af[8], bf[4];
+                #pragma unroll
+                for (int i = 0; i < 8; ++i) af[i] = Ab[i * 8 * LDS_ + ks * 4];
+                #pragma unroll
+                for (int j = 0; j < 4; ++j) bf[j] = Bb[j * 8 * LDS_ + ks * 4];
+                #pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    #pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            }
+        }
+        __syncthreads();
+    }
+    if (!warp_active) return;
+    const int colbase = a.cen_off[t.c] + a.lam_off[t.c][lam] + t.n0;
+    #pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        int p = m0 + wm + 8 * i + fr;
+        if (p >= a.n_pos) continue;
+        double *Frow = a.F + (size_t)p * a.ldF + colbase;
+        #pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            int n = wn + 8 * j + 2 * fk;
+            if (n < t.cnt) Frow[n] = acc[i][j][0];
+            if (n + 1 < t.cnt) Frow[n + 1] = acc[i][j][1];
+        }
+    }
+}
+
+// Associated Legendre functions P_lambda^mu(x), Condon-Shortley phase, all 0 <= lambda <= L, |mu| <= lambda,
+// into P[lambda * ldp + mu + L].  One thread; L <= WP_MAX_LAMBDA.
+__device__ void assoc_legendre_all(int L, double x, double *P, int ldp) {
+    const double s = sqrt(fmax(0.0, 1.0 - x * x));
+    double pmm = 1.0;
+    for (int m = 0; m <= L; ++m) {
+        if (m > 0) pmm = -pmm * (2 * m - 1) * s;
+        double p0 = pmm, p1 = x * (2 * m + 1) * pmm;
+        // factorial ratio (lambda-m)!/(lambda+m)! built incrementally
+        for (int lam = m; lam <= L; ++lam) {
+            double val;
+            if (lam == m) val = p0;
+            else if (lam == m + 1) val = p1;
+            else { val = ((2 * lam - 1) * x * p1 - (lam + m - 1) * p0) / (lam - m); p0 = p1; p1 = val; }
+            P[lam * ldp + m + L] = val;
+            if (m > 0) {
+                double ratio = 1.0;                      // (lam-m)!/(lam+m)!
+                for (int q = lam - m + 1; q <= lam + m; ++q) ratio /= q;
+                P[lam * ldp - m + L] = ((m & 1) ? -ratio : ratio) * val;
+            }
+        }
+    }
+}
+
+struct AsmArgs {
+    const double *G; const int *ent_lookup; const int *st_rad, *st_l, *st_m;
+    const double *cosT; const double *F; double *out;
+    int n_rad, N, Lc, lambda_max, ldF, f_off, ld_out, complex_out;
+    long long pos_stride;
+    double charge; int alt_sign;
+};
+
+// grid: (n_pos, ceil(N*N/256)).  out[p*pos_stride + i*ld_out + j] (real, or complex with zero imaginary part).
+__global__ void __launch_bounds__(256) k_direct_assemble(const AsmArgs a) {
+    __shared__ double sP[(WP_MAX_LAMBDA + 1) * (2 * WP_MAX_LAMBDA + 1)];
+    const int p = blockIdx.x, L = a.lambda_max, ldp = 2 * L + 1;
+    if (threadIdx.x == 0) assoc_legendre_all(L, a.cosT[p], sP, ldp);
+    __syncthreads();
+    const int idx = blockIdx.y * blockDim.x + threadIdx.x;
+    if (idx >= a.N * a.N) return;
+    const int i = idx / a.N, j = idx % a.N;
+    const int ap = a.st_rad[i], lp = a.st_l[i], mp = a.st_m[i];
+    const int aa = a.st_rad[j], l = a.st_l[j], m = a.st_m[j];
+    const int mu = mp - m, nlm = (a.Lc + 1) * (a.Lc + 1);
+    const int alo = min(ap, aa), ahi = max(ap, aa);
+    const double *Gp = a.G + ((size_t)lm_index(lp, mp) * nlm + lm_index(l, m)) * (L + 1);
+    const double *Fp = a.F + (size_t)p * a.ldF + a.f_off;
+    double acc = 0.0;
+    int lam0 = abs(lp - l);
+    for (int lam = lam0; lam <= min(lp + l, L); lam += 2) {
+        if (abs(mu) > lam) continue;
+        int e = a.ent_lookup[((size_t)lam * a.n_rad + alo) * a.n_rad + ahi];
+        double term = Gp[lam] * sP[lam * ldp + mu + L] * Fp[e];
+        acc += (a.alt_sign && (lam & 1)) ? -term : term;
+    }
+    const double val = -a.charge * acc;
+    const size_t o = (size_t)p * a.pos_stride + (size_t)i * a.ld_out + j;
+    if (a.complex_out) { a.out[2 * o] = val; a.out[2 * o + 1] = 0.0; }
+    else a.out[o] = val;
+}
+
+}  // namespace
+
+int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s) {
+    if (n_pos <= 0) return 0;
+    GemmArgs a{};
+    a.tiles = B->d_tiles;
+    int off = 0;
+    for (int c = 0; c < B->n_centres; ++c) {
+        a.PP[c] = B->c[c].d_PP; a.ent_pair[c] = B->c[c].d_ent_pair;
+        for (int lam = 0; lam <= B->lambda_max + 1; ++lam) a.lam_off[c][lam] = B->c[c].lam_off[lam];
+        a.cen_off[c] = off; off += B->c[c].E;
+    }
+    a.rp = B->d_rp; a.rm = B->d_rm; a.rk = B->d_rk; a.R = d_R; a.F = d_F; a.ldF = ldF; a.n_pos = n_pos; a.Kpad = B->Kpad;
+    const size_t smem = (size_t)2 * (BM + BN) * LDS_ * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        WP_CUDA(cudaFuncSetAttribute(k_direct_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    dim3 grid((n_pos + BM - 1) / BM, (unsigned)B->tiles.size());
+    wp_span_begin(B, FAM_GEMM, s);
+    k_direct_gemm<<<grid, GEMM_THREADS, smem, s>>>(a);
+    wp_span_end(B, s, 1);
+    WP_CUDA(cudaGetLastError());
+    return 0;
+}
+
+int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, const double *d_F, int ldF,
+                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s) {
+    if (n_pos <= 0) return 0;
+    const CentreTab &C = B->c[c];
+    AsmArgs a{};
+    a.G = C.d_G; a.ent_lookup = C.d_ent_lookup; a.st_rad = C.d_st_rad; a.st_l = C.d_st_l; a.st_m = C.d_st_m;
+    a.cosT = d_cos; a.F = d_F; a.out = d_out;
+    a.n_rad = C.n_rad; a.N = C.n_states; a.Lc = C.l_max; a.lambda_max = B->lambda_max; a.ldF = ldF;
+    a.f_off = (c == 0) ? 0 : B->c[0].E; a.ld_out = ld_out; a.complex_out = complex_out; a.pos_stride = pos_stride;
+    // eq. (6): target-centred states see the projectile charge; projectile-centred states see Z_T with (-1)^lambda (A15)
+    a.charge = (c == 0) ? B->Z_proj : B->c[0].Z;
+    a.alt_sign = (c == 1);
+    dim3 grid(n_pos, (C.n_states * C.n_states + 255) / 256);
+    wp_span_begin(B, FAM_DASM, s);
+    k_direct_assemble<<<grid, 256, 0, s>>>(a);
+    wp_span_end(B, s, 1);
+    WP_CUDA(cudaGetLastError());
+    return 0;
+}

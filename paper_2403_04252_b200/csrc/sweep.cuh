@@ -1,0 +1,35 @@
+// a8: RK4 sweep kernels (Algorithm 1) -- declarations shared by api.cu and sweep.cu.
+#pragma once
+#include "common.cuh"
+
+// One sweep unit = up to nv trajectories that share the impact parameter b (hence the same matrices).
+struct SweepUnit { int group; int n; int traj[4]; };
+constexpr int SWEEP_NV = 4;
+
+struct Sweep1Args {          // one-centre: S = I, H = D^T (eq. (5))
+    const SweepUnit *units;
+    const double *D;         // [group][n_idx][N][N] real D^T without time phase
+    const int *st_rad; const double *eps;   // per state radial index, per radial energy
+    const double *v;         // [n_traj]
+    double *C;               // [n_traj][N] complex amplitudes (in/out)
+    double *drift;           // [n_traj] running max |sum|c|^2 - 1| (in/out) or nullptr
+    int N, n_rad, n_idx;     // n_idx = half-step positions in this window (2 * steps + 1)
+    int steps;               // RK4 steps in this window
+    long long i0;            // global half-step index of the window's first position
+    double z_min, h;         // z_i = z_min + 0.5 * i * h
+};
+int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s);
+
+struct Sweep2Args {          // two-centre: S = [[I, K^H], [K, I]], H full (eq. (1)-(4))
+    const double *H;         // [traj][n_idx][N][N] complex, no time phase
+    const double *K;         // [traj][n_idx][NP][NT] complex S_PT, no time phase
+    const double *LU;        // [traj][n_idx][NP][NP] complex LU factors of I - K K^H
+    const int *piv;          // [traj][n_idx][NP]
+    const int *st_rad_T, *st_rad_P; const double *eps_T, *eps_P;
+    const double *v;
+    double *C; double *drift;
+    int NT, NP, n_idx, steps;
+    long long i0;
+    double z_min, h;
+};
+int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStream_t s);

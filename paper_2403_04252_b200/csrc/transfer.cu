@@ -1,0 +1,617 @@
+// Two-centre overlap and electron-transfer elements: eq. (8)-(9) structure of the paper in the
+// body-frame cylindrical Gauss-Legendre form fixed by BASELINE.json configs[1], [3] (A1, A4, A5, A10).
+//
+// Per projectile position (b, z, v), with R = |R|, Theta = angle(R, v):
+//   body-frame integrals over the (rho', z') product nodes with the discrete azimuthal sum Phi_Delta folded in
+//     Sb [(b,q'),(a,q)] = sum_{i,k} W_ik e^{-i v cosTh (z'_k - R/2)} Phi_{q-q'}(v sinTh rho'_i) B_{bq'}(i,k) A_{aq}(i,k)
+//     Hb [(b,q'),(a,q)] = same with A -> Ah = -(Z_P/r_P) A + Ag                       (H_PT)
+//     Tb [(b,q'),(a,q)] = same with B -> Bh = -(Z_T/r_T) B + Bg;  H_TP^body = conj(Tb)^T
+//   A_{aq} = u_a(r_T)/r_T Theta~_{l_a q}(cos th'_T),  B_{bq'} = u_b(r_P)/r_P Theta~_{l_b q'}(cos th'_P),
+//   radial functions by five-point Lagrange interpolation on the r-grid.
+//   Then the Wigner rotation of eq. (8):  X_lab = d(Theta) X_body d(Theta)^T per (l_b, l_a) block.
+//
+// What this file does differently from a literal evaluation:
+//   * the weight separates, W Phi e^{..} = [w_rho rho Phi_Delta(i)] [w_z e^{..}(k)]: the z'-sum is one uniform
+//     complex-weighted GEMM per ring i (FP64 DMMA), the Delta-dependent ring weight is applied to its result;
+//   * Theta~_{l,-q} = (-1)^q Theta~_{lq} and Phi_{-Delta} = Phi_Delta (the phi' nodes are symmetric about pi), so
+//     only q, q' >= 0 columns are tabulated and contracted; the two families Phi_{|q-q'|} and Phi_{q+q'} of ring
+//     weights rebuild all sign combinations;
+//   * Phi^+_{-Delta} = conj(Phi^-_Delta) and the axial phases are conjugate, so H_TP shares the weights of S_PT.
+#include "common.cuh"
+
+namespace {
+
+struct cplx { double x, y; };
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
+
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+constexpr int MAXD = 2 * WP_MAX_L;          // largest Delta
+constexpr int NLQ = (WP_MAX_L + 1) * (WP_MAX_L + 2) / 2;
+__host__ __device__ inline int lq_index(int l, int q) { return l * (l + 1) / 2 + q; }
+
+__constant__ double c_fact[2 * WP_MAX_L + 2];
+__constant__ double c_thnorm[NLQ];          // sqrt((2l+1)/2 (l-q)!/(l+q)!)
+
+// ------------------------------------------------------------------------------------------------ per-position tables
+struct PosTabs {      // layout of the small per-position table block (doubles), filled by k_tpos
+    int n_rho, n_z, n_phi, dmax;
+    __host__ __device__ int off_zq() const { return 0; }                       // z'_k                 [n_z]
+    __host__ __device__ int off_ck() const { return n_z; }                     // w_z e^{-i v cosTh (z'-R/2)}  [n_z][2]
+    __host__ __device__ int off_rho() const { return 3 * n_z; }                // rho'_i               [n_rho]
+    __host__ __device__ int off_rw() const { return 3 * n_z + n_rho; }         // w_rho rho Phi_d(i)   [dmax+1][n_rho][2]
+    __host__ __device__ int size() const { return (3 * n_z + n_rho + 2 * (dmax + 1) * n_rho + 3) & ~3; }
+};
+
+struct TposArgs {
+    PosTabs L; const double *R, *cosT, *sinT, *v; const double *gl_rho, *gl_phi, *gl_zq, *gl_zh;
+    double rho_max, z_pad; int phi_rule; double *out;
+};
+
+// grid = positions, block = 128
+__global__ void __launch_bounds__(128) k_tpos(const TposArgs a) {
+    const int p = blockIdx.x, tid = threadIdx.x;
+    const PosTabs &L = a.L;
+    double *o = a.out + (size_t)p * L.size();
+    const double R = a.R[p], cT = a.cosT[p], sT = a.sinT[p], v = a.v[p];
+    const int nq = L.n_z / 4, nh = L.n_z / 2;
+    for (int k = tid; k < L.n_z; k += blockDim.x) {
+        double lo, hi, x, w;
+        if (k < nq) { lo = -a.z_pad; hi = 0.0; x = a.gl_zq[k]; w = a.gl_zq[nq + k]; }
+        else if (k < nq + nh) { lo = 0.0; hi = R; x = a.gl_zh[k - nq]; w = a.gl_zh[nh + k - nq]; }
+        else { lo = R; hi = __dadd_rn(R, a.z_pad); x = a.gl_zq[k - nq - nh]; w = a.gl_zq[nq + k - nq - nh]; }
+        const double half = __dmul_rn(0.5, __dsub_rn(hi, lo)), mid = __dmul_rn(0.5, __dadd_rn(hi, lo));
+        const double zk = __dadd_rn(__dmul_rn(half, x), mid), wz = __dmul_rn(half, w);
+        double sn, cs; sincos(-(v * cT) * (zk - 0.5 * R), &sn, &cs);
+        o[L.off_zq() + k] = zk;
+        o[L.off_ck() + 2 * k] = wz * cs; o[L.off_ck() + 2 * k + 1] = wz * sn;
+    }
+    const double twopi = 6.283185307179586476925286766559;
+    for (int i = tid; i < L.n_rho; i += blockDim.x) {
+        const double half = __dmul_rn(0.5, a.rho_max);
+        const double rho = __dadd_rn(__dmul_rn(half, a.gl_rho[i]), half), wr = __dmul_rn(__dmul_rn(half, a.gl_rho[L.n_rho + i]), rho);
+        o[L.off_rho() + i] = rho;
+        const double x = (v * sT) * rho;
+        double sr[MAXD + 1], si[MAXD + 1];
+        for (int d = 0; d <= L.dmax; ++d) { sr[d] = 0.0; si[d] = 0.0; }
+        const int nphi = a.phi_rule ? 512 : L.n_phi;
+        for (int j = 0; j < nphi; ++j) {
+            double phi, wj;
+            if (a.phi_rule) { phi = twopi * (double)j / 512.0; wj = twopi / 512.0; }
+            else { phi = __dadd_rn(__dmul_rn(0.5 * twopi, a.gl_phi[j]), 0.5 * twopi); wj = __dmul_rn(0.5 * twopi, a.gl_phi[L.n_phi + j]); }
+            double s1, c1; sincos(phi, &s1, &c1);
+            double sx, cx; sincos(x * c1, &sx, &cx);          // e^{+i x cos phi}
+            for (int d = 0; d <= L.dmax; ++d) {
+                double sd, cd; sincos((double)d * phi, &sd, &cd);
+                sr[d] += wj * (cd * cx - sd * sx); si[d] += wj * (cd * sx + sd * cx);
+            }
+        }
+        for (int d = 0; d <= L.dmax; ++d) {
+            o[L.off_rw() + 2 * (d * L.n_rho + i)] = wr * sr[d] / twopi;
+            o[L.off_rw() + 2 * (d * L.n_rho + i) + 1] = wr * si[d] / twopi;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ node tables (a4)
+// Table of one side for one position, fragment-major for m8n8k4:  T[tile][ring][kc][c8][32] with
+//   column = tile*64 + c8*8 + lane/4,  z' node k = kc*4 + lane%4.
+// Columns: [X (nqc, padded to nq8) | Xh (nq8)], X = A (side 0, centre T) or B (side 1, centre P).
+struct TtabArgs {
+    PosTabs L; const double *pos;            // per-position tables
+    const double *R;
+    const double *Ut[2]; const int *lrad[2]; int n_rad[2], nf_pad[2], nq8[2], ntile[2];
+    const int *colidx[2];                    // [n_rad][WP_MAX_L+1] column of (a, q) or -1
+    double Zother[2];                        // side 0 (T functions): Z_P;  side 1: Z_T
+    double h; int Nr, KC;                    // KC: z' nodes per CTA (multiple of 4)
+    double *out[2]; size_t pos_stride[2];    // doubles per position for each side
+    int lmax[2];
+};
+
+// grid = (ring * n_kchunks, side, position), block = 256, dynamic smem.
+__global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
+    extern __shared__ __align__(16) double sm[];
+    const int side = blockIdx.y, p = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nkch = a.L.n_z / a.KC, ring = blockIdx.x / nkch, k0 = (blockIdx.x % nkch) * a.KC, KC = a.KC;
+    const int ld = KC + 2, ncols = a.ntile[side] * 64, nq8 = a.nq8[side], lmax = a.lmax[side];
+    const int nlq = (lmax + 1) * (lmax + 2) / 2;
+    double *tile = sm;                                   // [ncols][ld]
+    double *sLag = tile + (size_t)ncols * ld;            // [5][KC]
+    double *sRinv = sLag + 5 * KC, *sPot = sRinv + KC;   // [KC] 1/r_side, -Z_other/r_other
+    double *sTh = sPot + KC;                             // [nlq][KC]
+    int *sJ = reinterpret_cast<int *>(sTh + (size_t)nlq * KC);   // [KC] stencil centre, -1 beyond r_max
+    const double *pt = a.pos + (size_t)p * a.L.size();
+    const double R = a.R[p];
+
+    for (int i = tid; i < ncols * ld; i += blockDim.x) tile[i] = 0.0;
+    if (tid < KC) {
+        const double rho = pt[a.L.off_rho() + ring], zk = pt[a.L.off_zq() + k0 + tid];
+        const double zP = __dsub_rn(zk, R);
+        const double rT = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zk, zk)));
+        const double rP = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zP, zP)));
+        const double rs = side ? rP : rT, ro = side ? rT : rP;
+        const double c = (side ? zP : zk) / rs;
+        int j = (int)floor(rs / a.h + 0.5);
+        j = max(2, min(a.Nr - 2, j));
+        const double t = rs / a.h - (double)j;
+        // Lagrange basis on offsets -2..2
+        sLag[0 * KC + tid] = (t + 1.0) * t * (t - 1.0) * (t - 2.0) / 24.0;
+        sLag[1 * KC + tid] = -(t + 2.0) * t * (t - 1.0) * (t - 2.0) / 6.0;
+        sLag[2 * KC + tid] = (t + 2.0) * (t + 1.0) * (t - 1.0) * (t - 2.0) / 4.0;
+        sLag[3 * KC + tid] = -(t + 2.0) * (t + 1.0) * t * (t - 2.0) / 6.0;
+        sLag[4 * KC + tid] = (t + 2.0) * (t + 1.0) * t * (t - 1.0) / 24.0;
+        sJ[tid] = (rs > a.Nr * a.h) ? -1 : j;
+        sRinv[tid] = 1.0 / rs;
+        sPot[tid] = -a.Zother[side] / ro;
+        // Theta~_{lq}(c), q >= 0
+        const double s = sqrt(fmax(0.0, __dsub_rn(1.0, __dmul_rn(c, c))));
+        double pmm = 1.0;
+        for (int q = 0; q <= lmax; ++q) {
+            if (q > 0) pmm = -pmm * (2 * q - 1) * s;
+            double p0 = pmm, p1 = c * (2 * q + 1) * pmm;
+            for (int l = q; l <= lmax; ++l) {
+                double val;
+                if (l == q) val = p0;
+                else if (l == q + 1) val = p1;
+                else { val = ((2 * l - 1) * c * p1 - (l + q - 1) * p0) / (l - q); p0 = p1; p1 = val; }
+                sTh[lq_index(l, q) * KC + tid] = c_thnorm[lq_index(l, q)] * val;
+            }
+        }
+    }
+    __syncthreads();
+    const double *Ut = a.Ut[side];
+    const int nr = a.n_rad[side], nf = a.nf_pad[side];
+    for (int n = warp; n < KC; n += 8) {
+        const int j = sJ[n];
+        if (j < 0) continue;
+        const double L0 = sLag[n], L1 = sLag[KC + n], L2 = sLag[2 * KC + n], L3 = sLag[3 * KC + n], L4 = sLag[4 * KC + n];
+        const double rinv = sRinv[n], pot = sPot[n];
+        const double *row = Ut + (size_t)(j - 2) * nf;
+        for (int aa = lane; aa < nr; aa += 32) {
+            double fu = L0 * row[aa]; double fg = L0 * row[nr + aa];
+            fu += L1 * row[nf + aa]; fg += L1 * row[nf + nr + aa];
+            fu += L2 * row[2 * nf + aa]; fg += L2 * row[2 * nf + nr + aa];
+            fu += L3 * row[3 * nf + aa]; fg += L3 * row[3 * nf + nr + aa];
+            fu += L4 * row[4 * nf + aa]; fg += L4 * row[4 * nf + nr + aa];
+            fu *= rinv; fg *= rinv;
+            const int l = a.lrad[side][aa];
+            for (int q = 0; q <= l; ++q) {
+                const int col = a.colidx[side][aa * (WP_MAX_L + 1) + q];
+                const double th = sTh[lq_index(l, q) * KC + n];
+                const double X = fu * th, Xg = fg * th;
+                tile[(size_t)col * ld + n] = X;
+                tile[(size_t)(nq8 + col) * ld + n] = pot * X + Xg;
+            }
+        }
+    }
+    __syncthreads();
+    // coalesced write-out in fragment order
+    double *out = a.out[side] + (size_t)p * a.pos_stride[side];
+    const int nkc = a.L.n_z / 4, kcs = KC / 4;
+    for (int t = 0; t < a.ntile[side]; ++t) {
+        double *dst = out + (((size_t)t * a.L.n_rho + ring) * nkc + k0 / 4) * 256;
+        for (int e = tid; e < kcs * 256; e += blockDim.x) {
+            const int kc = e >> 8, c8 = (e >> 5) & 7, ln = e & 31;
+            dst[e] = tile[(size_t)(t * 64 + c8 * 8 + (ln >> 2)) * ld + kc * 4 + (ln & 3)];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ contraction (a5)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
+        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+constexpr int TC_THREADS = 256, TC_STAGES = 3, TC_KCS = 16;     // stage = 16 k4-groups = 64 z' nodes per operand
+constexpr int TC_STAGE_DOUBLES = TC_KCS * 256;                  // per operand
+
+struct TconArgs {
+    PosTabs L; const double *pos;
+    const double *tabT, *tabP; size_t strideT, strideP;         // node tables (doubles per position)
+    int nq8T, nq8P, ntT, ntP;                                    // padded half widths, number of 64-tiles
+    const int *qT, *qP;                                          // [nq8] q of column (q >= 0), -1 padding
+    const int2 *tiles; int n_tiles;                              // (row tile over [B|Bh], col tile over [A|Ah])
+    int n_split;                                                 // ring splits
+    double *part;                                                // [p][split][fam 2][prod 3][nq8P][nq8T] complex
+};
+
+// grid = (tile, ring split, position); block = 256 = 8 warps as 4 (rows) x 2 (cols); warp tile 16 x 32 complex.
+__global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
+    extern __shared__ __align__(128) double sm[];
+    double *sA = sm;                                          // [STAGES][TC_STAGE_DOUBLES]  A-side (mma "B" operand)
+    double *sB = sA + TC_STAGES * TC_STAGE_DOUBLES;           // [STAGES][TC_STAGE_DOUBLES]  B-side (mma "A" operand)
+    double *sCk = sB + TC_STAGES * TC_STAGE_DOUBLES;          // [n_z][2]
+    double *sRw = sCk + 2 * a.L.n_z;                          // [dmax+1][n_rho][2]
+    __shared__ __align__(8) unsigned long long bar[TC_STAGES];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int p = blockIdx.z, split = blockIdx.y;
+    const int2 tl = a.tiles[blockIdx.x];
+    const int rt = tl.x, ct = tl.y;
+    const double *pt = a.pos + (size_t)p * a.L.size();
+    const int n_rho = a.L.n_rho, n_z = a.L.n_z, nkc = n_z / 4;
+    const int ring0 = (int)((long long)n_rho * split / a.n_split), ring1 = (int)((long long)n_rho * (split + 1) / a.n_split);
+    const int spr = (nkc + TC_KCS - 1) / TC_KCS;              // stages per ring
+    const int n_st = (ring1 - ring0) * spr;
+
+    for (int i = tid; i < 2 * n_z; i += TC_THREADS) sCk[i] = pt[a.L.off_ck() + i];
+    for (int i = tid; i < 2 * (a.L.dmax + 1) * n_rho; i += TC_THREADS) sRw[i] = pt[a.L.off_rw() + i];
+    if (tid == 0) { for (int s = 0; s < TC_STAGES; ++s) mbar_init(&bar[s], 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::); }
+    __syncthreads();
+
+    const double *gA = a.tabT + (size_t)p * a.strideT + (size_t)ct * n_rho * nkc * 256;
+    const double *gB = a.tabP + (size_t)p * a.strideP + (size_t)rt * n_rho * nkc * 256;
+    auto issue = [&](int st) {
+        const int ring = ring0 + st / spr, kc0 = (st % spr) * TC_KCS, nk = min(TC_KCS, nkc - kc0), buf = st % TC_STAGES;
+        const unsigned bytes = (unsigned)nk * 256 * 8;
+        mbar_expect_tx(&bar[buf], 2 * bytes);
+        tma_bulk_g2s(sA + buf * TC_STAGE_DOUBLES, gA + ((size_t)ring * nkc + kc0) * 256, bytes, &bar[buf]);
+        tma_bulk_g2s(sB + buf * TC_STAGE_DOUBLES, gB + ((size_t)ring * nkc + kc0) * 256, bytes, &bar[buf]);
+    };
+    if (tid == 0) for (int st = 0; st < min(TC_STAGES, n_st); ++st) issue(st);
+
+    const int wr = warp >> 1, wc = warp & 1;                  // warp rows 16*wr.., cols 32*wc..
+    const int fr = lane >> 2, fk = lane & 3;
+    // per-thread output bookkeeping: element (i, j, e): row = rt*64 + 16 wr + 8 i + fr, col = ct*64 + 32 wc + 8 j + 2 fk + e
+    // needed sub-tiles: not (Bh x Ah)
+    bool need[2][4];
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int r8 = rt * 64 + 16 * wr + 8 * i, c8 = ct * 64 + 32 * wc + 8 * j;
+            need[i][j] = (r8 < 2 * a.nq8P) && (c8 < 2 * a.nq8T) && !(r8 >= a.nq8P && c8 >= a.nq8T);
+        }
+    bool any_need = false;
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < 4; ++j) any_need |= need[i][j];
+
+    double Cre[2][4][2], Cim[2][4][2], Mre[2][4][2], Mim[2][4][2], Pre[2][4][2], Pim[2][4][2];
+    int dm[2][4][2], dp[2][4][2];
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < 4; ++j)
+            #pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                Cre[i][j][e] = Cim[i][j][e] = Mre[i][j][e] = Mim[i][j][e] = Pre[i][j][e] = Pim[i][j][e] = 0.0;
+                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 32 * wc + 8 * j + 2 * fk + e;
+                int qp = -1, qq = -1;
+                if (gr < 2 * a.nq8P) qp = a.qP[gr % a.nq8P];
+                if (gc < 2 * a.nq8T) qq = a.qT[gc % a.nq8T];
+                const bool ok = need[i][j] && qp >= 0 && qq >= 0;
+                dm[i][j][e] = ok ? abs(qq - qp) : -1;
+                dp[i][j][e] = (ok && qp > 0 && qq > 0) ? qq + qp : -1;
+            }
+
+    for (int st = 0; st < n_st; ++st) {
+        const int buf = st % TC_STAGES, ring = ring0 + st / spr, kc0 = (st % spr) * TC_KCS, nk = min(TC_KCS, nkc - kc0);
+        mbar_wait(&bar[buf], (st / TC_STAGES) & 1);
+        if (any_need) {
+            const double *Ab = sA + buf * TC_STAGE_DOUBLES + (4 * wc) * 32 + lane;
+            const double *Bb = sB + buf * TC_STAGE_DOUBLES + (2 * wr) * 32 + lane;
+            const double *ck = sCk + 2 * (kc0 * 4 + fk);
+            #pragma unroll 4
+            for (int kc = 0; kc < nk; ++kc) {
+                const double cr = ck[8 * kc], ci = ck[8 * kc + 1];
+                double af[4], br[2], bi[2];
+                #pragma unroll
+                for (int j = 0; j < 4; ++j) af[j] = Ab[kc * 256 + j * 32];
+                #pragma unroll
+                for (int i = 0; i < 2; ++i) { const double b = Bb[kc * 256 + i * 32]; br[i] = b * cr; bi[i] = b * ci; }
+                #pragma unroll
+                for (int i = 0; i < 2; ++i)
+                    #pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (need[i][j]) {
+                            dmma884(Cre[i][j][0], Cre[i][j][1], br[i], af[j]);
+                            dmma884(Cim[i][j][0], Cim[i][j][1], bi[i], af[j]);
+                        }
+            }
+        }
+        __syncthreads();                                   // everyone is done with this buffer
+        if (tid == 0 && st + TC_STAGES < n_st) issue(st + TC_STAGES);
+        if ((st % spr) == spr - 1) {
+            // ring epilogue: acc(-) += w_rho rho Phi_{|q-q'|}(ring) C,  acc(+) += w_rho rho Phi_{q+q'}(ring) C
+            #pragma unroll
+            for (int i = 0; i < 2; ++i)
+                #pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    #pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const double cr = Cre[i][j][e], ci = Cim[i][j][e];
+                        if (dm[i][j][e] >= 0) {
+                            const double wr_ = sRw[2 * (dm[i][j][e] * n_rho + ring)], wi_ = sRw[2 * (dm[i][j][e] * n_rho + ring) + 1];
+                            Mre[i][j][e] += wr_ * cr - wi_ * ci; Mim[i][j][e] += wr_ * ci + wi_ * cr;
+                        }
+                        if (dp[i][j][e] >= 0) {
+                            const double wr_ = sRw[2 * (dp[i][j][e] * n_rho + ring)], wi_ = sRw[2 * (dp[i][j][e] * n_rho + ring) + 1];
+                            Pre[i][j][e] += wr_ * cr - wi_ * ci; Pim[i][j][e] += wr_ * ci + wi_ * cr;
+                        }
+                        Cre[i][j][e] = 0.0; Cim[i][j][e] = 0.0;
+                    }
+        }
+    }
+    // write partial sums
+    const size_t blk = (size_t)a.nq8P * a.nq8T;
+    double *o = a.part + ((size_t)p * a.n_split + split) * 6 * blk * 2;
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < 4; ++j)
+            #pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                if (dm[i][j][e] < 0) continue;
+                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 32 * wc + 8 * j + 2 * fk + e;
+                const int hr = gr / a.nq8P, ir = gr % a.nq8P, hc = gc / a.nq8T, ic = gc % a.nq8T;
+                const int prod = hr ? 2 : (hc ? 1 : 0);
+                const size_t idx = ((size_t)prod * blk + (size_t)ir * a.nq8T + ic) * 2;
+                o[idx] = Mre[i][j][e]; o[idx + 1] = Mim[i][j][e];
+                double *op = o + 3 * blk * 2;
+                op[idx] = Pre[i][j][e]; op[idx + 1] = Pim[i][j][e];
+            }
+}
+
+// ------------------------------------------------------------------------------------------------ rotation (a6)
+struct TrotArgs {
+    const double *part; int n_split; int nq8T, nq8P;
+    const double *theta;                     // [p] Theta = angle between R and v
+    const int *lT, *lP, *firstT, *firstP;    // per radial function: l, first state index
+    const int *colT, *colP;                  // [n_rad][WP_MAX_L+1] column of (a, |q|)
+    int nradT, nradP, NT, NP, lmax;
+    double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex
+};
+
+// Wigner d^l_{m' m}(beta) = <l m'| e^{-i beta J_y} |l m>, Wigner's sum formula.
+__device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
+    double tot = 0.0;
+    const double num = sqrt(c_fact[l + m] * c_fact[l - m] * c_fact[l + mp] * c_fact[l - mp]);
+    for (int k = max(0, m - mp); k <= min(l + m, l - mp); ++k) {
+        const double den = c_fact[l + m - k] * c_fact[k] * c_fact[l - k - mp] * c_fact[k - m + mp];
+        double term = num / den * pow(cb, 2 * l - 2 * k + m - mp) * pow(sb, 2 * k - m + mp);
+        tot += ((k - m + mp) & 1) ? -term : term;
+    }
+    return tot;
+}
+
+// grid = (position, ceil(nradP*nradT/128)); block 128: one thread per radial pair (b, a).
+__global__ void __launch_bounds__(128) k_trot(const TrotArgs a) {
+    __shared__ double sd[(WP_MAX_L + 1) * (2 * WP_MAX_L + 1) * (2 * WP_MAX_L + 1)];
+    const int p = blockIdx.x, tid = threadIdx.x, W = 2 * WP_MAX_L + 1;
+    {
+        double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
+        for (int e = tid; e < (a.lmax + 1) * W * W; e += blockDim.x) {
+            const int l = e / (W * W), mp = (e / W) % W - WP_MAX_L, m = e % W - WP_MAX_L;
+            sd[e] = (abs(mp) <= l && abs(m) <= l) ? wigner_d(l, mp, m, cb, sb) : 0.0;
+        }
+    }
+    __syncthreads();
+    const int pair = blockIdx.y * blockDim.x + tid;
+    if (pair >= a.nradP * a.nradT) return;
+    const int rb = pair / a.nradT, ra = pair % a.nradT;
+    const int lb = a.lP[rb], la = a.lT[ra];
+    const size_t blk = (size_t)a.nq8P * a.nq8T;
+    const int N = a.NT + a.NP;
+    const double *dB = sd + lb * W * W, *dA = sd + la * W * W;
+    for (int prod = 0; prod < 3; ++prod) {
+        // signed body-frame block X[q'][q] from the two families
+        cplx X[2 * WP_MAX_L + 1][2 * WP_MAX_L + 1];
+        for (int qp = -lb; qp <= lb; ++qp)
+            for (int q = -la; q <= la; ++q) {
+                const int aq = abs(q), aqp = abs(qp);
+                const bool same = (q >= 0) == (qp >= 0);           // family (-) when the signs agree, or one of them is 0
+                const int fam = (same || aq == 0 || aqp == 0) ? 0 : 1;
+                const size_t idx = (((size_t)fam * 3 + prod) * blk + (size_t)a.colP[rb * (WP_MAX_L + 1) + aqp] * a.nq8T + a.colT[ra * (WP_MAX_L + 1) + aq]) * 2;
+                double xr = 0.0, xi = 0.0;
+                for (int s = 0; s < a.n_split; ++s) {
+                    const double *src = a.part + ((size_t)p * a.n_split + s) * 6 * blk * 2 + idx;
+                    xr += src[0]; xi += src[1];
+                }
+                int sg = 0;
+                if (q < 0) sg += aq;
+                if (qp < 0) sg += aqp;
+                if (sg & 1) { xr = -xr; xi = -xi; }
+                X[qp + lb][q + la] = {xr, xi};
+            }
+        for (int mp = -lb; mp <= lb; ++mp)
+            for (int m = -la; m <= la; ++m) {
+                double sr = 0.0, si = 0.0;
+                for (int qp = -lb; qp <= lb; ++qp) {
+                    const double dbv = dB[(mp + WP_MAX_L) * W + qp + WP_MAX_L];
+                    double tr = 0.0, ti = 0.0;
+                    for (int q = -la; q <= la; ++q) {
+                        const double dav = dA[(m + WP_MAX_L) * W + q + WP_MAX_L];
+                        tr += dav * X[qp + lb][q + la].x; ti += dav * X[qp + lb][q + la].y;
+                    }
+                    sr += dbv * tr; si += dbv * ti;
+                }
+                const int ib = a.firstP[rb] + mp + lb, ia = a.firstT[ra] + m + la;
+                if (prod == 0) {
+                    double *o = a.K + (((size_t)p * a.NP + ib) * a.NT + ia) * 2;
+                    o[0] = sr; o[1] = si;
+                } else if (prod == 1) {
+                    double *o = a.H + (((size_t)p * N + a.NT + ib) * N + ia) * 2;       // H_PT
+                    o[0] = sr; o[1] = si;
+                } else {
+                    double *o = a.H + (((size_t)p * N + ia) * N + a.NT + ib) * 2;       // H_TP = conj(rot Tb)^T
+                    o[0] = sr; o[1] = -si;
+                }
+            }
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------- host side
+struct TransferPlan {
+    PosTabs L; int nq8[2], ntile[2]; size_t stride[2]; size_t part_per_pos; int n_split; std::vector<int2> tiles;
+    size_t per_pos_bytes() const { return ((size_t)L.size() + stride[0] + stride[1]) * 8 + part_per_pos * 8 + 64; }
+};
+
+static TransferPlan make_plan(const wpccc_basis *B, int n_split) {
+    TransferPlan P;
+    P.L.n_rho = B->quad.n_rho; P.L.n_z = B->quad.n_z; P.L.n_phi = B->quad.n_phi; P.L.dmax = B->c[0].l_max + B->c[1].l_max;
+    for (int s = 0; s < 2; ++s) {
+        P.nq8[s] = B->c[s].nqc_pad;
+        P.ntile[s] = (2 * P.nq8[s] + 63) / 64;
+        P.stride[s] = (size_t)P.ntile[s] * 64 * P.L.n_rho * P.L.n_z;
+    }
+    P.n_split = n_split;
+    P.part_per_pos = (size_t)n_split * 6 * P.nq8[0] * P.nq8[1] * 2;
+    for (int rt = 0; rt < P.ntile[1]; ++rt)
+        for (int ct = 0; ct < P.ntile[0]; ++ct)
+            if (!(rt * 64 >= P.nq8[1] && ct * 64 >= P.nq8[0])) P.tiles.push_back(make_int2(rt, ct));
+    return P;
+}
+
+static int pick_split(const wpccc_basis *B) {
+    // enough CTAs per position that a chunk of few positions (tables resident in L2) fills the 148 SMs
+    TransferPlan P = make_plan(B, 1);
+    int s = std::max(1, std::min(B->quad.n_rho, (int)(16 / std::max<size_t>(1, P.tiles.size() / 3))));
+    while (B->quad.n_rho / s < 4 && s > 1) --s;
+    return s;
+}
+
+size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk) {
+    TransferPlan P = make_plan(B, pick_split(B));
+    return P.per_pos_bytes() * (size_t)n_pos_chunk + P.tiles.size() * sizeof(int2) + 4096 +
+           2 * (size_t)(B->c[0].n_rad + B->c[1].n_rad) * (WP_MAX_L + 1) * sizeof(int) +
+           2 * (size_t)(B->c[0].nqc_pad + B->c[1].nqc_pad) * sizeof(int);
+}
+
+int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes) {
+    const size_t fixed = wp_transfer_ws_bytes(B, 0);
+    const size_t per = wp_transfer_ws_bytes(B, 1) - fixed;
+    if (ws_bytes <= fixed) return 0;
+    return (int)std::min<size_t>((ws_bytes - fixed) / per, 1 << 20);
+}
+
+int wp_transfer_default_chunk(const wpccc_basis *B) {
+    // node tables of one chunk ~ 64 MB (half of the 126 MB L2), at least enough CTAs for two waves of 148 SMs
+    TransferPlan P = make_plan(B, pick_split(B));
+    const size_t tab = (P.stride[0] + P.stride[1]) * 8;
+    int c = (int)std::max<size_t>(1, ((size_t)64 << 20) / tab);
+    const int ctas = (int)P.tiles.size() * P.n_split;
+    while (c * ctas < 296 && (size_t)c * tab < ((size_t)256 << 20)) ++c;
+    return c;
+}
+
+int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
+                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s) {
+    if (n_pos <= 0) return 0;
+    static bool consts = false;
+    if (!consts) {
+        double f[2 * WP_MAX_L + 2]; f[0] = 1.0;
+        for (int i = 1; i < 2 * WP_MAX_L + 2; ++i) f[i] = f[i - 1] * i;
+        WP_CUDA(cudaMemcpyToSymbol(c_fact, f, sizeof f));
+        double tn[NLQ];
+        for (int l = 0; l <= WP_MAX_L; ++l) for (int q = 0; q <= l; ++q) tn[lq_index(l, q)] = std::sqrt((2 * l + 1) / 2.0 * f[l - q] / f[l + q]);
+        WP_CUDA(cudaMemcpyToSymbol(c_thnorm, tn, sizeof tn));
+        consts = true;
+    }
+    const int n_split = pick_split(B);
+    TransferPlan P = make_plan(B, n_split);
+    const int max_chunk = wp_transfer_chunk_positions(B, ws_bytes);
+    if (max_chunk < 1) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small (%zu bytes)", ws_bytes);
+    chunk = std::max(1, std::min(std::min(chunk, max_chunk), n_pos));
+
+    // carve the workspace
+    char *w = (char *)ws; size_t off = 0;
+    auto take = [&](size_t bytes) { off = (off + 255) & ~(size_t)255; void *p = w + off; off += bytes; return p; };
+    double *d_pos = (double *)take((size_t)chunk * P.L.size() * 8);
+    double *d_tab[2] = {(double *)take((size_t)chunk * P.stride[0] * 8), (double *)take((size_t)chunk * P.stride[1] * 8)};
+    double *d_part = (double *)take((size_t)chunk * P.part_per_pos * 8);
+    int2 *d_tiles = (int2 *)take(P.tiles.size() * sizeof(int2));
+    int *d_colidx[2], *d_qcol[2];
+    for (int c = 0; c < 2; ++c) { d_colidx[c] = (int *)take((size_t)B->c[c].n_rad * (WP_MAX_L + 1) * 4); d_qcol[c] = (int *)take((size_t)B->c[c].nqc_pad * 4); }
+    if (off > ws_bytes) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small");
+    WP_CUDA(cudaMemcpyAsync(d_tiles, P.tiles.data(), P.tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, s));
+    std::vector<int> hcol[2], hq[2];
+    for (int c = 0; c < 2; ++c) {
+        const CentreTab &C = B->c[c];
+        hcol[c].assign((size_t)C.n_rad * (WP_MAX_L + 1), -1);
+        hq[c].assign(C.nqc_pad, -1);
+        for (int col = 0; col < C.nqc; ++col) { hcol[c][(size_t)C.col_rad[col] * (WP_MAX_L + 1) + C.col_q[col]] = col; hq[c][col] = C.col_q[col]; }
+        WP_CUDA(cudaMemcpyAsync(d_colidx[c], hcol[c].data(), hcol[c].size() * 4, cudaMemcpyHostToDevice, s));
+        WP_CUDA(cudaMemcpyAsync(d_qcol[c], hq[c].data(), hq[c].size() * 4, cudaMemcpyHostToDevice, s));
+    }
+
+    // node-table kernel configuration
+    int KC = P.L.n_z;
+    size_t tab_smem = 0;
+    const int lmx = std::max(B->c[0].l_max, B->c[1].l_max), nlq = (lmx + 1) * (lmx + 2) / 2;
+    const int maxcols = std::max(P.ntile[0], P.ntile[1]) * 64;
+    for (;; ) {
+        tab_smem = ((size_t)maxcols * (KC + 2) + (size_t)(7 + nlq) * KC) * 8 + (size_t)KC * 4 + 64;
+        if (tab_smem <= 200 * 1024 && KC <= 256) break;
+        // next smaller divisor of n_z that is a multiple of 4
+        int k2 = KC - 4;
+        while (k2 >= 4 && P.L.n_z % k2) k2 -= 4;
+        if (k2 < 4) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the node-table kernel");
+        KC = k2;
+    }
+    static size_t tab_attr = 0, con_attr = 0;
+    if (tab_smem > tab_attr) { WP_CUDA(cudaFuncSetAttribute(k_ttab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_smem)); tab_attr = tab_smem; }
+    const size_t con_smem = ((size_t)2 * TC_STAGES * TC_STAGE_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 1) * P.L.n_rho) * 8;
+    if (con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
+    if (con_smem > con_attr) { WP_CUDA(cudaFuncSetAttribute(k_tcon, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem)); con_attr = con_smem; }
+
+    const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
+    for (int p0 = 0; p0 < n_pos; p0 += chunk) {
+        const int np = std::min(chunk, n_pos - p0);
+        TposArgs ta{}; ta.L = P.L; ta.R = d_R + p0; ta.cosT = d_cos + p0; ta.sinT = d_sin + p0; ta.v = d_v + p0;
+        ta.gl_rho = B->d_gl_rho; ta.gl_phi = B->d_gl_phi; ta.gl_zq = B->d_gl_zq; ta.gl_zh = B->d_gl_zh;
+        ta.rho_max = B->quad.rho_max; ta.z_pad = B->quad.z_pad; ta.phi_rule = B->quad.phi_rule; ta.out = d_pos;
+        wp_span_begin(B, FAM_TTAB, s);
+        k_tpos<<<np, 128, 0, s>>>(ta);
+        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R + p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC;
+        for (int c = 0; c < 2; ++c) {
+            tb.Ut[c] = B->c[c].d_Ut; tb.lrad[c] = B->c[c].d_l; tb.n_rad[c] = B->c[c].n_rad; tb.nf_pad[c] = B->c[c].nf_pad;
+            tb.nq8[c] = P.nq8[c]; tb.ntile[c] = P.ntile[c]; tb.colidx[c] = d_colidx[c]; tb.out[c] = d_tab[c]; tb.pos_stride[c] = P.stride[c];
+            tb.lmax[c] = B->c[c].l_max;
+        }
+        tb.Zother[0] = B->c[1].Z; tb.Zother[1] = B->c[0].Z;
+        dim3 gt(P.L.n_rho * (P.L.n_z / KC), 2, np);
+        k_ttab<<<gt, 256, tab_smem, s>>>(tb);
+        wp_span_end(B, s, 2);
+        WP_CUDA(cudaGetLastError());
+
+        TconArgs tc{}; tc.L = P.L; tc.pos = d_pos; tc.tabT = d_tab[0]; tc.tabP = d_tab[1]; tc.strideT = P.stride[0]; tc.strideP = P.stride[1];
+        tc.nq8T = P.nq8[0]; tc.nq8P = P.nq8[1]; tc.ntT = P.ntile[0]; tc.ntP = P.ntile[1]; tc.qT = d_qcol[0]; tc.qP = d_qcol[1];
+        tc.tiles = d_tiles; tc.n_tiles = (int)P.tiles.size(); tc.n_split = n_split; tc.part = d_part;
+        dim3 gc((unsigned)P.tiles.size(), n_split, np);
+        wp_span_begin(B, FAM_TCON, s);
+        k_tcon<<<gc, TC_THREADS, con_smem, s>>>(tc);
+        wp_span_end(B, s, 1);
+        WP_CUDA(cudaGetLastError());
+
+        TrotArgs tr{}; tr.part = d_part; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta + p0;
+        tr.lT = B->c[0].d_l; tr.lP = B->c[1].d_l; tr.firstT = B->c[0].d_rad_first; tr.firstP = B->c[1].d_rad_first;
+        tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.nradT = B->c[0].n_rad; tr.nradP = B->c[1].n_rad; tr.NT = NT; tr.NP = NP;
+        tr.lmax = lmx; tr.K = d_K + (size_t)p0 * NP * NT * 2; tr.H = d_H + (size_t)p0 * N * N * 2;
+        dim3 gr(np, (tr.nradP * tr.nradT + 127) / 128);
+        wp_span_begin(B, FAM_ROT, s);
+        k_trot<<<gr, 128, 0, s>>>(tr);
+        wp_span_end(B, s, 1);
+        WP_CUDA(cudaGetLastError());
+    }
+    return 0;
+}

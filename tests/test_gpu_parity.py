@@ -1,0 +1,178 @@
+"""-m gpu: parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): matrix elements 1e-11 relative with a 1e-13 absolute floor;
+transition probabilities 1e-9 absolute."""
+import numpy as np
+import pytest
+
+from oracle import assemble, direct, observables
+from oracle import propagate as oprop
+from oracle import transfer as otr
+from wpccc_inputs import tiny_problem
+
+pytestmark = pytest.mark.gpu
+
+REL, FLOOR, PTOL = 1e-11, 1e-13, 1e-9
+
+
+def assert_elements(got, ref, what, scale=None):
+    got, ref = np.asarray(got), np.asarray(ref)
+    assert got.shape == ref.shape, (what, got.shape, ref.shape)
+    err = np.abs(got - ref)
+    tol = REL * np.abs(ref) + FLOOR
+    bad = err > tol
+    assert not bad.any(), "%s: %d of %d elements out of tolerance; worst |err| %.3e at |ref| %.3e" % (
+        what, bad.sum(), bad.size, err[bad].max(), np.abs(ref[bad][np.argmax(err[bad])]))
+
+
+POS1 = [(0.5, -0.37, 2.0), (0.5, 5.3, 2.0), (1.7, 0.0, 1.0), (4.0, -12.25, 0.7), (0.05, 0.02, 3.0), (3.0, 90.0, 1.0)]
+
+
+@pytest.fixture(scope="module")
+def one_centre(lib):
+    prob = tiny_problem(False, l_max=2, n_max=3, bins=3, k_max=2.5, Nr=437, h=0.1, lambda_max=4)   # ragged Nr (not a multiple of 32)
+    return prob, lib.setup_basis(prob)
+
+
+def test_fp64_peaks_report(lib):
+    dfma, dmma = lib.fp64_peak(0), lib.fp64_peak(1)
+    print("FP64 peak: DFMA %.2f TFLOP/s, DMMA %.2f TFLOP/s" % (dfma, dmma))
+    assert dfma > 5 and dmma > 5
+
+
+def test_direct_radial_entries_and_elements(lib, one_centre):
+    prob, basis = one_centre
+    b, z, v = map(np.array, zip(*POS1))
+    S, H, F = lib.matrix_elements(basis, b, z, v, phases=True, want_F=True)
+    S, H, F = S.cpu().numpy(), H.cpu().numpy(), F.cpu().numpy()
+    ent = basis.radial_entries(0)
+    r = prob.h * np.arange(prob.Nr + 1)
+    for p in range(len(b)):
+        R = float(np.hypot(b[p], z[p]))
+        Fo = direct.radial_F_all(prob.centres[0], prob.w, r, R, prob.lambda_max)
+        ref = np.array([Fo[lam, a1, a] for (a1, a, lam) in ent])
+        assert_elements(F[p], ref, "F at position %d" % p)
+        So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
+        assert_elements(H[p], Ho, "D^T at position %d" % p)
+        assert_elements(S[p], So, "S (identity) at position %d" % p)
+    # element-by-element definition (loops) at one position
+    Dl = direct.direct_block_loops(prob.centres[0], prob.w, r, prob.lambda_max, b[0], z[0], v[0], prob.Z_proj, False)
+    assert_elements(H[0], Dl, "D^T vs loop definition")
+
+
+def test_direct_many_positions_span_tiles(lib, one_centre):
+    """300 positions (3 M-tiles with a ragged tail); sampled rows against the oracle, all rows for symmetry."""
+    prob, basis = one_centre
+    rng = np.random.default_rng(7)
+    n = 300
+    b, z, v = rng.uniform(0.05, 6.0, n), rng.uniform(-30.0, 30.0, n), np.full(n, 1.3)
+    _, H, F = lib.matrix_elements(basis, b, z, v, phases=False, want_S=False, want_F=True)
+    H, F = H.cpu().numpy(), F.cpu().numpy()
+    assert np.abs(H.imag).max() == 0.0 and np.abs(H - H.transpose(0, 2, 1)).max() < 1e-15
+    ent = basis.radial_entries(0)
+    r = prob.h * np.arange(prob.Nr + 1)
+    for p in (0, 127, 128, 255, 256, 299):
+        Fo = direct.radial_F_all(prob.centres[0], prob.w, r, float(np.hypot(b[p], z[p])), prob.lambda_max)
+        assert_elements(F[p], np.array([Fo[lam, a1, a] for (a1, a, lam) in ent]), "F at position %d" % p)
+
+
+def test_one_centre_propagation_and_probabilities(lib, one_centre):
+    prob, basis = one_centre
+    b = np.array([0.6, 0.6, 2.0, 0.6, 1.1])          # repeated b: trajectories share matrices
+    v = np.array([1.0, 2.0, 2.0, 0.7, 1.5])
+    n_steps = 90
+    Cg, drift = lib.propagate(basis, b, v, -15.0, 15.0, n_steps, track_norm=True)
+    Cg, drift = Cg.cpu().numpy(), drift.cpu().numpy()
+    for t in range(len(b)):
+        co, do = oprop.propagate(prob, b[t], v[t], -15.0, 15.0, n_steps, track_norm=True)
+        assert np.abs(np.abs(Cg[t]) ** 2 - np.abs(co) ** 2).max() < PTOL
+        assert np.abs(Cg[t] - co).max() < PTOL
+        assert abs(drift[t] - do) < 1e-12 + 1e-6 * do
+    out = lib.probabilities(basis, lib._torch().as_tensor(Cg, device="cuda"), b=b, vgroup=np.array([0, 1, 1, 2, 3]), n_vgroups=4)
+    Ps, Pnl, Pc = observables.probabilities(prob, Cg)
+    assert np.abs(out["P_state"].cpu().numpy() - Ps).max() < 1e-15
+    assert np.abs(out["P_nl"].cpu().numpy() - Pnl).max() < 1e-15
+    assert np.abs(out["P_class"].cpu().numpy() - Pc).max() < 1e-14
+    sig = observables.cross_sections(b, np.array([0, 1, 1, 2, 3]), Pnl, 4)
+    assert np.abs(out["sigma_nl"].cpu().numpy() - sig).max() < 1e-13
+
+
+def test_one_centre_windows_do_not_change_the_result(lib, one_centre):
+    """A workspace that forces short windows gives the same amplitudes (window boundaries are exact restarts)."""
+    prob, basis = one_centre
+    b, v = np.array([0.9, 2.5]), np.array([1.0, 1.0])
+    big = lib.propagate(basis, b, v, -10.0, 10.0, 70).cpu().numpy()
+    small_ws = lib._lib.wpccc_workspace_bytes(basis._h, 2, 70, 2) + (1 << 20)
+    small = lib.propagate(basis, b, v, -10.0, 10.0, 70, ws_bytes=small_ws).cpu().numpy()
+    assert np.abs(big - small).max() < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------ two centres
+QUAD = dict(n_rho=24, n_phi=8, n_z=48, rho_max=30.0, z_pad=30.0, phi_rule=0)
+POS2 = [(1.3, -0.8, 1.0), (0.4, 2.2, 1.5), (2.5, 0.0, 0.8), (0.2, -6.0, 1.0)]
+
+
+@pytest.fixture(scope="module")
+def two_centre(lib):
+    prob = tiny_problem(True, l_max=2, n_max=3, bins=2, k_max=2.0, Nr=400, h=0.1, Z_T=1.0, Z_P=2.0, quad=dict(QUAD), seed=11)
+    return prob, lib.setup_basis(prob)
+
+
+def test_two_centre_elements(lib, two_centre):
+    prob, basis = two_centre
+    b, z, v = map(np.array, zip(*POS2))
+    S, H = lib.matrix_elements(basis, b, z, v, phases=True)
+    S, H = S.cpu().numpy(), H.cpu().numpy()
+    NT = prob.centres[0].n_states
+    for p in range(len(b)):
+        So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
+        assert_elements(S[p], So, "S at position %d" % p)
+        assert_elements(H[p][:NT, :NT], Ho[:NT, :NT], "D^T at position %d" % p)
+        assert_elements(H[p][NT:, NT:], Ho[NT:, NT:], "D^P at position %d" % p)
+        assert_elements(H[p][NT:, :NT], Ho[NT:, :NT], "H_PT at position %d" % p)
+        assert_elements(H[p][:NT, NT:], Ho[:NT, NT:], "H_TP at position %d" % p)
+    # lab-frame definition (L0) on a few seeded pairs, no time phases
+    S0, H0 = lib.matrix_elements(basis, b[:1], z[:1], v[:1], phases=False)
+    S0, H0 = S0.cpu().numpy()[0], H0.cpu().numpy()[0]
+    T, P = prob.centres
+    rng = np.random.default_rng(3)
+    stT, stP = T.states(), P.states()
+    for _ in range(6):
+        ia, ib = int(rng.integers(len(stT))), int(rng.integers(len(stP)))
+        for kind, got in (("S", S0[NT + ib, ia]), ("HPT", H0[NT + ib, ia]), ("HTP", H0[ia, NT + ib])):
+            ref = otr.lab_frame_element(prob, stP[ib], stT[ia], b[0], z[0], v[0], kind)
+            assert abs(got - ref) <= REL * abs(ref) + FLOOR, (kind, ia, ib, got, ref)
+
+
+def test_two_centre_bessel_rule(lib):
+    q = dict(QUAD); q["phi_rule"] = 1
+    prob = tiny_problem(True, l_max=1, n_max=2, bins=1, k_max=1.5, Nr=300, h=0.1, quad=q)
+    basis = lib.setup_basis(prob)
+    S, H = lib.matrix_elements(basis, [0.9], [-1.3], [1.0])
+    So, Ho = assemble.S_and_H(prob, 0.9, -1.3, 1.0)
+    assert_elements(S.cpu().numpy()[0], So, "S (Bessel azimuth)")
+    assert_elements(H.cpu().numpy()[0], Ho, "H (Bessel azimuth)")
+
+
+def test_two_centre_propagation(lib, two_centre):
+    prob, basis = two_centre
+    b, v = np.array([0.7, 1.9, 0.7]), np.array([1.0, 1.0, 1.6])
+    n_steps = 40
+    Cg, drift = lib.propagate(basis, b, v, -8.0, 8.0, n_steps, track_norm=True)
+    Cg, drift = Cg.cpu().numpy(), drift.cpu().numpy()
+    for t in range(len(b)):
+        co, do = oprop.propagate(prob, b[t], v[t], -8.0, 8.0, n_steps, track_norm=True)
+        assert np.abs(np.abs(Cg[t]) ** 2 - np.abs(co) ** 2).max() < PTOL, t
+        assert np.abs(Cg[t] - co).max() < PTOL, t
+        assert abs(drift[t] - do) < 1e-10 + 1e-4 * do
+    small_ws = lib._lib.wpccc_workspace_bytes(basis._h, 3, n_steps, 2) + (4 << 20)
+    Cs = lib.propagate(basis, b, v, -8.0, 8.0, n_steps, ws_bytes=small_ws).cpu().numpy()
+    assert np.abs(Cs - Cg).max() < 1e-13
+
+
+def test_argument_errors(lib, one_centre):
+    prob, basis = one_centre
+    with pytest.raises(lib.WpcccError):
+        lib.propagate(basis, [1.0], [0.0], -1.0, 1.0, 10)             # v = 0
+    with pytest.raises(lib.WpcccError):
+        lib.propagate(basis, [1.0], [1.0], -1.0, 1.0, 10, ws_bytes=1024)   # workspace too small
+    assert lib.propagate(basis, np.zeros(0), np.zeros(0), -1.0, 1.0, 10).shape == (0, basis.n_tot)   # empty batch
