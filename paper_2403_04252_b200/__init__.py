@@ -4,7 +4,7 @@ Argument marshalling only: every step of the hot path (direct-coupling GEMM, tra
 RK4 sweep, probabilities) runs in the CUDA kernels of ``csrc/``.  PyTorch supplies device memory and the stream.
 There is no CPU fallback: importing works without a GPU (so that the symbol table can be checked), but every
 compute call raises ``WpcccError`` when the library cannot run on a CUDA device, and importing raises
-``ImportError`` when ``libwpccc.so`` has not been built (``python -m paper_2403_04252_b200.build``).
+``ImportError`` when ``libwpccc.so`` has not been built (``python paper_2403_04252_b200/build.py`` or ``__graft_entry__.build()``).
 
 The function names mirror the C entry points: ``setup_basis`` (wpccc_setup_basis), ``matrix_elements``,
 ``propagate``, ``probabilities``, ``fp64_peak``, ``last_timing``.
@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libwpccc.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "wpccc.h")
 
 if not os.path.exists(LIB_PATH):
-    raise ImportError("paper_2403_04252_b200: %s is missing -- build it with `python -m paper_2403_04252_b200.build` "
+    raise ImportError("paper_2403_04252_b200: %s is missing -- build it with `python paper_2403_04252_b200/build.py` "
                       "(there is no CPU fallback)" % LIB_PATH)
 _lib = C.CDLL(LIB_PATH)
 

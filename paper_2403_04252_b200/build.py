@@ -1,6 +1,8 @@
 """Builds libwpccc.so (the C-ABI CUDA library, include/wpccc.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_2403_04252_b200.build [--force]
+    python paper_2403_04252_b200/build.py [--force] [-v]      (or __graft_entry__.build())
+
+Run it by path: the package refuses to import while the library is missing.
 
 The shared library is written next to this file so that it travels to the GPU box with the repo snapshot.
 """

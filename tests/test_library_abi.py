@@ -12,8 +12,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 @pytest.fixture(scope="module")
 def wp():
-    from paper_2403_04252_b200 import build
-    build.build()
+    import __graft_entry__
+    __graft_entry__.build()
     import paper_2403_04252_b200 as wp
     return wp
 
