@@ -374,13 +374,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
 struct TrotArgs {
     const double *part; int n_split; int nq8T, nq8P;
     const double *theta;                     // [p] Theta = angle between R and v
-    const int *lT, *lP, *firstT, *firstP;    // per radial function: l, first state index
+    const int *radT, *lT_st, *mT_st;         // per target state: radial function, l, m
+    const int *radP, *lP_st, *mP_st;         // per projectile state
     const int *colT, *colP;                  // [n_rad][WP_MAX_L+1] column of (a, |q|)
-    int nradT, nradP, NT, NP, lmax;
+    int NT, NP, lmax;
     double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex
 };
 
-// Wigner d^l_{m' m}(beta) = <l m'| e^{-i beta J_y} |l m>, Wigner's sum formula.
+// Wigner d^l_{m' m}(beta) = <l m'| e^{-i beta J_y} |l m>, Wigner's sum formula; cb = cos(beta/2), sb = sin(beta/2).
 __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
     double tot = 0.0;
     const double num = sqrt(c_fact[l + m] * c_fact[l - m] * c_fact[l + mp] * c_fact[l - mp]);
@@ -392,69 +393,55 @@ __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
     return tot;
 }
 
-// grid = (position, ceil(nradP*nradT/128)); block 128: one thread per radial pair (b, a).
-__global__ void __launch_bounds__(128) k_trot(const TrotArgs a) {
-    __shared__ double sd[(WP_MAX_L + 1) * (2 * WP_MAX_L + 1) * (2 * WP_MAX_L + 1)];
-    const int p = blockIdx.x, tid = threadIdx.x, W = 2 * WP_MAX_L + 1;
+// grid = positions; block 256: one thread per lab-frame output element (product, beta, alpha), eq. (8):
+//   X_lab[beta, alpha] = sum_{q', q} d^{l_b}_{m_b q'}(Theta) d^{l_a}_{m_a q}(Theta) X_body[(b, q'), (a, q)],
+// where the signed body-frame element comes from the two q >= 0 families of the contraction:
+//   family (-) (weights Phi_{|q-q'|}) when q, q' have the same sign or one is 0, family (+) (Phi_{q+q'}) otherwise,
+//   times (-1)^q for q < 0 and (-1)^q' for q' < 0.
+__global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
+    extern __shared__ double sd[];           // [lmax+1][W][W], W = 2 lmax + 1
+    const int p = blockIdx.x, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
     {
         double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
-        for (int e = tid; e < (a.lmax + 1) * W * W; e += blockDim.x) {
-            const int l = e / (W * W), mp = (e / W) % W - WP_MAX_L, m = e % W - WP_MAX_L;
+        for (int e = tid; e < (L + 1) * W * W; e += blockDim.x) {
+            const int l = e / (W * W), mp = (e / W) % W - L, m = e % W - L;
             sd[e] = (abs(mp) <= l && abs(m) <= l) ? wigner_d(l, mp, m, cb, sb) : 0.0;
         }
     }
     __syncthreads();
-    const int pair = blockIdx.y * blockDim.x + tid;
-    if (pair >= a.nradP * a.nradT) return;
-    const int rb = pair / a.nradT, ra = pair % a.nradT;
-    const int lb = a.lP[rb], la = a.lT[ra];
+    const int NT = a.NT, NP = a.NP, N = NT + NP, npair = NT * NP;
     const size_t blk = (size_t)a.nq8P * a.nq8T;
-    const int N = a.NT + a.NP;
-    const double *dB = sd + lb * W * W, *dA = sd + la * W * W;
-    for (int prod = 0; prod < 3; ++prod) {
-        // signed body-frame block X[q'][q] from the two families
-        cplx X[2 * WP_MAX_L + 1][2 * WP_MAX_L + 1];
-        for (int qp = -lb; qp <= lb; ++qp)
+    const double *part = a.part + (size_t)p * a.n_split * 6 * blk * 2;
+    for (int e = tid; e < 3 * npair; e += blockDim.x) {
+        const int prod = e / npair, r = e - prod * npair;
+        // products 0, 1 are written row-major in (beta, alpha); product 2 (H_TP) in (alpha, beta): coalesced stores
+        const int ib = (prod < 2) ? r / NT : r % NP, ia = (prod < 2) ? r % NT : r / NP;
+        const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
+        const int ra = a.radT[ia], la = a.lT_st[ia], ma = a.mT_st[ia];
+        const double *dB = sd + (lb * W + mb + L) * W + L, *dA = sd + (la * W + ma + L) * W + L;
+        const int *cP = a.colP + rb * (WP_MAX_L + 1), *cT = a.colT + ra * (WP_MAX_L + 1);
+        double sr = 0.0, si = 0.0;
+        for (int qp = -lb; qp <= lb; ++qp) {
+            const int aqp = abs(qp);
+            const size_t rowoff = (size_t)cP[aqp] * a.nq8T;
+            double tr = 0.0, ti = 0.0;
             for (int q = -la; q <= la; ++q) {
-                const int aq = abs(q), aqp = abs(qp);
-                const bool same = (q >= 0) == (qp >= 0);           // family (-) when the signs agree, or one of them is 0
-                const int fam = (same || aq == 0 || aqp == 0) ? 0 : 1;
-                const size_t idx = (((size_t)fam * 3 + prod) * blk + (size_t)a.colP[rb * (WP_MAX_L + 1) + aqp] * a.nq8T + a.colT[ra * (WP_MAX_L + 1) + aq]) * 2;
+                const int aq = abs(q);
+                const int fam = ((q >= 0) == (qp >= 0) || aq == 0 || aqp == 0) ? 0 : 1;
+                const double *src = part + (((size_t)fam * 3 + prod) * blk + rowoff + cT[aq]) * 2;
                 double xr = 0.0, xi = 0.0;
-                for (int s = 0; s < a.n_split; ++s) {
-                    const double *src = a.part + ((size_t)p * a.n_split + s) * 6 * blk * 2 + idx;
-                    xr += src[0]; xi += src[1];
-                }
-                int sg = 0;
-                if (q < 0) sg += aq;
-                if (qp < 0) sg += aqp;
-                if (sg & 1) { xr = -xr; xi = -xi; }
-                X[qp + lb][q + la] = {xr, xi};
+                for (int s = 0; s < a.n_split; ++s) { xr += src[0]; xi += src[1]; src += 6 * blk * 2; }
+                int sg = (q < 0 ? aq : 0) + (qp < 0 ? aqp : 0);
+                const double dav = (sg & 1) ? -dA[q] : dA[q];
+                tr += dav * xr; ti += dav * xi;
             }
-        for (int mp = -lb; mp <= lb; ++mp)
-            for (int m = -la; m <= la; ++m) {
-                double sr = 0.0, si = 0.0;
-                for (int qp = -lb; qp <= lb; ++qp) {
-                    const double dbv = dB[(mp + WP_MAX_L) * W + qp + WP_MAX_L];
-                    double tr = 0.0, ti = 0.0;
-                    for (int q = -la; q <= la; ++q) {
-                        const double dav = dA[(m + WP_MAX_L) * W + q + WP_MAX_L];
-                        tr += dav * X[qp + lb][q + la].x; ti += dav * X[qp + lb][q + la].y;
-                    }
-                    sr += dbv * tr; si += dbv * ti;
-                }
-                const int ib = a.firstP[rb] + mp + lb, ia = a.firstT[ra] + m + la;
-                if (prod == 0) {
-                    double *o = a.K + (((size_t)p * a.NP + ib) * a.NT + ia) * 2;
-                    o[0] = sr; o[1] = si;
-                } else if (prod == 1) {
-                    double *o = a.H + (((size_t)p * N + a.NT + ib) * N + ia) * 2;       // H_PT
-                    o[0] = sr; o[1] = si;
-                } else {
-                    double *o = a.H + (((size_t)p * N + ia) * N + a.NT + ib) * 2;       // H_TP = conj(rot Tb)^T
-                    o[0] = sr; o[1] = -si;
-                }
-            }
+            sr += dB[qp] * tr; si += dB[qp] * ti;
+        }
+        double *o;
+        if (prod == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
+        else if (prod == 1) o = a.H + (((size_t)p * N + NT + ib) * N + ia) * 2;            // H_PT
+        else { o = a.H + (((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
+        o[0] = sr; o[1] = si;
     }
 }
 
@@ -482,35 +469,35 @@ static TransferPlan make_plan(const wpccc_basis *B, int n_split) {
     return P;
 }
 
-static int pick_split(const wpccc_basis *B) {
-    // enough CTAs per position that a chunk of few positions (tables resident in L2) fills the 148 SMs
+// Ring splits (split-K of the contraction) as a function of the positions per launch: none once a launch has two
+// waves of CTAs on the 148 SMs; for a handful of positions (wpccc_matrix_elements) enough to occupy the GPU.
+static int pick_split(const wpccc_basis *B, int chunk) {
     TransferPlan P = make_plan(B, 1);
-    int s = std::max(1, std::min(B->quad.n_rho, (int)(16 / std::max<size_t>(1, P.tiles.size() / 3))));
-    while (B->quad.n_rho / s < 4 && s > 1) --s;
-    return s;
+    const long long ctas = (long long)P.tiles.size() * std::max(chunk, 1);
+    int s = (int)std::min<long long>((296 + ctas - 1) / ctas, std::max(1, B->quad.n_rho / 4));
+    return std::max(1, s);
 }
 
 size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk) {
-    TransferPlan P = make_plan(B, pick_split(B));
+    TransferPlan P = make_plan(B, pick_split(B, n_pos_chunk));
     return P.per_pos_bytes() * (size_t)n_pos_chunk + P.tiles.size() * sizeof(int2) + 4096 +
            2 * (size_t)(B->c[0].n_rad + B->c[1].n_rad) * (WP_MAX_L + 1) * sizeof(int) +
            2 * (size_t)(B->c[0].nqc_pad + B->c[1].nqc_pad) * sizeof(int);
 }
 
 int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes) {
-    const size_t fixed = wp_transfer_ws_bytes(B, 0);
-    const size_t per = wp_transfer_ws_bytes(B, 1) - fixed;
-    if (ws_bytes <= fixed) return 0;
-    return (int)std::min<size_t>((ws_bytes - fixed) / per, 1 << 20);
+    if (wp_transfer_ws_bytes(B, 1) > ws_bytes) return 0;
+    int lo = 1, hi = 1 << 16;                       // largest chunk whose workspace fits (bytes grow with the chunk)
+    while (lo < hi) { const int mid = (lo + hi + 1) / 2; if (wp_transfer_ws_bytes(B, mid) <= ws_bytes) lo = mid; else hi = mid - 1; }
+    return lo;
 }
 
 int wp_transfer_default_chunk(const wpccc_basis *B) {
-    // node tables of one chunk ~ 64 MB (half of the 126 MB L2), at least enough CTAs for two waves of 148 SMs
-    TransferPlan P = make_plan(B, pick_split(B));
+    // a multiple of the SM count (every tile CTA has the same work, so launches are whole waves), node tables <= 6 GB
+    TransferPlan P = make_plan(B, 1);
     const size_t tab = (P.stride[0] + P.stride[1]) * 8;
-    int c = (int)std::max<size_t>(1, ((size_t)64 << 20) / tab);
-    const int ctas = (int)P.tiles.size() * P.n_split;
-    while (c * ctas < 296 && (size_t)c * tab < ((size_t)256 << 20)) ++c;
+    int c = 148;
+    while (c > 1 && (size_t)c * tab > ((size_t)6 << 30)) c /= 2;
     return c;
 }
 
@@ -527,11 +514,11 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         WP_CUDA(cudaMemcpyToSymbol(c_thnorm, tn, sizeof tn));
         consts = true;
     }
-    const int n_split = pick_split(B);
-    TransferPlan P = make_plan(B, n_split);
     const int max_chunk = wp_transfer_chunk_positions(B, ws_bytes);
     if (max_chunk < 1) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small (%zu bytes)", ws_bytes);
     chunk = std::max(1, std::min(std::min(chunk, max_chunk), n_pos));
+    const int n_split = pick_split(B, chunk);
+    TransferPlan P = make_plan(B, n_split);
 
     // carve the workspace
     char *w = (char *)ws; size_t off = 0;
@@ -604,12 +591,12 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         WP_CUDA(cudaGetLastError());
 
         TrotArgs tr{}; tr.part = d_part; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta + p0;
-        tr.lT = B->c[0].d_l; tr.lP = B->c[1].d_l; tr.firstT = B->c[0].d_rad_first; tr.firstP = B->c[1].d_rad_first;
-        tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.nradT = B->c[0].n_rad; tr.nradP = B->c[1].n_rad; tr.NT = NT; tr.NP = NP;
+        tr.radT = B->c[0].d_st_rad; tr.lT_st = B->c[0].d_st_l; tr.mT_st = B->c[0].d_st_m;
+        tr.radP = B->c[1].d_st_rad; tr.lP_st = B->c[1].d_st_l; tr.mP_st = B->c[1].d_st_m;
+        tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
         tr.lmax = lmx; tr.K = d_K + (size_t)p0 * NP * NT * 2; tr.H = d_H + (size_t)p0 * N * N * 2;
-        dim3 gr(np, (tr.nradP * tr.nradT + 127) / 128);
         wp_span_begin(B, FAM_ROT, s);
-        k_trot<<<gr, 128, 0, s>>>(tr);
+        k_trot<<<np, 256, (size_t)(lmx + 1) * (2 * lmx + 1) * (2 * lmx + 1) * sizeof(double), s>>>(tr);
         wp_span_end(B, s, 1);
         WP_CUDA(cudaGetLastError());
     }
