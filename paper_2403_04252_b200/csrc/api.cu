@@ -152,7 +152,7 @@ PropPlan plan_propagate(const wpccc_basis *B, int n_traj, int n_groups, int n_un
         P.tws = align256(wp_transfer_ws_bytes(B, wp_transfer_default_chunk(B)));
         P.fixed = P.tws + 64 * 1024 + (size_t)n_traj * 64;
         P.per_idx_single = (size_t)n_traj * (6 * 8 + (size_t)B->E_tot * 8) + 4096;                                   // geometry + F
-        P.per_idx_double = (size_t)n_traj * (N * N * 16 + NP * NT * 16 + NP * NP * 16 + NP * 4) + 4096;              // H0, K, LU, piv
+        P.per_idx_double = (size_t)n_traj * (N * N * 16 + NP * NT * 16 + NP * NP * 16) + 4096;                       // H0, K, Ainv
     } else {
         P.tws = 0;
         P.fixed = 64 * 1024 + (size_t)n_traj * 64 + (size_t)n_units * sizeof(SweepUnit);
@@ -261,7 +261,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
     if (init_state < 0 || init_state >= N) WP_FAIL(WPCCC_EINVAL, "init_state out of range");
     for (int t = 0; t < n_traj; ++t) if (!(b[t] > 0.0) || !(v[t] > 0.0)) WP_FAIL(WPCCC_EINVAL, "trajectory %d: need b > 0 and v > 0", t);
     if (!ws) WP_FAIL(WPCCC_ENOMEM, "workspace is NULL");
-    cudaStream_t s = (cudaStream_t)stream, e = B->side;
+    cudaStream_t s = (cudaStream_t)stream, e = B->side, sw = B->hi;
     wp_timing_reset(B);
     const bool two = B->n_centres == 2;
     const double h = (z_max - z_min) / n_steps;
@@ -302,12 +302,11 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
     GeomOut g = carve_geom(cv, npos_max);
     double *d_F = cv.take<double>(npos_max * B->E_tot);
     double *d_H[2] = {nullptr, nullptr}, *d_K[2] = {nullptr, nullptr}, *d_LU[2] = {nullptr, nullptr}, *d_D[2] = {nullptr, nullptr};
-    int *d_piv[2] = {nullptr, nullptr};
     const size_t NT = B->c[0].n_states, NP = two ? B->c[1].n_states : 0;
     for (int k = 0; k < 2; ++k) {
         if (two) {
             d_H[k] = cv.take<double>(npos_max * N * N * 2); d_K[k] = cv.take<double>(npos_max * NP * NT * 2);
-            d_LU[k] = cv.take<double>(npos_max * NP * NP * 2); d_piv[k] = cv.take<int>(npos_max * NP);
+            d_LU[k] = cv.take<double>(npos_max * NP * NP * 2);
         } else d_D[k] = cv.take<double>(npos_max * N * N);
     }
     if (!cv.ok) WP_FAIL(WPCCC_ENOMEM, "workspace too small (internal plan mismatch)");
@@ -321,11 +320,12 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
     if (d_norm_drift) WP_CUDA(cudaMemsetAsync(d_norm_drift, 0, n_traj * sizeof(double), s));
     const int tchunk = two ? wp_transfer_default_chunk(B) : 0;
 
-    // element stream `e` forks from the caller's stream; sweep stays on `s`
+    // element stream `e` and sweep stream `sw` fork from the caller's stream and join back at the end
     cudaEvent_t ev_elem[2], ev_sweep[2];
     for (int k = 0; k < 2; ++k) { WP_CUDA(cudaEventCreateWithFlags(&ev_elem[k], cudaEventDisableTiming)); WP_CUDA(cudaEventCreateWithFlags(&ev_sweep[k], cudaEventDisableTiming)); }
     WP_CUDA(cudaEventRecord(B->ev_fork, s));
     WP_CUDA(cudaStreamWaitEvent(e, B->ev_fork, 0));
+    WP_CUDA(cudaStreamWaitEvent(sw, B->ev_fork, 0));
     int rc = 0, wi = 0;
     for (int s0 = 0; s0 < n_steps && !rc; s0 += W, ++wi) {
         const int steps = std::min(W, n_steps - s0), n_idx = 2 * steps + 1, buf = wi & 1;
@@ -338,36 +338,39 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         if (two) {
             WP_CUDA(cudaMemsetAsync(d_H[buf], 0, (size_t)n_pos * N * N * 16, e));
             rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e);
-            if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], d_piv[buf], e);
+            if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], e);
         } else {
             rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, e);
             if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_D[buf], N, (long long)N * N, 0, e);
         }
         if (rc) break;
         WP_CUDA(cudaEventRecord(ev_elem[buf], e));
-        WP_CUDA(cudaStreamWaitEvent(s, ev_elem[buf], 0));
+        WP_CUDA(cudaStreamWaitEvent(sw, ev_elem[buf], 0));
         if (two) {
             Sweep2Args a{};
-            a.H = d_H[buf]; a.K = d_K[buf]; a.LU = d_LU[buf]; a.piv = d_piv[buf];
+            a.H = d_H[buf]; a.K = d_K[buf]; a.Ainv = d_LU[buf];
             a.st_rad_T = B->c[0].d_st_rad; a.st_rad_P = B->c[1].d_st_rad; a.eps_T = B->c[0].d_eps; a.eps_P = B->c[1].d_eps;
             a.v = d_v; a.C = dC; a.drift = d_norm_drift; a.NT = (int)NT; a.NP = (int)NP; a.n_idx = n_idx; a.steps = steps; a.i0 = i0; a.z_min = z_min; a.h = h;
-            rc = wp_sweep_two_centre(B, n_traj, a, s);
+            rc = wp_sweep_two_centre(B, n_traj, a, sw);
         } else {
             Sweep1Args a{};
             a.units = d_units; a.D = d_D[buf]; a.st_rad = B->c[0].d_st_rad; a.eps = B->c[0].d_eps; a.v = d_v; a.C = dC; a.drift = d_norm_drift;
             a.N = N; a.n_rad = B->c[0].n_rad; a.n_idx = n_idx; a.steps = steps; a.i0 = i0; a.z_min = z_min; a.h = h;
-            rc = wp_sweep_one_centre(B, (int)units.size(), a, s);
+            rc = wp_sweep_one_centre(B, (int)units.size(), a, sw);
         }
         if (rc) break;
-        WP_CUDA(cudaEventRecord(ev_sweep[buf], s));
+        WP_CUDA(cudaEventRecord(ev_sweep[buf], sw));
     }
     // join: the caller's stream waits for everything enqueued on the element stream
     cudaEventRecord(B->ev_join, e);
     cudaStreamWaitEvent(s, B->ev_join, 0);
+    cudaEventRecord(B->ev_join2, sw);
+    cudaStreamWaitEvent(s, B->ev_join2, 0);
     int status[4] = {0, 0, 0, 0};
     cudaError_t ce = cudaMemcpyAsync(status, B->d_status, sizeof status, cudaMemcpyDeviceToHost, s);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
     cudaStreamSynchronize(e);
+    cudaStreamSynchronize(sw);
     for (int k = 0; k < 2; ++k) { cudaEventDestroy(ev_elem[k]); cudaEventDestroy(ev_sweep[k]); }
     if (rc) return rc;
     if (ce != cudaSuccess) WP_FAIL(WPCCC_ECUDA, "propagate: %s", cudaGetErrorString(ce));

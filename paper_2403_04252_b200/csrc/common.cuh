@@ -69,8 +69,9 @@ struct wpccc_basis {
     int    *d_status = nullptr; // [4] device status word (0 ok; 1 zero pivot; 2 |S_PT| >= 1), position index
     char *arena = nullptr; size_t arena_bytes = 0;
     // timing
-    cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t side = nullptr;   // element kernels of wpccc_propagate
+    cudaStream_t hi = nullptr;     // RK4 sweep of wpccc_propagate (highest priority: few CTAs, on the critical path)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;
     std::vector<cudaEvent_t> ev_pool;
     struct Span { int fam; cudaEvent_t a, b; };
     std::vector<Span> spans;
@@ -104,7 +105,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
 int wp_transfer_default_chunk(const wpccc_basis *B);
 
 // ---- sweep.cu ----
-int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_LU, int *d_piv, cudaStream_t s);
+int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cudaStream_t s);
 
 // ---- device helpers ----
 __host__ __device__ inline int lm_index(int l, int m) { return l * l + l + m; }

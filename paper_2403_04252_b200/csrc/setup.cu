@@ -290,7 +290,11 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     }
     if (!rc && cudaStreamSynchronize(s) != cudaSuccess) { wp_set_error("setup: stream synchronize failed"); rc = WPCCC_ECUDA; }
     if (!rc) {
-        if (cudaStreamCreateWithFlags(&B->side, cudaStreamNonBlocking) != cudaSuccess ||
+        int pr_least = 0, pr_greatest = 0;
+        cudaDeviceGetStreamPriorityRange(&pr_least, &pr_greatest);
+        if (cudaStreamCreateWithPriority(&B->side, cudaStreamNonBlocking, pr_least) != cudaSuccess ||
+            cudaStreamCreateWithPriority(&B->hi, cudaStreamNonBlocking, pr_greatest) != cudaSuccess ||
+            cudaEventCreateWithFlags(&B->ev_join2, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&B->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&B->ev_join, cudaEventDisableTiming) != cudaSuccess) { wp_set_error("stream/event creation failed"); rc = WPCCC_ECUDA; }
     }
@@ -304,7 +308,9 @@ extern "C" void wpccc_free_basis(wpccc_basis *B) {
     for (auto e : B->ev_pool) cudaEventDestroy(e);
     if (B->ev_fork) cudaEventDestroy(B->ev_fork);
     if (B->ev_join) cudaEventDestroy(B->ev_join);
+    if (B->ev_join2) cudaEventDestroy(B->ev_join2);
     if (B->side) cudaStreamDestroy(B->side);
+    if (B->hi) cudaStreamDestroy(B->hi);
     delete B;
 }
 

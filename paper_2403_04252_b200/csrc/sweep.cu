@@ -9,8 +9,11 @@
 // a7: S0 = [[I, K^H], [K, I]].  Gaussian elimination with partial pivoting of S0 picks the unit diagonal as pivot
 // in its first N_T columns whenever every |K_ij| < 1 (the other candidates in column j are exactly K[:,j]), which
 // leaves the Schur complement A = I - K K^H in the projectile block.  The kernel forms A, checks |K_ij| < 1, and
-// continues the same elimination (partial pivoting, first maximal pivot wins) on A.  Solve:
-//     y_P' = y_P - K y_T;  A w_P = y_P';  w_T = y_T - K^H w_P.
+// continues the elimination (partial pivoting, first maximal pivot wins) on A in Gauss-Jordan form, which yields
+// A^{-1} explicitly: the four solves of an RK4 step then have no sequential dependency chain,
+//     y_P' = y_P - K y_T;  w_P = A^{-1} y_P';  w_T = y_T - K^H w_P.
+#include <algorithm>
+
 #include "sweep.cuh"
 
 namespace {
@@ -126,193 +129,322 @@ __global__ void __launch_bounds__(256) k_sweep1(const Sweep1Args a) {
     }
 }
 
-// ------------------------------------------------------------------ a7: Schur complement + LU
-// grid = positions; block = 256.  A (column-major, ld = NP) lives in shared memory when it fits, else in LU (global).
-struct FactorArgs { const double *K; double *LU; int *piv; int *status; int NT, NP, use_smem; };
+// ------------------------------------------------------------------ a7: Schur complement + inverse
+// grid = positions; block = 256.  A = I - K K^H (row-major, ld = NP) lives in shared memory when it fits, else in
+// the output buffer (global).  K is staged through shared memory in column chunks of odd width cw (conflict-free).
+// A^{-1} by in-place Gauss-Jordan elimination with partial (row) pivoting, first maximal |pivot| wins; the row
+// interchanges are undone as column interchanges in reverse order at the end.
+struct FactorArgs { const double *K; double *Ainv; int *status; int NT, NP, use_smem, cw; };
 
 __global__ void __launch_bounds__(256) k_factor(const FactorArgs a) {
     extern __shared__ __align__(16) double sm[];
-    const int NP = a.NP, NT = a.NT, tid = threadIdx.x, nt = blockDim.x;
+    const int n = a.NP, NT = a.NT, cw = a.cw, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const size_t p = blockIdx.x;
-    const cplx *K = reinterpret_cast<const cplx *>(a.K) + p * (size_t)NP * NT;
-    cplx *G = reinterpret_cast<cplx *>(a.LU) + p * (size_t)NP * NP;
-    cplx *A = a.use_smem ? reinterpret_cast<cplx *>(sm) : G;
-    int *piv = a.piv + p * NP;
-    __shared__ double s_red[256]; __shared__ int s_idx[256]; __shared__ int s_flag;
+    const cplx *K = reinterpret_cast<const cplx *>(a.K) + p * (size_t)n * NT;
+    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + p * (size_t)n * n;
+    cplx *smc = reinterpret_cast<cplx *>(sm);
+    cplx *A = a.use_smem ? smc : G;
+    cplx *Kc = smc + (a.use_smem ? (size_t)n * n : 0);     // [n][cw]
+    cplx *col = Kc + (size_t)n * cw, *rowj = col + n;      // [n] each
+    int *piv = reinterpret_cast<int *>(rowj + n), *idx = piv + n;
+    __shared__ int s_flag, s_piv;
     if (tid == 0) s_flag = 0;
     __syncthreads();
-    // |K_ij| < 1 check (pivot-order precondition)
-    int bad = 0;
-    for (int i = tid; i < NP * NT; i += nt) { cplx k = K[i]; if (!(k.x * k.x + k.y * k.y < 1.0)) bad = 1; }
-    if (bad) s_flag = 2;
     // A[r][s] = delta_rs - sum_i K[r][i] conj(K[s][i]), accumulated in the order i = 0..NT-1 (the elimination order)
-    for (int e = tid; e < NP * NP; e += nt) {
-        const int r = e % NP, s = e / NP;
-        const cplx *Kr = K + (size_t)r * NT, *Ks = K + (size_t)s * NT;
-        double ar = (r == s) ? 1.0 : 0.0, ai = 0.0;
-        for (int i = 0; i < NT; ++i) { cplx x = Kr[i], y = Ks[i]; ar -= x.x * y.x + x.y * y.y; ai -= x.y * y.x - x.x * y.y; }
-        A[(size_t)s * NP + r] = {ar, ai};
-    }
-    __syncthreads();
-    for (int j = 0; j < NP; ++j) {
-        // pivot search in column j, rows j..NP-1 (first maximal |.| wins)
-        double best = -1.0; int bi = j;
-        for (int i = j + tid; i < NP; i += nt) { cplx x = A[(size_t)j * NP + i]; double m = x.x * x.x + x.y * x.y; if (m > best) { best = m; bi = i; } }
-        s_red[tid] = best; s_idx[tid] = bi;
+    int bad = 0;
+    for (int i0 = 0; i0 < NT; i0 += cw) {
+        const int w = min(cw, NT - i0);
+        for (int e = tid; e < n * w; e += nt) {
+            const int r = e / w, ii = e - r * w;
+            const cplx k = K[(size_t)r * NT + i0 + ii];
+            Kc[r * cw + ii] = k;
+            if (!(k.x * k.x + k.y * k.y < 1.0)) bad = 1;       // pivot-order precondition |K_ij| < 1
+        }
         __syncthreads();
-        for (int o = nt >> 1; o > 0; o >>= 1) {
-            if (tid < o) {
-                double m2 = s_red[tid + o]; int i2 = s_idx[tid + o];
-                if (m2 > s_red[tid] || (m2 == s_red[tid] && i2 < s_idx[tid])) { s_red[tid] = m2; s_idx[tid] = i2; }
+        for (int e = tid; e < n * n; e += nt) {
+            const int r = e / n, s = e - r * n;
+            cplx acc = (i0 == 0) ? cplx{(r == s) ? 1.0 : 0.0, 0.0} : A[e];
+            const cplx *Kr = Kc + r * cw, *Ks = Kc + s * cw;
+            for (int ii = 0; ii < w; ++ii) { const cplx x = Kr[ii], y = Ks[ii]; acc.x -= x.x * y.x + x.y * y.y; acc.y -= x.y * y.x - x.x * y.y; }
+            A[e] = acc;
+        }
+        __syncthreads();
+    }
+    if (bad) s_flag = 2;
+    for (int j = 0; j < n; ++j) {
+        if (warp == 0) {                                       // pivot search in column j, rows j..n-1
+            double best = -1.0; int bi = j;
+            for (int i = j + lane; i < n; i += 32) { const cplx x = A[(size_t)i * n + j]; const double m = x.x * x.x + x.y * x.y; if (m > best) { best = m; bi = i; } }
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double m2 = __shfl_xor_sync(0xffffffffu, best, o); const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
             }
+            if (lane == 0) { s_piv = bi; piv[j] = bi; if (!(best > 0.0)) s_flag = 1; }
+        }
+        __syncthreads();
+        const int pr = s_piv;
+        if (pr != j) {
+            for (int c = tid; c < n; c += nt) { const cplx t = A[(size_t)j * n + c]; A[(size_t)j * n + c] = A[(size_t)pr * n + c]; A[(size_t)pr * n + c] = t; }
             __syncthreads();
         }
-        const int pr = s_idx[0];
-        const double pm = s_red[0];
-        if (tid == 0) { piv[j] = pr; if (!(pm > 0.0)) s_flag = 1; }
-        if (pr != j)
-            for (int c = tid; c < NP; c += nt) { cplx t = A[(size_t)c * NP + j]; A[(size_t)c * NP + j] = A[(size_t)c * NP + pr]; A[(size_t)c * NP + pr] = t; }
-        __syncthreads();
-        const cplx d = A[(size_t)j * NP + j];
+        const cplx d = A[(size_t)j * n + j];
         const double dn = d.x * d.x + d.y * d.y;
         const cplx dinv = (dn > 0.0) ? cplx{d.x / dn, -d.y / dn} : cplx{0.0, 0.0};
+        for (int i = tid; i < n; i += nt) {
+            col[i] = A[(size_t)i * n + j];
+            rowj[i] = (i == j) ? dinv : cmul(A[(size_t)j * n + i], dinv);
+        }
         __syncthreads();
-        for (int i = j + 1 + tid; i < NP; i += nt) A[(size_t)j * NP + i] = cmul(A[(size_t)j * NP + i], dinv);
-        __syncthreads();
-        // trailing update A[i][c] -= L[i][j] * U[j][c], i, c > j
-        const int rem = NP - 1 - j;
-        for (int e = tid; e < rem * rem; e += nt) {
-            const int i = j + 1 + e % rem, c = j + 1 + e / rem;
-            A[(size_t)c * NP + i] = csub(A[(size_t)c * NP + i], cmul(A[(size_t)j * NP + i], A[(size_t)c * NP + j]));
+        {   // A[i][c] = (i == j) ? rowj[c] : (c == j ? 0 : A[i][c]) - col[i] rowj[c]
+            int i = tid / n, c = tid - i * n;
+            const int di = nt / n, dc = nt - di * n;
+            for (int e = tid; e < n * n; e += nt) {
+                const cplx rj = rowj[c];
+                cplx v = A[e];
+                if (c == j) v = {0.0, 0.0};
+                A[e] = (i == j) ? rj : csub(v, cmul(col[i], rj));
+                i += di; c += dc; if (c >= n) { c -= n; ++i; }
+            }
         }
         __syncthreads();
     }
-    if (a.use_smem) for (int e = tid; e < NP * NP; e += nt) G[e] = A[e];
+    if (a.use_smem) {
+        if (tid == 0) {
+            for (int c = 0; c < n; ++c) idx[c] = c;
+            for (int j = n - 1; j >= 0; --j) { const int q = piv[j]; const int t = idx[j]; idx[j] = idx[q]; idx[q] = t; }
+        }
+        __syncthreads();
+        for (int e = tid; e < n * n; e += nt) { const int r = e / n, c = e - r * n; G[e] = A[(size_t)r * n + idx[c]]; }
+    } else {
+        for (int j = n - 1; j >= 0; --j) {
+            const int q = piv[j];
+            if (q != j) {
+                for (int r = tid; r < n; r += nt) { const cplx t = A[(size_t)r * n + j]; A[(size_t)r * n + j] = A[(size_t)r * n + q]; A[(size_t)r * n + q] = t; }
+                __syncthreads();
+            }
+        }
+    }
     if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
 }
 
 // ------------------------------------------------------------------ two-centre sweep
-// grid = trajectories; block = 256.  smem: C, Acc, X, Kn, Y, W [N] complex + ph [N] complex + partial[8][NT].
-__global__ void __launch_bounds__(256) k_sweep2(const Sweep2Args a) {
-    extern __shared__ __align__(16) double sm[];
-    const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+// grid = trajectories; block = 8 consumer warps + 1 producer warp.  Per RK4 stage, with phase-free H0, K and
+// Ainv = (I - K K^H)^{-1} of the stage's position:
+//     y = H0 x;   y_P -= K y_T;   w_P = Ainv y_P;   w_T = y_T - K^H w_P;   k = -(i/v) P w.
+// The matrices do not depend on the amplitudes, so the producer warp streams them (rows of H0, K, Ainv, K again)
+// through a shared-memory ring with TMA bulk copies, running ahead of the consumers across stage boundaries.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
+        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
+
+constexpr int SW_STAGES = 4;
+constexpr int SW_CONSUMERS = 256;
+
+// Chunk schedule of one RK4 step: stages 0..3 each [H rows | K rows | Ainv rows | K rows], then (drift only) K rows.
+struct SweepSched {
+    int N, NT, NP, rH, rK, rA, nH, nK, nA, per_stage, per_step;
+    __device__ SweepSched(int NT_, int NP_, int chunk_bytes, bool drift) {
+        NT = NT_; NP = NP_; N = NT + NP;
+        rH = max(1, chunk_bytes / (16 * N)); rK = max(1, chunk_bytes / (16 * NT)); rA = max(1, chunk_bytes / (16 * NP));
+        nH = (N + rH - 1) / rH; nK = (NP + rK - 1) / rK; nA = (NP + rA - 1) / rA;
+        per_stage = nH + 2 * nK + nA; per_step = 4 * per_stage + (drift ? nK : 0);
+    }
+};
+
+// sum over c of row[c] * x[c], c = 0..n-1, by one warp (every lane returns the sum)
+__device__ __forceinline__ cplx warp_dot(const cplx *row, const cplx *x, int n, int lane) {
+    double sr = 0.0, si = 0.0;
+    for (int c = lane; c < n; c += 32) { const cplx k = row[c], v = x[c]; sr += k.x * v.x - k.y * v.y; si += k.x * v.y + k.y * v.x; }
+    return {warp_sum(sr), warp_sum(si)};
+}
+
+__global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a, const int chunk_bytes) {
+    extern __shared__ __align__(128) unsigned char smraw[];
+    const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int t = blockIdx.x;
-    cplx *C = reinterpret_cast<cplx *>(sm);
-    cplx *Acc = C + N, *X = Acc + N, *Kn = X + N, *Y = Kn + N, *ph = Y + N, *part = ph + N;   // part [nw][NT]
+    const bool track = a.drift != nullptr;
+    const SweepSched S(NT, NP, chunk_bytes, track);
+    unsigned char *ring = smraw;
+    cplx *C = reinterpret_cast<cplx *>(smraw + (size_t)SW_STAGES * chunk_bytes);
+    cplx *Acc = C + N, *X = Acc + N, *Kn = X + N, *Y = Kn + N, *ph = Y + N, *Wp = ph + N, *part = Wp + NP;   // part [8][NT]
+    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
     __shared__ double red[8];
-    const double vel = a.v[t], h = a.h;
-    for (int j = tid; j < N; j += blockDim.x) { const double *src = a.C + ((size_t)t * N + j) * 2; C[j] = {src[0], src[1]}; }
-    double drift = a.drift ? a.drift[t] : 0.0;
+    if (tid == 0) {
+        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+    }
     __syncthreads();
+    const cplx *Hg = reinterpret_cast<const cplx *>(a.H), *Kg = reinterpret_cast<const cplx *>(a.K), *Ag = reinterpret_cast<const cplx *>(a.Ainv);
+
+    if (warp == SW_CONSUMERS / 32) {
+        // ---------------- producer: one lane streams the chunk sequence of the whole window
+        if (lane != 0) return;
+        const long long total = (long long)a.steps * S.per_step;
+        for (long long g = 0; g < total; ++g) {
+            const int slot = (int)(g % SW_STAGES); const long long use = g / SW_STAGES;
+            if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
+            const int s = (int)(g / S.per_step); int rem = (int)(g - (long long)s * S.per_step);
+            int st = rem / S.per_stage, phase, q;
+            if (st >= 4) { st = 4; phase = 1; q = rem - 4 * S.per_stage; }
+            else {
+                q = rem - st * S.per_stage;
+                if (q < S.nH) phase = 0;
+                else if (q < S.nH + S.nK) { phase = 1; q -= S.nH; }
+                else if (q < S.nH + S.nK + S.nA) { phase = 2; q -= S.nH + S.nK; }
+                else { phase = 3; q -= S.nH + S.nK + S.nA; }
+            }
+            const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
+            const size_t pos = (size_t)t * a.n_idx + li;
+            const cplx *src; unsigned bytes;
+            if (phase == 0) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); src = Hg + pos * (size_t)N * N + (size_t)r0 * N; bytes = (unsigned)rows * N * 16u; }
+            else if (phase == 2) { const int r0 = q * S.rA, rows = min(S.rA, NP - r0); src = Ag + pos * (size_t)NP * NP + (size_t)r0 * NP; bytes = (unsigned)rows * NP * 16u; }
+            else { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); src = Kg + pos * (size_t)NP * NT + (size_t)r0 * NT; bytes = (unsigned)rows * NT * 16u; }
+            mbar_expect_tx(&full[slot], bytes);
+            tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
+        }
+        return;
+    }
+    // ---------------- consumers (256 threads)
+    const double vel = a.v[t], h = a.h;
+    for (int j = tid; j < N; j += SW_CONSUMERS) {
+        const double *src = a.C + ((size_t)t * N + j) * 2;
+        C[j] = {src[0], src[1]}; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0};
+    }
+    double drift = track ? a.drift[t] : 0.0;
+    long long g = 0;                                         // chunk counter, in step with the producer
+    auto acquire = [&]() -> const cplx * {
+        const int slot = (int)(g % SW_STAGES);
+        mbar_wait(&full[slot], (unsigned)((g / SW_STAGES) & 1));
+        return reinterpret_cast<const cplx *>(ring + (size_t)slot * chunk_bytes);
+    };
+    auto release = [&]() {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[(int)(g % SW_STAGES)]);
+        ++g;
+    };
+    consumer_sync();
 
     for (int s = 0; s < a.steps; ++s) {
-        for (int j = tid; j < N; j += blockDim.x) { Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
-        __syncthreads();
         #pragma unroll 1
         for (int st = 0; st < 5; ++st) {
             // st = 0..3: RK4 stages; st = 4: norm c^H S c at z_new (only when drift is tracked)
-            if (st == 4 && !a.drift) break;
+            if (st == 4 && !track) break;
             const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
             const double alpha = (st == 0 || st == 4) ? 0.0 : (st == 3 ? h : 0.5 * h);
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
             const double z = zpos(a.z_min, h, a.i0 + li);
-            const size_t pos = (size_t)t * a.n_idx + li;
-            for (int j = tid; j < N; j += blockDim.x) {
-                double e = (j < NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - NT]];
+            for (int j = tid; j < N; j += SW_CONSUMERS) {
+                const double e = (j < NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - NT]];
                 double sn, cs; sincos(e * z / vel, &sn, &cs);
                 ph[j] = {cs, sn};
-                cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
+                const cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
                 X[j] = cmulc(x, {cs, sn});
             }
-            __syncthreads();
-            const cplx *Kp = reinterpret_cast<const cplx *>(a.K) + pos * (size_t)NP * NT;
+            for (int j = tid; j < 8 * NT; j += SW_CONSUMERS) part[j] = {0.0, 0.0};
+            consumer_sync();
             if (st == 4) {
                 // c^H S c = |c|^2 + 2 Re( X_P^H K X_T )
                 double acc = 0.0;
-                for (int row = warp; row < NP; row += nw) {
-                    double sr = 0.0, si = 0.0;
-                    for (int col = lane; col < NT; col += 32) { cplx k = Kp[(size_t)row * NT + col], x = X[col]; sr += k.x * x.x - k.y * x.y; si += k.x * x.y + k.y * x.x; }
-                    sr = warp_sum(sr); si = warp_sum(si);
-                    acc += 2.0 * (X[NT + row].x * sr + X[NT + row].y * si);
+                for (int q = 0; q < S.nK; ++q) {
+                    const cplx *buf = acquire();
+                    const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
+                    for (int r = warp; r < rows; r += 8) {
+                        const cplx d = warp_dot(buf + (size_t)r * NT, X, NT, lane);
+                        acc += 2.0 * (X[NT + r0 + r].x * d.x + X[NT + r0 + r].y * d.y);
+                    }
+                    release();
                 }
                 double nrm = 0.0;
-                for (int j = lane + 32 * warp; j < N; j += blockDim.x) nrm += X[j].x * X[j].x + X[j].y * X[j].y;
+                for (int j = tid; j < N; j += SW_CONSUMERS) nrm += X[j].x * X[j].x + X[j].y * X[j].y;
                 nrm = warp_sum(nrm);
                 if (lane == 0) red[warp] = acc + nrm;
-                __syncthreads();
+                consumer_sync();
                 double tot = 0.0;
-                for (int w = 0; w < nw; ++w) tot += red[w];
+                for (int w = 0; w < 8; ++w) tot += red[w];
                 drift = fmax(drift, fabs(tot - 1.0));
-                __syncthreads();
+                consumer_sync();
                 break;
             }
-            // Y = H0 X
-            const cplx *Hp = reinterpret_cast<const cplx *>(a.H) + pos * (size_t)N * N;
-            for (int row = warp; row < N; row += nw) {
-                const cplx *Hr = Hp + (size_t)row * N;
-                double sr = 0.0, si = 0.0;
-                for (int col = lane; col < N; col += 32) { cplx hh = Hr[col], x = X[col]; sr += hh.x * x.x - hh.y * x.y; si += hh.x * x.y + hh.y * x.x; }
-                sr = warp_sum(sr); si = warp_sum(si);
-                if (lane == 0) Y[row] = {sr, si};
+            // y = H0 x
+            for (int q = 0; q < S.nH; ++q) {
+                const cplx *buf = acquire();
+                const int r0 = q * S.rH, rows = min(S.rH, N - r0);
+                for (int r = warp; r < rows; r += 8) {
+                    const cplx d = warp_dot(buf + (size_t)r * N, X, N, lane);
+                    if (lane == 0) Y[r0 + r] = d;
+                }
+                release();
             }
-            __syncthreads();
-            // Y_P -= K Y_T
-            for (int row = warp; row < NP; row += nw) {
-                double sr = 0.0, si = 0.0;
-                for (int col = lane; col < NT; col += 32) { cplx k = Kp[(size_t)row * NT + col], x = Y[col]; sr += k.x * x.x - k.y * x.y; si += k.x * x.y + k.y * x.x; }
-                sr = warp_sum(sr); si = warp_sum(si);
-                if (lane == 0) { Y[NT + row].x -= sr; Y[NT + row].y -= si; }
+            consumer_sync();
+            // y_P -= K y_T
+            for (int q = 0; q < S.nK; ++q) {
+                const cplx *buf = acquire();
+                const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
+                for (int r = warp; r < rows; r += 8) {
+                    const cplx d = warp_dot(buf + (size_t)r * NT, Y, NT, lane);
+                    if (lane == 0) { Y[NT + r0 + r].x -= d.x; Y[NT + r0 + r].y -= d.y; }
+                }
+                release();
             }
-            __syncthreads();
-            // A w_P = Y_P by the LU factors (column-major), in place in Y_P
-            const cplx *LU = reinterpret_cast<const cplx *>(a.LU) + pos * (size_t)NP * NP;
-            const int *piv = a.piv + pos * NP;
-            cplx *yp = Y + NT;
-            if (tid == 0) for (int j = 0; j < NP; ++j) { int pr = piv[j]; if (pr != j) { cplx tt = yp[j]; yp[j] = yp[pr]; yp[pr] = tt; } }
-            __syncthreads();
-            for (int j = 0; j < NP - 1; ++j) {
-                const cplx wj = yp[j];
-                __syncthreads();
-                for (int i = j + 1 + tid; i < NP; i += blockDim.x) yp[i] = csub(yp[i], cmul(LU[(size_t)j * NP + i], wj));
-                __syncthreads();
+            consumer_sync();
+            // w_P = Ainv y_P
+            for (int q = 0; q < S.nA; ++q) {
+                const cplx *buf = acquire();
+                const int r0 = q * S.rA, rows = min(S.rA, NP - r0);
+                for (int r = warp; r < rows; r += 8) {
+                    const cplx d = warp_dot(buf + (size_t)r * NP, Y + NT, NP, lane);
+                    if (lane == 0) Wp[r0 + r] = d;
+                }
+                release();
             }
-            for (int j = NP - 1; j >= 0; --j) {
-                if (tid == 0) { cplx d = LU[(size_t)j * NP + j]; double dn = d.x * d.x + d.y * d.y; yp[j] = cmul(yp[j], {d.x / dn, -d.y / dn}); }
-                __syncthreads();
-                const cplx wj = yp[j];
-                for (int i = tid; i < j; i += blockDim.x) yp[i] = csub(yp[i], cmul(LU[(size_t)j * NP + i], wj));
-                __syncthreads();
+            consumer_sync();
+            // w_T = y_T - K^H w_P: per-warp partial sums over its rows of K
+            for (int q = 0; q < S.nK; ++q) {
+                const cplx *buf = acquire();
+                const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
+                for (int r = warp; r < rows; r += 8) {
+                    const cplx x = Wp[r0 + r];
+                    const cplx *Kr = buf + (size_t)r * NT;
+                    cplx *pw = part + warp * NT;
+                    for (int c = lane; c < NT; c += 32) { const cplx k = Kr[c]; pw[c].x += k.x * x.x + k.y * x.y; pw[c].y += k.x * x.y - k.y * x.x; }
+                }
+                release();
             }
-            // w_T = Y_T - K^H w_P: partial sums over rows of K per warp, then reduce
-            for (int col = lane; col < NT; col += 32) {
-                double sr = 0.0, si = 0.0;
-                for (int row = warp; row < NP; row += nw) { cplx k = Kp[(size_t)row * NT + col], x = yp[row]; sr += k.x * x.x + k.y * x.y; si += k.x * x.y - k.y * x.x; }
-                part[warp * NT + col] = {sr, si};
-            }
-            __syncthreads();
-            for (int col = tid; col < NT; col += blockDim.x) {
-                double sr = 0.0, si = 0.0;
-                for (int w = 0; w < nw; ++w) { sr += part[w * NT + col].x; si += part[w * NT + col].y; }
-                Y[col].x -= sr; Y[col].y -= si;
-            }
-            __syncthreads();
+            consumer_sync();
             // k = -(i/v) P w
-            for (int j = tid; j < N; j += blockDim.x) {
-                cplx y = cmul(Y[j], ph[j]);
-                cplx k = {y.y / vel, -y.x / vel};
+            for (int j = tid; j < N; j += SW_CONSUMERS) {
+                cplx w;
+                if (j < NT) { w = Y[j]; for (int q = 0; q < 8; ++q) { w.x -= part[q * NT + j].x; w.y -= part[q * NT + j].y; } }
+                else w = Wp[j - NT];
+                const cplx y = cmul(w, ph[j]);
+                const cplx k = {y.y / vel, -y.x / vel};
                 Kn[j] = k; Acc[j].x += wgt * k.x; Acc[j].y += wgt * k.y;
+                if (st == 3) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
             }
-            __syncthreads();
-            if (st == 3) {
-                for (int j = tid; j < N; j += blockDim.x) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; Kn[j] = {0.0, 0.0}; }
-                __syncthreads();
-            }
+            consumer_sync();
         }
     }
-    for (int j = tid; j < N; j += blockDim.x) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = C[j].x; dst[1] = C[j].y; }
-    if (a.drift && tid == 0) a.drift[t] = drift;
+    for (int j = tid; j < N; j += SW_CONSUMERS) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = C[j].x; dst[1] = C[j].y; }
+    if (track && tid == 0) a.drift[t] = drift;
 }
-
 }  // namespace
 
 int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s) {
@@ -330,24 +462,38 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
 int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStream_t s) {
     if (n_traj <= 0 || a.steps <= 0) return 0;
     const int N = a.NT + a.NP;
-    const size_t smem = ((size_t)6 * N + (size_t)8 * a.NT) * 16;
-    if (smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
-    WP_CUDA(cudaFuncSetAttribute(k_sweep2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t vec = ((size_t)6 * N + a.NP + (size_t)8 * a.NT) * 16;
+    // ring chunk: at least one row of H0 (16 N bytes), about 40 KB, so that four of them and the vectors fit 220 KB
+    size_t chunk = 40 * 1024;
+    while (chunk > (size_t)16 * N && SW_STAGES * chunk + vec > 220 * 1024) chunk -= 1024;
+    chunk = std::max(chunk, (size_t)16 * N);
+    chunk = (chunk + 127) & ~(size_t)127;
+    const size_t smem = SW_STAGES * chunk + vec;
+    if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
+    static size_t attr = 0;
+    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_sweep2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     wp_span_begin(B, FAM_SWEEP, s);
-    k_sweep2<<<n_traj, 256, smem, s>>>(a);
+    k_sweep2<<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;
 }
 
-int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_LU, int *d_piv, cudaStream_t s) {
+int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cudaStream_t s) {
     if (n_pos <= 0) return 0;
     FactorArgs a{};
-    a.K = d_K; a.LU = d_LU; a.piv = d_piv; a.status = B->d_status; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states;
-    const size_t need = (size_t)a.NP * a.NP * 16;
-    a.use_smem = need <= 200 * 1024;
-    const size_t smem = a.use_smem ? need : 0;
-    WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024)));
+    a.K = d_K; a.Ainv = d_Ainv; a.status = B->d_status; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states;
+    const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
+    const size_t budget = 200 * 1024;
+    a.use_smem = n * n * 16 + n * 9 * 16 + small <= budget;
+    const size_t fixed = (a.use_smem ? n * n * 16 : 0) + small;
+    int cw = (int)std::min<size_t>((budget - fixed) / (n * 16), (size_t)a.NT);
+    if (cw > 1 && (cw & 1) == 0) --cw;                        // odd width: conflict-free column reads
+    if (cw < 1) WP_FAIL(WPCCC_EINVAL, "factorisation: N_P = %d too large", a.NP);
+    a.cw = cw;
+    const size_t smem = fixed + n * cw * 16;
+    static size_t attr = 0;
+    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     wp_span_begin(B, FAM_FACT, s);
     k_factor<<<n_pos, 256, smem, s>>>(a);
     wp_span_end(B, s, 1);

@@ -23,8 +23,7 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
 struct Sweep2Args {          // two-centre: S = [[I, K^H], [K, I]], H full (eq. (1)-(4))
     const double *H;         // [traj][n_idx][N][N] complex, no time phase
     const double *K;         // [traj][n_idx][NP][NT] complex S_PT, no time phase
-    const double *LU;        // [traj][n_idx][NP][NP] complex LU factors of I - K K^H
-    const int *piv;          // [traj][n_idx][NP]
+    const double *Ainv;      // [traj][n_idx][NP][NP] complex (I - K K^H)^{-1}, row-major
     const int *st_rad_T, *st_rad_P; const double *eps_T, *eps_P;
     const double *v;
     double *C; double *drift;
