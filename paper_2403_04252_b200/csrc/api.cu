@@ -196,6 +196,7 @@ extern "C" int wpccc_matrix_elements(const wpccc_basis *Bc, int n_pos, const dou
     }
     cudaStream_t s = (cudaStream_t)stream;
     wp_timing_reset(B);
+    B->tab_zeroed = nullptr;
     const bool two = B->n_centres == 2;
     const int NT = B->c[0].n_states, NP = two ? B->c[1].n_states : 0, N = NT + NP;
     // block size from the workspace
@@ -263,6 +264,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
     if (!ws) WP_FAIL(WPCCC_ENOMEM, "workspace is NULL");
     cudaStream_t s = (cudaStream_t)stream, e = B->side, sw = B->hi;
     wp_timing_reset(B);
+    B->tab_zeroed = nullptr;
     const bool two = B->n_centres == 2;
     const double h = (z_max - z_min) / n_steps;
 

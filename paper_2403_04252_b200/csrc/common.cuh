@@ -43,7 +43,7 @@ struct CentreTab {
     int    *d_ent_pair = nullptr;  // [E]              pair row of entry e
     int    *d_ent_lookup = nullptr;// [lambda_max+1][n_rad][n_rad]  entry index of (lambda, a', a), -1 if not allowed
     double *d_G = nullptr;         // [(Lc+1)^2][(Lc+1)^2][lambda_max+1]  G^lambda_{(l'm'),(lm)} of eq. (6)
-    double *d_Ut = nullptr;        // [Nr+1][nf_pad]   row k: u_a(r_k) (a = 0..n_rad-1) then g_a(r_k)
+    double *d_Ut = nullptr;        // [Nr+1][nf_pad]   row k: pairs (u_a(r_k), g_a(r_k)), a = 0..n_rad-1
     int    *d_st_rad = nullptr, *d_st_l = nullptr, *d_st_m = nullptr;   // [n_states]
     double *d_eps = nullptr;       // [n_rad]
     int    *d_l = nullptr;         // [n_rad]
@@ -68,6 +68,7 @@ struct wpccc_basis {
     double *d_gl_rho = nullptr, *d_gl_phi = nullptr, *d_gl_zq = nullptr, *d_gl_zh = nullptr;  // GL x,w on [-1,1]: [2][n]
     int    *d_status = nullptr; // [4] device status word (0 ok; 1 zero pivot; 2 |S_PT| >= 1), position index
     char *arena = nullptr; size_t arena_bytes = 0;
+    const void *tab_zeroed = nullptr; size_t tab_zeroed_bytes = 0;   // node-table buffer whose padding columns are zero (per API call)
     // timing
     cudaStream_t side = nullptr;   // element kernels of wpccc_propagate
     cudaStream_t hi = nullptr;     // RK4 sweep of wpccc_propagate (highest priority: few CTAs, on the critical path)

@@ -119,7 +119,7 @@ int fill_centre_host(CentreTab &C, const wpccc_centre &in, int lambda_max) {
     C.q_off.push_back((int)C.col_rad.size());
     C.nqc = (int)C.col_rad.size();
     C.nqc_pad = (C.nqc + 7) / 8 * 8;
-    C.nf_pad = (2 * C.n_rad + 1) / 2 * 2;
+    C.nf_pad = 2 * C.n_rad;
     return 0;
 }
 
@@ -187,7 +187,7 @@ __global__ void k_pair_products(const double *Ut, int nf_pad, int n_rad, const d
     const int a = a1 + rem;
     for (int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < Kpad; kk += gridDim.x * blockDim.x) {
         double v = 0.0;
-        if (kk < Nr) { const double *row = Ut + (size_t)(kk + 1) * nf_pad; v = w[kk + 1] * row[a1] * row[a]; }
+        if (kk < Nr) { const double *row = Ut + (size_t)(kk + 1) * nf_pad; v = w[kk + 1] * row[2 * a1] * row[2 * a]; }
         PP[(size_t)pair * Kpad + kk] = v;
     }
 }
@@ -273,13 +273,13 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
         chk(upload(C.d_eps, C.eps, s)); chk(upload(C.d_l, C.l, s)); chk(upload(C.d_rad_first, C.rad_first, s));
         keep_i.emplace_back(C.col_rad); keep_i.back().resize(C.nqc_pad, -1); chk(upload(C.d_col_rad, keep_i.back(), s));
         keep_i.emplace_back(C.col_q); keep_i.back().resize(C.nqc_pad, 0); chk(upload(C.d_col_q, keep_i.back(), s));
-        // transposed radial table: row k = [u_0..u_{n-1}, g_0..g_{n-1}] at r_k
+        // transposed radial table: row k = [(u_0, g_0), (u_1, g_1), ...] at r_k
         keep_d.emplace_back((size_t)(Nr + 1) * C.nf_pad, 0.0);
         std::vector<double> &Ut = keep_d.back();
         for (int a = 0; a < C.n_rad; ++a)
             for (int k = 0; k <= Nr; ++k) {
-                Ut[(size_t)k * C.nf_pad + a] = centres[ci].u[(size_t)a * (Nr + 1) + k];
-                Ut[(size_t)k * C.nf_pad + C.n_rad + a] = centres[ci].g ? centres[ci].g[(size_t)a * (Nr + 1) + k] : 0.0;
+                Ut[(size_t)k * C.nf_pad + 2 * a] = centres[ci].u[(size_t)a * (Nr + 1) + k];
+                Ut[(size_t)k * C.nf_pad + 2 * a + 1] = centres[ci].g ? centres[ci].g[(size_t)a * (Nr + 1) + k] : 0.0;
             }
         chk(upload(C.d_Ut, Ut, s));
         if (!rc) {

@@ -100,6 +100,7 @@ __global__ void __launch_bounds__(128) k_tpos(const TposArgs a) {
 // Table of one side for one position, fragment-major for m8n8k4:  T[tile][ring][kc][c8][32] with
 //   column = tile*64 + c8*8 + lane/4,  z' node k = kc*4 + lane%4.
 // Columns: [X (nqc, padded to nq8) | Xh (nq8)], X = A (side 0, centre T) or B (side 1, centre P).
+// Padding columns are never written: the caller zeroes the table buffer once.
 struct TtabArgs {
     PosTabs L; const double *pos;            // per-position tables
     const double *R;
@@ -111,22 +112,23 @@ struct TtabArgs {
     int lmax[2];
 };
 
-// grid = (ring * n_kchunks, side, position), block = 256, dynamic smem.
+// grid = (ring * n_kchunks, side, position), block = 256, dynamic smem (per-node quantities only).
+// Phase 1: one thread per node: geometry, Lagrange weights, Theta~_{lq}.  Phase 2: a warp covers 4 nodes x 8
+// radial functions (lane = 4 * (a % 8) + node % 4, the fragment order), interpolates (u_a, g_a) with one 16-byte
+// load per stencil point and stores X, Xh for q = 0..l_a straight into the fragment-major table.
 __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     extern __shared__ __align__(16) double sm[];
     const int side = blockIdx.y, p = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nkch = a.L.n_z / a.KC, ring = blockIdx.x / nkch, k0 = (blockIdx.x % nkch) * a.KC, KC = a.KC;
-    const int ld = KC + 2, ncols = a.ntile[side] * 64, nq8 = a.nq8[side], lmax = a.lmax[side];
+    const int nq8 = a.nq8[side], lmax = a.lmax[side];
     const int nlq = (lmax + 1) * (lmax + 2) / 2;
-    double *tile = sm;                                   // [ncols][ld]
-    double *sLag = tile + (size_t)ncols * ld;            // [5][KC]
+    double *sLag = sm;                                   // [5][KC]
     double *sRinv = sLag + 5 * KC, *sPot = sRinv + KC;   // [KC] 1/r_side, -Z_other/r_other
     double *sTh = sPot + KC;                             // [nlq][KC]
     int *sJ = reinterpret_cast<int *>(sTh + (size_t)nlq * KC);   // [KC] stencil centre, -1 beyond r_max
     const double *pt = a.pos + (size_t)p * a.L.size();
     const double R = a.R[p];
 
-    for (int i = tid; i < ncols * ld; i += blockDim.x) tile[i] = 0.0;
     if (tid < KC) {
         const double rho = pt[a.L.off_rho() + ring], zk = pt[a.L.off_zq() + k0 + tid];
         const double zP = __dsub_rn(zk, R);
@@ -162,40 +164,37 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
         }
     }
     __syncthreads();
-    const double *Ut = a.Ut[side];
-    const int nr = a.n_rad[side], nf = a.nf_pad[side];
-    for (int n = warp; n < KC; n += 8) {
-        const int j = sJ[n];
-        if (j < 0) continue;
+    const double2 *Ut = reinterpret_cast<const double2 *>(a.Ut[side]);
+    const int nr = a.n_rad[side], nf2 = a.nf_pad[side] / 2;        // row stride in (u, g) pairs
+    const int ai = lane >> 2, kn = lane & 3, nkc = a.L.n_z / 4;
+    double *out = a.out[side] + (size_t)p * a.pos_stride[side];
+    const size_t tile_stride = (size_t)a.L.n_rho * nkc * 256;
+    for (int kcl = warp; kcl < KC / 4; kcl += 8) {
+        const int n = kcl * 4 + kn, j = sJ[n];
         const double L0 = sLag[n], L1 = sLag[KC + n], L2 = sLag[2 * KC + n], L3 = sLag[3 * KC + n], L4 = sLag[4 * KC + n];
         const double rinv = sRinv[n], pot = sPot[n];
-        const double *row = Ut + (size_t)(j - 2) * nf;
-        for (int aa = lane; aa < nr; aa += 32) {
-            double fu = L0 * row[aa]; double fg = L0 * row[nr + aa];
-            fu += L1 * row[nf + aa]; fg += L1 * row[nf + nr + aa];
-            fu += L2 * row[2 * nf + aa]; fg += L2 * row[2 * nf + nr + aa];
-            fu += L3 * row[3 * nf + aa]; fg += L3 * row[3 * nf + nr + aa];
-            fu += L4 * row[4 * nf + aa]; fg += L4 * row[4 * nf + nr + aa];
-            fu *= rinv; fg *= rinv;
+        double *dst = out + ((size_t)ring * nkc + (k0 / 4 + kcl)) * 256 + kn;
+        for (int aa = ai; aa < nr; aa += 8) {
+            double fu = 0.0, fg = 0.0;
+            if (j >= 0) {
+                const double2 *row = Ut + (size_t)(j - 2) * nf2 + aa;
+                const double2 v0 = row[0], v1 = row[nf2], v2 = row[2 * nf2], v3 = row[3 * nf2], v4 = row[4 * nf2];
+                fu = L0 * v0.x; fg = L0 * v0.y;
+                fu += L1 * v1.x; fg += L1 * v1.y;
+                fu += L2 * v2.x; fg += L2 * v2.y;
+                fu += L3 * v3.x; fg += L3 * v3.y;
+                fu += L4 * v4.x; fg += L4 * v4.y;
+                fu *= rinv; fg *= rinv;
+            }
             const int l = a.lrad[side][aa];
+            const int *cix = a.colidx[side] + aa * (WP_MAX_L + 1);
             for (int q = 0; q <= l; ++q) {
-                const int col = a.colidx[side][aa * (WP_MAX_L + 1) + q];
+                const int col = cix[q], colh = nq8 + col;
                 const double th = sTh[lq_index(l, q) * KC + n];
                 const double X = fu * th, Xg = fg * th;
-                tile[(size_t)col * ld + n] = X;
-                tile[(size_t)(nq8 + col) * ld + n] = pot * X + Xg;
+                dst[(size_t)(col >> 6) * tile_stride + (col & 63) * 4] = X;
+                dst[(size_t)(colh >> 6) * tile_stride + (colh & 63) * 4] = pot * X + Xg;
             }
-        }
-    }
-    __syncthreads();
-    // coalesced write-out in fragment order
-    double *out = a.out[side] + (size_t)p * a.pos_stride[side];
-    const int nkc = a.L.n_z / 4, kcs = KC / 4;
-    for (int t = 0; t < a.ntile[side]; ++t) {
-        double *dst = out + (((size_t)t * a.L.n_rho + ring) * nkc + k0 / 4) * 256;
-        for (int e = tid; e < kcs * 256; e += blockDim.x) {
-            const int kc = e >> 8, c8 = (e >> 5) & 7, ln = e & 31;
-            dst[e] = tile[(size_t)(t * 64 + c8 * 8 + (ln >> 2)) * ld + kc * 4 + (ln & 3)];
         }
     }
 }
@@ -371,13 +370,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------ rotation (a6)
+struct TrotChunk { int b0, b1, st0, nst, nrows; };   // radial functions [b0, b1) of centre P, their states, their body rows
 struct TrotArgs {
     const double *part; int n_split; int nq8T, nq8P;
     const double *theta;                     // [p] Theta = angle between R and v
     const int *radT, *lT_st, *mT_st;         // per target state: radial function, l, m
     const int *radP, *lP_st, *mP_st;         // per projectile state
     const int *colT, *colP;                  // [n_rad][WP_MAX_L+1] column of (a, |q|)
-    int NT, NP, lmax;
+    const int *lradP;                        // [n_rad_P] l of each projectile radial function
+    const TrotChunk *chunks; const int *rowbase;   // rowbase[b]: first local body row of radial function b inside its chunk
+    int NT, NP, lmax, max_rows;
     double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex
 };
 
@@ -393,14 +395,21 @@ __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
     return tot;
 }
 
-// grid = positions; block 256: one thread per lab-frame output element (product, beta, alpha), eq. (8):
+// grid = (chunk of projectile radial functions, product, position); block 256.  The body-frame rows the chunk needs
+// (both families, ring splits summed in order) are staged in shared memory with coalesced loads; then one thread per
+// lab-frame output element (beta, alpha), eq. (8):
 //   X_lab[beta, alpha] = sum_{q', q} d^{l_b}_{m_b q'}(Theta) d^{l_a}_{m_a q}(Theta) X_body[(b, q'), (a, q)],
 // where the signed body-frame element comes from the two q >= 0 families of the contraction:
 //   family (-) (weights Phi_{|q-q'|}) when q, q' have the same sign or one is 0, family (+) (Phi_{q+q'}) otherwise,
 //   times (-1)^q for q < 0 and (-1)^q' for q' < 0.
 __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
-    extern __shared__ double sd[];           // [lmax+1][W][W], W = 2 lmax + 1
-    const int p = blockIdx.x, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
+    extern __shared__ __align__(16) double sd[];     // [lmax+1][W][W] Wigner d, W = 2 lmax + 1; then body rows [2][max_rows][nq8T] complex
+    const int p = blockIdx.z, prod = blockIdx.y, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
+    const TrotChunk ch = a.chunks[blockIdx.x];
+    const int nd = ((L + 1) * W * W + 1) & ~1;
+    double2 *body = reinterpret_cast<double2 *>(sd + nd);
+    const int nq8T = a.nq8T;
+    const size_t blk = (size_t)a.nq8P * nq8T, fam_stride = (size_t)a.max_rows * nq8T;
     {
         double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
         for (int e = tid; e < (L + 1) * W * W; e += blockDim.x) {
@@ -408,32 +417,45 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
             sd[e] = (abs(mp) <= l && abs(m) <= l) ? wigner_d(l, mp, m, cb, sb) : 0.0;
         }
     }
+    // stage the rows (b, q'), b in [b0, b1), q' = 0..l_b: local row = rowbase[b] + q'
+    const double2 *part = reinterpret_cast<const double2 *>(a.part) + (size_t)p * a.n_split * 6 * blk;
+    {
+        // rows are enumerated per radial function; each row is nq8T contiguous complex numbers in each family
+        const int *cP = a.colP;
+        for (int b = ch.b0; b < ch.b1; ++b) {
+            const int nrow_b = a.lradP[b] + 1;
+            for (int e = tid; e < 2 * nrow_b * nq8T; e += blockDim.x) {
+                const int fam = e / (nrow_b * nq8T), r = (e / nq8T) % nrow_b, c = e % nq8T;
+                const double2 *src = part + ((size_t)fam * 3 + prod) * blk + (size_t)cP[b * (WP_MAX_L + 1) + r] * nq8T + c;
+                double2 v = {0.0, 0.0};
+                for (int sp = 0; sp < a.n_split; ++sp) { const double2 x = src[(size_t)sp * 6 * blk]; v.x += x.x; v.y += x.y; }
+                body[fam * fam_stride + (size_t)(a.rowbase[b] + r) * nq8T + c] = v;
+            }
+        }
+    }
     __syncthreads();
-    const int NT = a.NT, NP = a.NP, N = NT + NP, npair = NT * NP;
-    const size_t blk = (size_t)a.nq8P * a.nq8T;
-    const double *part = a.part + (size_t)p * a.n_split * 6 * blk * 2;
-    for (int e = tid; e < 3 * npair; e += blockDim.x) {
-        const int prod = e / npair, r = e - prod * npair;
+    const int NT = a.NT, NP = a.NP, N = NT + NP;
+    for (int e = tid; e < ch.nst * NT; e += blockDim.x) {
         // products 0, 1 are written row-major in (beta, alpha); product 2 (H_TP) in (alpha, beta): coalesced stores
-        const int ib = (prod < 2) ? r / NT : r % NP, ia = (prod < 2) ? r % NT : r / NP;
+        const int ibl = (prod < 2) ? e / NT : e % ch.nst, ia = (prod < 2) ? e % NT : e / ch.nst;
+        const int ib = ch.st0 + ibl;
         const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
         const int ra = a.radT[ia], la = a.lT_st[ia], ma = a.mT_st[ia];
         const double *dB = sd + (lb * W + mb + L) * W + L, *dA = sd + (la * W + ma + L) * W + L;
-        const int *cP = a.colP + rb * (WP_MAX_L + 1), *cT = a.colT + ra * (WP_MAX_L + 1);
+        const int *cT = a.colT + ra * (WP_MAX_L + 1);
+        const int row0 = a.rowbase[rb];
         double sr = 0.0, si = 0.0;
         for (int qp = -lb; qp <= lb; ++qp) {
             const int aqp = abs(qp);
-            const size_t rowoff = (size_t)cP[aqp] * a.nq8T;
+            const size_t rowoff = (size_t)(row0 + aqp) * nq8T;
             double tr = 0.0, ti = 0.0;
             for (int q = -la; q <= la; ++q) {
                 const int aq = abs(q);
                 const int fam = ((q >= 0) == (qp >= 0) || aq == 0 || aqp == 0) ? 0 : 1;
-                const double *src = part + (((size_t)fam * 3 + prod) * blk + rowoff + cT[aq]) * 2;
-                double xr = 0.0, xi = 0.0;
-                for (int s = 0; s < a.n_split; ++s) { xr += src[0]; xi += src[1]; src += 6 * blk * 2; }
-                int sg = (q < 0 ? aq : 0) + (qp < 0 ? aqp : 0);
+                const double2 x = body[fam * fam_stride + rowoff + cT[aq]];
+                const int sg = (q < 0 ? aq : 0) + (qp < 0 ? aqp : 0);
                 const double dav = (sg & 1) ? -dA[q] : dA[q];
-                tr += dav * xr; ti += dav * xi;
+                tr += dav * x.x; ti += dav * x.y;
             }
             sr += dB[qp] * tr; si += dB[qp] * ti;
         }
@@ -482,7 +504,8 @@ size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk) {
     TransferPlan P = make_plan(B, pick_split(B, n_pos_chunk));
     return P.per_pos_bytes() * (size_t)n_pos_chunk + P.tiles.size() * sizeof(int2) + 4096 +
            2 * (size_t)(B->c[0].n_rad + B->c[1].n_rad) * (WP_MAX_L + 1) * sizeof(int) +
-           2 * (size_t)(B->c[0].nqc_pad + B->c[1].nqc_pad) * sizeof(int);
+           2 * (size_t)(B->c[0].nqc_pad + B->c[1].nqc_pad) * sizeof(int) +
+           (size_t)B->c[1].n_rad * (sizeof(TrotChunk) + sizeof(int)) + 1024;
 }
 
 int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes) {
@@ -529,7 +552,38 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     int2 *d_tiles = (int2 *)take(P.tiles.size() * sizeof(int2));
     int *d_colidx[2], *d_qcol[2];
     for (int c = 0; c < 2; ++c) { d_colidx[c] = (int *)take((size_t)B->c[c].n_rad * (WP_MAX_L + 1) * 4); d_qcol[c] = (int *)take((size_t)B->c[c].nqc_pad * 4); }
+    // rotation chunks: consecutive projectile radial functions whose body rows (both families) fit ~100 KB of shared memory
+    const int lmx = std::max(B->c[0].l_max, B->c[1].l_max);
+    const size_t rot_nd = (((size_t)(lmx + 1) * (2 * lmx + 1) * (2 * lmx + 1) + 1) & ~(size_t)1) * 8;
+    std::vector<TrotChunk> rchunks; std::vector<int> rowbase(B->c[1].n_rad, 0);
+    int rot_max_rows = 0;
+    {
+        const CentreTab &C = B->c[1];
+        const int cap = std::max(C.l_max + 1, (int)((100 * 1024 - rot_nd) / (2 * (size_t)P.nq8[0] * 16)));
+        TrotChunk cur{0, 0, 0, 0, 0};
+        for (int b = 0; b < C.n_rad; ++b) {
+            if (cur.nrows + C.l[b] + 1 > cap) { rchunks.push_back(cur); cur = TrotChunk{b, b, C.rad_first[b], 0, 0}; }
+            rowbase[b] = cur.nrows; cur.nrows += C.l[b] + 1; cur.nst += 2 * C.l[b] + 1; cur.b1 = b + 1;
+        }
+        rchunks.push_back(cur);
+        for (auto &c : rchunks) rot_max_rows = std::max(rot_max_rows, c.nrows);
+    }
+    TrotChunk *d_rchunks = (TrotChunk *)take(rchunks.size() * sizeof(TrotChunk));
+    int *d_rowbase = (int *)take(rowbase.size() * sizeof(int));
     if (off > ws_bytes) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small");
+    WP_CUDA(cudaMemcpyAsync(d_rchunks, rchunks.data(), rchunks.size() * sizeof(TrotChunk), cudaMemcpyHostToDevice, s));
+    WP_CUDA(cudaMemcpyAsync(d_rowbase, rowbase.data(), rowbase.size() * sizeof(int), cudaMemcpyHostToDevice, s));
+    const size_t rot_smem = rot_nd + 2 * (size_t)rot_max_rows * P.nq8[0] * 16;
+    if (rot_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the rotation kernel's shared memory");
+    static size_t rot_attr = 0;
+    if (rot_smem > rot_attr) { WP_CUDA(cudaFuncSetAttribute(k_trot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem)); rot_attr = rot_smem; }
+    {   // padding columns of the node tables are never written by k_ttab: zero the buffer once per API call
+        const size_t tab_bytes = (size_t)((char *)d_part - (char *)d_tab[0]);
+        if (B->tab_zeroed != d_tab[0] || B->tab_zeroed_bytes != tab_bytes) {      // (the layout depends on the chunk size)
+            WP_CUDA(cudaMemsetAsync(d_tab[0], 0, tab_bytes, s));
+            B->tab_zeroed = d_tab[0]; B->tab_zeroed_bytes = tab_bytes;
+        }
+    }
     WP_CUDA(cudaMemcpyAsync(d_tiles, P.tiles.data(), P.tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, s));
     std::vector<int> hcol[2], hq[2];
     for (int c = 0; c < 2; ++c) {
@@ -541,22 +595,11 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         WP_CUDA(cudaMemcpyAsync(d_qcol[c], hq[c].data(), hq[c].size() * 4, cudaMemcpyHostToDevice, s));
     }
 
-    // node-table kernel configuration
-    int KC = P.L.n_z;
-    size_t tab_smem = 0;
-    const int lmx = std::max(B->c[0].l_max, B->c[1].l_max), nlq = (lmx + 1) * (lmx + 2) / 2;
-    const int maxcols = std::max(P.ntile[0], P.ntile[1]) * 64;
-    for (;; ) {
-        tab_smem = ((size_t)maxcols * (KC + 2) + (size_t)(7 + nlq) * KC) * 8 + (size_t)KC * 4 + 64;
-        if (tab_smem <= 200 * 1024 && KC <= 256) break;
-        // next smaller divisor of n_z that is a multiple of 4
-        int k2 = KC - 4;
-        while (k2 >= 4 && P.L.n_z % k2) k2 -= 4;
-        if (k2 < 4) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the node-table kernel");
-        KC = k2;
-    }
-    static size_t tab_attr = 0, con_attr = 0;
-    if (tab_smem > tab_attr) { WP_CUDA(cudaFuncSetAttribute(k_ttab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_smem)); tab_attr = tab_smem; }
+    // node-table kernel configuration: 64 z' nodes per CTA when n_z allows (n_z is a multiple of 16)
+    const int nlq = (lmx + 1) * (lmx + 2) / 2;
+    const int KC = (P.L.n_z % 64 == 0) ? 64 : ((P.L.n_z % 32 == 0) ? 32 : 16);
+    const size_t tab_smem = (size_t)(7 + nlq) * KC * 8 + (size_t)KC * 4 + 64;
+    static size_t con_attr = 0;
     const size_t con_smem = ((size_t)2 * TC_STAGES * TC_STAGE_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 1) * P.L.n_rho) * 8;
     if (con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
     if (con_smem > con_attr) { WP_CUDA(cudaFuncSetAttribute(k_tcon, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem)); con_attr = con_smem; }
@@ -596,7 +639,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
         tr.lmax = lmx; tr.K = d_K + (size_t)p0 * NP * NT * 2; tr.H = d_H + (size_t)p0 * N * N * 2;
         wp_span_begin(B, FAM_ROT, s);
-        k_trot<<<np, 256, (size_t)(lmx + 1) * (2 * lmx + 1) * (2 * lmx + 1) * sizeof(double), s>>>(tr);
+        tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
+        k_trot<<<dim3((unsigned)rchunks.size(), 3, np), 256, rot_smem, s>>>(tr);
         wp_span_end(B, s, 1);
         WP_CUDA(cudaGetLastError());
     }
