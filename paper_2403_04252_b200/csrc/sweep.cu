@@ -18,7 +18,7 @@
 
 namespace {
 
-struct cplx { double x, y; };
+struct __align__(16) cplx { double x, y; };
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
 __device__ __forceinline__ cplx cmulc(cplx a, cplx b) { return {a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y}; }  // a * conj(b)
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return {a.x + b.x, a.y + b.y}; }
@@ -130,13 +130,13 @@ __global__ void __launch_bounds__(256) k_sweep1(const Sweep1Args a) {
 }
 
 // ------------------------------------------------------------------ a7: Schur complement + inverse
-// grid = positions; block = 256.  A = I - K K^H (row-major, ld = NP) lives in shared memory when it fits, else in
+// grid = positions; block = 512.  A = I - K K^H (row-major, ld = NP) lives in shared memory when it fits, else in
 // the output buffer (global).  K is staged through shared memory in column chunks of odd width cw (conflict-free).
 // A^{-1} by in-place Gauss-Jordan elimination with partial (row) pivoting, first maximal |pivot| wins; the row
 // interchanges are undone as column interchanges in reverse order at the end.
 struct FactorArgs { const double *K; double *Ainv; int *status; int NT, NP, use_smem, cw; };
 
-__global__ void __launch_bounds__(256) k_factor(const FactorArgs a) {
+__global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
     extern __shared__ __align__(16) double sm[];
     const int n = a.NP, NT = a.NT, cw = a.cw, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const size_t p = blockIdx.x;
@@ -495,7 +495,7 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     static size_t attr = 0;
     if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     wp_span_begin(B, FAM_FACT, s);
-    k_factor<<<n_pos, 256, smem, s>>>(a);
+    k_factor<<<n_pos, 512, smem, s>>>(a);
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;

@@ -17,6 +17,8 @@
 //     only q, q' >= 0 columns are tabulated and contracted; the two families Phi_{|q-q'|} and Phi_{q+q'} of ring
 //     weights rebuild all sign combinations;
 //   * Phi^+_{-Delta} = conj(Phi^-_Delta) and the axial phases are conjugate, so H_TP shares the weights of S_PT.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
@@ -217,7 +219,7 @@ __device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigne
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int TC_THREADS = 256, TC_STAGES = 3, TC_KCS = 16;     // stage = 16 k4-groups = 64 z' nodes per operand
+constexpr int TC_STAGES = 3, TC_KCS = 16;     // stage = 16 k4-groups = 64 z' nodes per operand
 constexpr int TC_STAGE_DOUBLES = TC_KCS * 256;                  // per operand
 
 struct TconArgs {
@@ -230,14 +232,62 @@ struct TconArgs {
     double *part;                                                // [p][split][fam 2][prod 3][nq8P][nq8T] complex
 };
 
-// grid = (tile, ring split, position); block = 256 = 8 warps as 4 (rows) x 2 (cols); warp tile 16 x 32 complex.
-__global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
+// One stage (nk k4-groups of z' nodes) of a warp's 16 x 8 NJ complex tile: C += (B ck)^T A with the complex weight
+// ck = w_z e^{..} folded into the B fragments.  ALL: every 8 x 8 sub-tile is needed (no predicates in the loop);
+// FULL: nk == TC_KCS (fully unrolled, fragments of the next k4-group loaded while the current DMMAs issue).
+template <int NJ, bool ALL, bool FULL>
+__device__ __forceinline__ void tcon_stage(const double *Ab, const double *Bb, const double *ck, int nk, const bool (&need)[2][NJ],
+                                           double (&Cre)[2][NJ][2], double (&Cim)[2][NJ][2]) {
+    double af[2][NJ], bb[2][2], cc[2][2];
+    auto load = [&](int s, int kc) {
+        #pragma unroll
+        for (int j = 0; j < NJ; ++j) af[s][j] = Ab[kc * 256 + j * 32];
+        #pragma unroll
+        for (int i = 0; i < 2; ++i) bb[s][i] = Bb[kc * 256 + i * 32];
+        cc[s][0] = ck[8 * kc]; cc[s][1] = ck[8 * kc + 1];
+    };
+    auto mma = [&](int s) {
+        double br[2], bi[2];
+        #pragma unroll
+        for (int i = 0; i < 2; ++i) { br[i] = bb[s][i] * cc[s][0]; bi[i] = bb[s][i] * cc[s][1]; }
+        #pragma unroll
+        for (int i = 0; i < 2; ++i)
+            #pragma unroll
+            for (int j = 0; j < NJ; ++j)
+                if (ALL || need[i][j]) {
+                    dmma884(Cre[i][j][0], Cre[i][j][1], br[i], af[s][j]);
+                    dmma884(Cim[i][j][0], Cim[i][j][1], bi[i], af[s][j]);
+                }
+    };
+    if (FULL) {
+        load(0, 0);
+        #pragma unroll
+        for (int kc = 0; kc < TC_KCS; ++kc) {
+            if (kc + 1 < TC_KCS) load((kc + 1) & 1, kc + 1);
+            mma(kc & 1);
+        }
+    } else {
+        #pragma unroll 2
+        for (int kc = 0; kc < nk; ++kc) { load(0, kc); mma(0); }
+    }
+}
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// grid = (tile, ring split, position); block = 4 (rows) x 8/NJ (cols) warps; warp tile 16 x 8 NJ complex
+// (NJ = 4: 8 warps, NJ = 2: 16 warps).  Stages are released per warp through `empty` mbarriers (no block-wide
+// barrier in the main loop); thread 0 refills the buffer of stage st - 1 once it has finished stage st itself.
+template <int NJ>
+__global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
+    constexpr int WC = 8 / NJ, NW = 4 * WC, TC_THREADS = 32 * NW;
     extern __shared__ __align__(128) double sm[];
     double *sA = sm;                                          // [STAGES][TC_STAGE_DOUBLES]  A-side (mma "B" operand)
     double *sB = sA + TC_STAGES * TC_STAGE_DOUBLES;           // [STAGES][TC_STAGE_DOUBLES]  B-side (mma "A" operand)
     double *sCk = sB + TC_STAGES * TC_STAGE_DOUBLES;          // [n_z][2]
-    double *sRw = sCk + 2 * a.L.n_z;                          // [dmax+1][n_rho][2]
-    __shared__ __align__(8) unsigned long long bar[TC_STAGES];
+    double *sRw = sCk + 2 * a.L.n_z;                          // [dmax+2][n_rho][2], last row zero (weight of unused elements)
+    __shared__ __align__(8) unsigned long long bar[TC_STAGES], empty[TC_STAGES];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int p = blockIdx.z, split = blockIdx.y;
@@ -251,7 +301,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
 
     for (int i = tid; i < 2 * n_z; i += TC_THREADS) sCk[i] = pt[a.L.off_ck() + i];
     for (int i = tid; i < 2 * (a.L.dmax + 1) * n_rho; i += TC_THREADS) sRw[i] = pt[a.L.off_rw() + i];
-    if (tid == 0) { for (int s = 0; s < TC_STAGES; ++s) mbar_init(&bar[s], 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::); }
+    for (int i = tid; i < 2 * n_rho; i += TC_THREADS) sRw[2 * (a.L.dmax + 1) * n_rho + i] = 0.0;
+    if (tid == 0) { for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&bar[s], 1); mbar_init(&empty[s], NW); } asm volatile("fence.mbarrier_init.release.cluster;\n" ::); }
     __syncthreads();
 
     const double *gA = a.tabT + (size_t)p * a.strideT + (size_t)ct * n_rho * nkc * 256;
@@ -265,86 +316,75 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
     };
     if (tid == 0) for (int st = 0; st < min(TC_STAGES, n_st); ++st) issue(st);
 
-    const int wr = warp >> 1, wc = warp & 1;                  // warp rows 16*wr.., cols 32*wc..
+    const int wr = warp / WC, wc = warp % WC;                 // warp rows 16*wr.., cols 8*NJ*wc..
     const int fr = lane >> 2, fk = lane & 3;
-    // per-thread output bookkeeping: element (i, j, e): row = rt*64 + 16 wr + 8 i + fr, col = ct*64 + 32 wc + 8 j + 2 fk + e
+    // per-thread output bookkeeping: element (i, j, e): row = rt*64 + 16 wr + 8 i + fr, col = ct*64 + 8 NJ wc + 8 j + 2 fk + e
     // needed sub-tiles: not (Bh x Ah)
-    bool need[2][4];
+    bool need[2][NJ];
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int r8 = rt * 64 + 16 * wr + 8 * i, c8 = ct * 64 + 32 * wc + 8 * j;
+        for (int j = 0; j < NJ; ++j) {
+            const int r8 = rt * 64 + 16 * wr + 8 * i, c8 = ct * 64 + 8 * NJ * wc + 8 * j;
             need[i][j] = (r8 < 2 * a.nq8P) && (c8 < 2 * a.nq8T) && !(r8 >= a.nq8P && c8 >= a.nq8T);
         }
-    bool any_need = false;
+    bool any_need = false, all_need = true;
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
-        for (int j = 0; j < 4; ++j) any_need |= need[i][j];
+        for (int j = 0; j < NJ; ++j) { any_need |= need[i][j]; all_need &= need[i][j]; }
 
-    double Cre[2][4][2], Cim[2][4][2], Mre[2][4][2], Mim[2][4][2], Pre[2][4][2], Pim[2][4][2];
-    int dm[2][4][2], dp[2][4][2];
+    double Cre[2][NJ][2], Cim[2][NJ][2], Mre[2][NJ][2], Mim[2][NJ][2], Pre[2][NJ][2], Pim[2][NJ][2];
+    int dm[2][NJ][2], dp[2][NJ][2];                          // offsets of the ring-weight rows in sRw (zero row if unused)
+    unsigned okmask = 0;                                     // bit (i NJ + j) 2 + e: element is a wanted output
+    const int zrow = 2 * (a.L.dmax + 1) * n_rho;
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
-        for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < NJ; ++j)
             #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 Cre[i][j][e] = Cim[i][j][e] = Mre[i][j][e] = Mim[i][j][e] = Pre[i][j][e] = Pim[i][j][e] = 0.0;
-                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 32 * wc + 8 * j + 2 * fk + e;
+                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 8 * NJ * wc + 8 * j + 2 * fk + e;
                 int qp = -1, qq = -1;
                 if (gr < 2 * a.nq8P) qp = a.qP[gr % a.nq8P];
                 if (gc < 2 * a.nq8T) qq = a.qT[gc % a.nq8T];
                 const bool ok = need[i][j] && qp >= 0 && qq >= 0;
-                dm[i][j][e] = ok ? abs(qq - qp) : -1;
-                dp[i][j][e] = (ok && qp > 0 && qq > 0) ? qq + qp : -1;
+                if (ok) okmask |= 1u << ((i * NJ + j) * 2 + e);
+                dm[i][j][e] = ok ? 2 * abs(qq - qp) * n_rho : zrow;
+                dp[i][j][e] = (ok && qp > 0 && qq > 0) ? 2 * (qq + qp) * n_rho : zrow;
             }
 
     for (int st = 0; st < n_st; ++st) {
         const int buf = st % TC_STAGES, ring = ring0 + st / spr, kc0 = (st % spr) * TC_KCS, nk = min(TC_KCS, nkc - kc0);
         mbar_wait(&bar[buf], (st / TC_STAGES) & 1);
         if (any_need) {
-            const double *Ab = sA + buf * TC_STAGE_DOUBLES + (4 * wc) * 32 + lane;
+            const double *Ab = sA + buf * TC_STAGE_DOUBLES + (NJ * wc) * 32 + lane;
             const double *Bb = sB + buf * TC_STAGE_DOUBLES + (2 * wr) * 32 + lane;
             const double *ck = sCk + 2 * (kc0 * 4 + fk);
-            #pragma unroll 4
-            for (int kc = 0; kc < nk; ++kc) {
-                const double cr = ck[8 * kc], ci = ck[8 * kc + 1];
-                double af[4], br[2], bi[2];
-                #pragma unroll
-                for (int j = 0; j < 4; ++j) af[j] = Ab[kc * 256 + j * 32];
-                #pragma unroll
-                for (int i = 0; i < 2; ++i) { const double b = Bb[kc * 256 + i * 32]; br[i] = b * cr; bi[i] = b * ci; }
-                #pragma unroll
-                for (int i = 0; i < 2; ++i)
-                    #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        if (need[i][j]) {
-                            dmma884(Cre[i][j][0], Cre[i][j][1], br[i], af[j]);
-                            dmma884(Cim[i][j][0], Cim[i][j][1], bi[i], af[j]);
-                        }
-            }
+            if (all_need && nk == TC_KCS) tcon_stage<NJ, true, true>(Ab, Bb, ck, nk, need, Cre, Cim);
+            else if (all_need) tcon_stage<NJ, true, false>(Ab, Bb, ck, nk, need, Cre, Cim);
+            else tcon_stage<NJ, false, false>(Ab, Bb, ck, nk, need, Cre, Cim);
         }
-        __syncthreads();                                   // everyone is done with this buffer
-        if (tid == 0 && st + TC_STAGES < n_st) issue(st + TC_STAGES);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[buf]);           // this warp is done with the buffer
+        if (tid == 0 && st >= 1 && st - 1 + TC_STAGES < n_st) {
+            mbar_wait(&empty[(st - 1) % TC_STAGES], ((st - 1) / TC_STAGES) & 1);
+            issue(st - 1 + TC_STAGES);
+        }
         if ((st % spr) == spr - 1) {
-            // ring epilogue: acc(-) += w_rho rho Phi_{|q-q'|}(ring) C,  acc(+) += w_rho rho Phi_{q+q'}(ring) C
+            // ring epilogue (branch-free): acc(-) += w_rho rho Phi_{|q-q'|}(ring) C,  acc(+) += w_rho rho Phi_{q+q'}(ring) C
+            const double2 *rw = reinterpret_cast<const double2 *>(sRw) + ring;
             #pragma unroll
             for (int i = 0; i < 2; ++i)
                 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NJ; ++j)
                     #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const double cr = Cre[i][j][e], ci = Cim[i][j][e];
-                        if (dm[i][j][e] >= 0) {
-                            const double wr_ = sRw[2 * (dm[i][j][e] * n_rho + ring)], wi_ = sRw[2 * (dm[i][j][e] * n_rho + ring) + 1];
-                            Mre[i][j][e] += wr_ * cr - wi_ * ci; Mim[i][j][e] += wr_ * ci + wi_ * cr;
-                        }
-                        if (dp[i][j][e] >= 0) {
-                            const double wr_ = sRw[2 * (dp[i][j][e] * n_rho + ring)], wi_ = sRw[2 * (dp[i][j][e] * n_rho + ring) + 1];
-                            Pre[i][j][e] += wr_ * cr - wi_ * ci; Pim[i][j][e] += wr_ * ci + wi_ * cr;
-                        }
+                        const double2 wm = rw[dm[i][j][e] >> 1], wp = rw[dp[i][j][e] >> 1];
+                        Mre[i][j][e] += wm.x * cr - wm.y * ci; Mim[i][j][e] += wm.x * ci + wm.y * cr;
+                        Pre[i][j][e] += wp.x * cr - wp.y * ci; Pim[i][j][e] += wp.x * ci + wp.y * cr;
                         Cre[i][j][e] = 0.0; Cim[i][j][e] = 0.0;
                     }
         }
@@ -355,11 +395,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_tcon(const TconArgs a) {
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
-        for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < NJ; ++j)
             #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                if (dm[i][j][e] < 0) continue;
-                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 32 * wc + 8 * j + 2 * fk + e;
+                if (!((okmask >> ((i * NJ + j) * 2 + e)) & 1u)) continue;
+                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 8 * NJ * wc + 8 * j + 2 * fk + e;
                 const int hr = gr / a.nq8P, ir = gr % a.nq8P, hc = gc / a.nq8T, ic = gc % a.nq8T;
                 const int prod = hr ? 2 : (hc ? 1 : 0);
                 const size_t idx = ((size_t)prod * blk + (size_t)ir * a.nq8T + ic) * 2;
@@ -600,9 +640,14 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     const int KC = (P.L.n_z % 64 == 0) ? 64 : ((P.L.n_z % 32 == 0) ? 32 : 16);
     const size_t tab_smem = (size_t)(7 + nlq) * KC * 8 + (size_t)KC * 4 + 64;
     static size_t con_attr = 0;
-    const size_t con_smem = ((size_t)2 * TC_STAGES * TC_STAGE_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 1) * P.L.n_rho) * 8;
+    const size_t con_smem = ((size_t)2 * TC_STAGES * TC_STAGE_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho) * 8;
     if (con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
-    if (con_smem > con_attr) { WP_CUDA(cudaFuncSetAttribute(k_tcon, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem)); con_attr = con_smem; }
+    static const int tcon_nj = []() { const char *e = getenv("WPCCC_TCON_NJ"); return (e && atoi(e) == 2) ? 2 : 4; }();
+    if (con_smem > con_attr) {
+        WP_CUDA(cudaFuncSetAttribute(k_tcon<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+        WP_CUDA(cudaFuncSetAttribute(k_tcon<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+        con_attr = con_smem;
+    }
 
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
     for (int p0 = 0; p0 < n_pos; p0 += chunk) {
@@ -629,7 +674,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         tc.tiles = d_tiles; tc.n_tiles = (int)P.tiles.size(); tc.n_split = n_split; tc.part = d_part;
         dim3 gc((unsigned)P.tiles.size(), n_split, np);
         wp_span_begin(B, FAM_TCON, s);
-        k_tcon<<<gc, TC_THREADS, con_smem, s>>>(tc);
+        if (tcon_nj == 4) k_tcon<4><<<gc, 256, con_smem, s>>>(tc); else k_tcon<2><<<gc, 512, con_smem, s>>>(tc);
         wp_span_end(B, s, 1);
         WP_CUDA(cudaGetLastError());
 
