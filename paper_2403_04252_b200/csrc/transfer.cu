@@ -130,6 +130,8 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     int *sJ = reinterpret_cast<int *>(sTh + (size_t)nlq * KC);   // [KC] stencil centre, -1 beyond r_max
     const double *pt = a.pos + (size_t)p * a.L.size();
     const double R = a.R[p];
+    const int nkc = a.L.n_z / 4;
+    const int tile_stride = a.L.n_rho * nkc * 256;
 
     if (tid < KC) {
         const double rho = pt[a.L.off_rho() + ring], zk = pt[a.L.off_zq() + k0 + tid];
@@ -168,9 +170,8 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     __syncthreads();
     const double2 *Ut = reinterpret_cast<const double2 *>(a.Ut[side]);
     const int nr = a.n_rad[side], nf2 = a.nf_pad[side] / 2;        // row stride in (u, g) pairs
-    const int ai = lane >> 2, kn = lane & 3, nkc = a.L.n_z / 4;
+    const int ai = lane >> 2, kn = lane & 3;
     double *out = a.out[side] + (size_t)p * a.pos_stride[side];
-    const size_t tile_stride = (size_t)a.L.n_rho * nkc * 256;
     for (int kcl = warp; kcl < KC / 4; kcl += 8) {
         const int n = kcl * 4 + kn, j = sJ[n];
         const double L0 = sLag[n], L1 = sLag[KC + n], L2 = sLag[2 * KC + n], L3 = sLag[3 * KC + n], L4 = sLag[4 * KC + n];
@@ -190,12 +191,13 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
             }
             const int l = a.lrad[side][aa];
             const int *cix = a.colidx[side] + aa * (WP_MAX_L + 1);
+            const double *th_l = sTh + (size_t)lq_index(l, 0) * KC + n;
             for (int q = 0; q <= l; ++q) {
                 const int col = cix[q], colh = nq8 + col;
-                const double th = sTh[lq_index(l, q) * KC + n];
+                const double th = th_l[q * KC];
                 const double X = fu * th, Xg = fg * th;
-                dst[(size_t)(col >> 6) * tile_stride + (col & 63) * 4] = X;
-                dst[(size_t)(colh >> 6) * tile_stride + (colh & 63) * 4] = pot * X + Xg;
+                dst[(col >> 6) * tile_stride + (col & 63) * 4] = X;
+                dst[(colh >> 6) * tile_stride + (colh & 63) * 4] = pot * X + Xg;
             }
         }
     }
