@@ -1,0 +1,142 @@
+"""-m gpu: parity at the sizes of BASELINE.json configs[0..4] (rule-literal bases, SURVEY.md 8(d) "Parity protocol").
+
+T1 elements: the CUDA path evaluates a batch of positions large enough to use the launch configuration of the timed
+   run (whole-wave position chunks, several GEMM M-tiles with a ragged tail); sampled positions are compared
+   element by element with the oracle (1e-11 relative, 1e-13 absolute floor).
+T2 propagation: trajectories of each config on a window of RK4 steps of the configured size around closest approach
+   (full CPU trajectories of these configs take hours); amplitudes and probabilities to 1e-9 absolute.
+T3 the timed configuration itself (configs[1], all 16 trajectories x 1600 steps): invariants that hold at any size.
+"""
+import numpy as np
+import pytest
+
+from oracle import assemble, direct, observables
+from oracle import propagate as oprop
+from wpccc_inputs import build_config
+
+pytestmark = pytest.mark.gpu
+
+REL, FLOOR, PTOL = 1e-11, 1e-13, 1e-9
+_cache = {}
+
+
+def config(lib, idx):
+    """(problem, run, basis) of configs[idx]; configs[4] shares the basis of configs[2]."""
+    key = 2 if idx == 4 else idx
+    if key not in _cache:
+        prob, _ = build_config(key)
+        _cache[key] = (prob, lib.setup_basis(prob))
+    return _cache[key]
+
+
+def run_of(idx):
+    from wpccc_inputs.configs import CONFIGS
+    c = CONFIGS[idx]
+    return dict(b=np.asarray(c["b"], float), v=np.asarray(c["v"], float), z_min=c["z_min"], z_max=c["z_max"], n_steps=c["n_steps"])
+
+
+def assert_elements(got, ref, what):
+    err = np.abs(np.asarray(got) - np.asarray(ref))
+    tol = REL * np.abs(ref) + FLOOR
+    bad = err > tol
+    assert not bad.any(), "%s: %d of %d elements out of tolerance; worst |err| %.3e" % (what, bad.sum(), bad.size, err[bad].max())
+
+
+def sample_positions(run, n_total, picks, seed):
+    """n_total positions: the sampled (b, z) picks of the parity protocol first, then seeded filler positions drawn
+    from the config's own ranges (they make the batch span whole launch chunks; only the picks are compared)."""
+    rng = np.random.default_rng(seed)
+    b = np.concatenate([[p[0] for p in picks], rng.choice(run["b"], n_total - len(picks))])
+    z = np.concatenate([[p[1] for p in picks], rng.uniform(run["z_min"], run["z_max"], n_total - len(picks))])
+    v = np.full(n_total, float(run["v"][0]))
+    perm = rng.permutation(n_total)                 # the picks land anywhere in the batch (different chunks / tiles)
+    inv = np.argsort(perm)
+    return b[perm], z[perm], v[perm], inv[:len(picks)]
+
+
+@pytest.mark.parametrize("idx,n_total,n_picks", [(0, 300, 6), (1, 150, 6), (3, 40, 2), (2, 260, 2)])
+def test_T1_elements_at_config_size(lib, idx, n_total, n_picks):
+    prob, basis = config(lib, idx)
+    run = run_of(idx)
+    bs = run["b"]
+    picks = [(bs[0], -0.37), (bs[len(bs) // 2], 5.3), (bs[-1], -0.37), (bs[0], 5.3), (bs[len(bs) // 2], -0.37), (bs[-1], 5.3)][:n_picks]
+    b, z, v, where = sample_positions(run, n_total, picks, seed=100 + idx)
+    two = len(prob.centres) == 2
+    S, H = lib.matrix_elements(basis, b, z, v, phases=True, want_S=two)
+    for k, p in enumerate(where):
+        So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
+        assert_elements(H[p].cpu().numpy(), Ho, "configs[%d] H at pick %d (b=%.3g, z=%.3g)" % (idx, k, b[p], z[p]))
+        if two:
+            assert_elements(S[p].cpu().numpy(), So, "configs[%d] S at pick %d" % (idx, k))
+    del S, H
+
+
+def test_T1_radial_entries_config2(lib):
+    """The DMMA GEMM at configs[2]/[4] size (N_r = 8000, 15 428 entries) against the plain grid sum of eq. (7)."""
+    prob, basis = config(lib, 2)
+    run = run_of(2)
+    rng = np.random.default_rng(5)
+    n = 130                                                      # two M-tiles, ragged
+    b, z = rng.choice(run["b"], n), rng.uniform(-20.0, 20.0, n)
+    _, _, F = lib.matrix_elements(basis, b, z, np.ones(n), phases=False, want_S=False, want_H=False, want_F=True)
+    F = F.cpu().numpy()
+    ent = basis.radial_entries(0)
+    r = prob.h * np.arange(prob.Nr + 1)
+    for p in (0, 127, 129):
+        Fo = direct.radial_F_all(prob.centres[0], prob.w, r, float(np.hypot(b[p], z[p])), prob.lambda_max)
+        assert_elements(F[p], np.array([Fo[lam, a1, a] for (a1, a, lam) in ent]), "configs[2] F at position %d" % p)
+
+
+# (config, trajectory picks as (v index, b index), RK4 steps of the configured size around z = 0)
+T2 = [(0, [(0, 0), (0, 1), (0, 2), (0, 3)], 30), (1, [(0, 4), (0, 11)], 10), (4, [(5, 40)], 2), (3, [(0, 100)], 2)]
+
+
+@pytest.mark.parametrize("idx,picks,steps", T2)
+def test_T2_propagation_window_at_config_size(lib, idx, picks, steps):
+    prob, basis = config(lib, idx)
+    run = run_of(idx)
+    h = (run["z_max"] - run["z_min"]) / run["n_steps"]
+    z0, z1 = -0.5 * steps * h, 0.5 * steps * h
+    b = np.array([run["b"][ib] for _, ib in picks])
+    v = np.array([run["v"][iv] for iv, _ in picks])
+    Cg, drift = lib.propagate(basis, b, v, z0, z1, steps, track_norm=True)
+    Cg = Cg.cpu().numpy()
+    for t in range(len(b)):
+        co, do = oprop.propagate(prob, b[t], v[t], z0, z1, steps, track_norm=True)
+        assert np.abs(Cg[t] - co).max() < PTOL, (idx, t, np.abs(Cg[t] - co).max())
+        assert np.abs(np.abs(Cg[t]) ** 2 - np.abs(co) ** 2).max() < PTOL
+        assert abs(float(drift[t]) - do) < 1e-10 + 1e-3 * do
+    out = lib.probabilities(basis, lib._torch().as_tensor(Cg, device="cuda"))
+    Ps, Pnl, Pc = observables.probabilities(prob, Cg)
+    assert np.abs(out["P_nl"].cpu().numpy() - Pnl).max() < 1e-14
+
+
+def test_T3_timed_configuration_invariants(lib):
+    """configs[1] exactly as bench.py runs it: unitarity (c^H S c conserved), reflection symmetry
+    P_{l,m} = P_{l,-m} of both centres, total probability, at every one of the 16 trajectories."""
+    prob, basis = config(lib, 1)
+    run = run_of(1)
+    b, v = run["b"], np.full(len(run["b"]), run["v"][0])
+    C, drift = lib.propagate(basis, b, v, run["z_min"], run["z_max"], run["n_steps"], track_norm=True)
+    C, drift = C.cpu().numpy(), drift.cpu().numpy()
+    assert np.isfinite(C).all()
+    # c^H S c is conserved only as far as the quadrature satisfies the Galerkin identity: the configured 64 x 16 x 128
+    # rule is not converged (A11/A24: 2e-3 at small b, unchanged under step refinement, identical in the
+    # oracle -- test_T2 compares the drift itself with the oracle's)
+    assert drift.max() < 5e-3, drift
+    P = np.abs(C) ** 2
+    off = 0
+    for c in prob.centres:
+        states = c.states()
+        index = {s: off + i for i, s in enumerate(states)}
+        for (ir, l, m) in states:
+            if m > 0:
+                assert np.abs(P[:, index[(ir, l, m)]] - P[:, index[(ir, l, -m)]]).max() < 1e-12
+        off += len(states)
+    # c^H S c = 1 and S -> I at |z| = 40: total probability within the overlap tail
+    assert np.abs(P.sum(1) - 1.0).max() < 5e-3
+    out = lib.probabilities(basis, lib._torch().as_tensor(C, device="cuda"), b=b, vgroup=np.zeros(len(b), np.int32), n_vgroups=1)
+    Ps, Pnl, Pc = observables.probabilities(prob, C)
+    assert np.abs(out["P_class"].cpu().numpy() - Pc).max() < 1e-13
+    sig = observables.cross_sections(b, np.zeros(len(b), np.int32), Pnl, 1)
+    assert np.abs(out["sigma_nl"].cpu().numpy() - sig).max() < 1e-12 * max(1.0, np.abs(sig).max())
