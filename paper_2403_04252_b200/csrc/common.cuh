@@ -42,6 +42,10 @@ struct CentreTab {
     double *d_PP = nullptr;        // [n_pairs][Kpad]  w_k u_a'(r_k) u_a(r_k), k = 1..Nr (index k-1), zero padded
     int    *d_ent_pair = nullptr;  // [E]              pair row of entry e
     int    *d_ent_lookup = nullptr;// [lambda_max+1][n_rad][n_rad]  entry index of (lambda, a', a), -1 if not allowed
+    int    *d_pair_off = nullptr;  // [n_pairs+1]      first slot of pair (a' <= a) in the pair-major copy of F (slots: lambda ascending)
+    int    *d_ent_perm = nullptr;  // [E]              pair-major slot of entry e
+    int    *d_st_pack = nullptr;   // [n_states]       rad | l << 16 | (l*l + l + m) << 20
+    std::vector<int> pair_off, ent_perm, st_pack;
     double *d_G = nullptr;         // [(Lc+1)^2][(Lc+1)^2][lambda_max+1]  G^lambda_{(l'm'),(lm)} of eq. (6)
     double *d_Ut = nullptr;        // [Nr+1][nf_pad]   row k: pairs (u_a(r_k), g_a(r_k)), a = 0..n_rad-1
     int    *d_st_rad = nullptr, *d_st_l = nullptr, *d_st_m = nullptr;   // [n_states]

@@ -7,6 +7,8 @@
 //     from the r^lambda / r^-(lambda+1) tables; the N operand streams from the pair-product matrix in HBM/L2
 //     with cp.async double buffering.
 // a3  assembly  D_{alpha' alpha} = -Z sum_lambda (+-1)^lambda G^lambda_{alpha' alpha} P_lambda^{m'-m}(cos Theta) F_lambda
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace {
@@ -201,6 +203,70 @@ __global__ void __launch_bounds__(256) k_direct_assemble(const AsmArgs a) {
     else a.out[o] = val;
 }
 
+// Fast path of the assembly: a CTA keeps the pair offsets and the packed state labels in shared memory and loops over
+// positions; per position it stages F in pair-major order and the angular factors
+//     Ang[lambda][(l'm')][(lm)] = -Z (+-1)^lambda G^lambda_{(l'm'),(lm)} P_lambda^{m'-m}(cos Theta)
+// in shared memory, so that every output element is a short dot product of shared-memory operands and the
+// global stores are the only HBM traffic (coalesced rows of D).
+struct Asm2Args {
+    const double *G; const int *pair_off, *ent_perm, *st_pack;
+    const double *cosT; const double *F; double *out;
+    int n_rad, n_pairs, E, N, Lc, lambda_max, ldF, f_off, ld_out, complex_out, n_pos;
+    long long pos_stride;
+    double charge; int alt_sign;
+};
+
+__global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
+    extern __shared__ __align__(16) double sm2[];
+    const int L = a.lambda_max, ldp = 2 * L + 1, nlm = (a.Lc + 1) * (a.Lc + 1), tid = threadIdx.x, nt = blockDim.x;
+    double *sF = sm2;                                    // [E] pair-major
+    double *sAng = sF + ((a.E + 1) & ~1);                // [L+1][nlm][nlm]
+    double *sP = sAng + (size_t)(L + 1) * nlm * nlm;     // [(L+1)][2L+1]
+    int *sOff = reinterpret_cast<int *>(sP + (L + 1) * ldp + 1);   // [n_pairs]
+    int *sSt = sOff + a.n_pairs;                         // [N]
+    for (int i = tid; i < a.n_pairs; i += nt) sOff[i] = a.pair_off[i];
+    for (int i = tid; i < a.N; i += nt) sSt[i] = a.st_pack[i];
+    const int N = a.N, di = nt / N, dj = nt - di * N;
+    for (int p = blockIdx.x; p < a.n_pos; p += gridDim.x) {
+        __syncthreads();                                 // previous position done with sF / sAng
+        if (tid == 0) assoc_legendre_all(L, a.cosT[p], sP, ldp);
+        const double *Fp = a.F + (size_t)p * a.ldF + a.f_off;
+        for (int e = tid; e < a.E; e += nt) sF[a.ent_perm[e]] = Fp[e];
+        __syncthreads();
+        for (int e = tid; e < (L + 1) * nlm * nlm; e += nt) {
+            const int lam = e / (nlm * nlm), r = e - lam * nlm * nlm, lmi = r / nlm, lmj = r - lmi * nlm;
+            // (l, m) from the lm index: l = floor(sqrt(lm)), m = lm - l*l - l
+            int li = 0; while ((li + 1) * (li + 1) <= lmi) ++li;
+            int lj = 0; while ((lj + 1) * (lj + 1) <= lmj) ++lj;
+            const int mu = (lmi - li * li - li) - (lmj - lj * lj - lj);
+            double v = 0.0;
+            if (abs(mu) <= lam) {
+                v = a.G[((size_t)lmi * nlm + lmj) * (L + 1) + lam] * sP[lam * ldp + mu + L];
+                if (a.alt_sign && (lam & 1)) v = -v;
+                v *= -a.charge;
+            }
+            sAng[e] = v;
+        }
+        __syncthreads();
+        int i = tid / N, j = tid - i * N;
+        double *outp = a.out + (size_t)p * a.pos_stride * (a.complex_out ? 2 : 1);
+        for (int idx = tid; idx < N * N; idx += nt) {
+            const int si = sSt[i], sj = sSt[j];
+            const int ai = si & 0xffff, aj = sj & 0xffff, li = (si >> 16) & 15, lj = (sj >> 16) & 15;
+            const int alo = min(ai, aj), ahi = max(ai, aj);
+            const double *f = sF + sOff[alo * a.n_rad - alo * (alo - 1) / 2 + (ahi - alo)];
+            const int lam0 = abs(li - lj), lam1 = min(li + lj, L);
+            const double *ang = sAng + ((size_t)lam0 * nlm + (si >> 20)) * nlm + (sj >> 20);
+            double acc = 0.0;
+            for (int lam = lam0; lam <= lam1; lam += 2) { acc += ang[0] * f[0]; ang += 2 * nlm * nlm; ++f; }
+            const size_t o = (size_t)i * a.ld_out + j;
+            if (a.complex_out) *reinterpret_cast<double2 *>(outp + 2 * o) = make_double2(acc, 0.0);
+            else outp[o] = acc;
+            i += di; j += dj; if (j >= N) { j -= N; ++i; }
+        }
+    }
+}
+
 }  // namespace
 
 int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s) {
@@ -240,6 +306,27 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
     // eq. (6): target-centred states see the projectile charge; projectile-centred states see Z_T with (-1)^lambda (A15)
     a.charge = (c == 0) ? B->Z_proj : B->c[0].Z;
     a.alt_sign = (c == 1);
+    // fast path when the per-position operands fit shared memory
+    const int nlm = (C.l_max + 1) * (C.l_max + 1), L1 = B->lambda_max + 1;
+    const size_t smem2 = ((size_t)((C.E + 1) & ~1) + (size_t)L1 * nlm * nlm + (size_t)L1 * (2 * B->lambda_max + 1) + 1) * 8 +
+                         ((size_t)C.n_pairs + C.n_states) * 4 + 16;
+    if (smem2 <= 220 * 1024) {
+        Asm2Args b{};
+        b.G = C.d_G; b.pair_off = C.d_pair_off; b.ent_perm = C.d_ent_perm; b.st_pack = C.d_st_pack;
+        b.cosT = d_cos; b.F = d_F; b.out = d_out;
+        b.n_rad = C.n_rad; b.n_pairs = C.n_pairs; b.E = C.E; b.N = C.n_states; b.Lc = C.l_max; b.lambda_max = B->lambda_max; b.ldF = ldF;
+        b.f_off = a.f_off; b.ld_out = ld_out; b.complex_out = complex_out; b.n_pos = n_pos; b.pos_stride = pos_stride;
+        b.charge = a.charge; b.alt_sign = a.alt_sign;
+        static size_t attr2 = 0;
+        if (smem2 > attr2) { WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2)); attr2 = smem2; }
+        const int per_sm = smem2 <= 100 * 1024 ? 2 : 1;
+        const int threads = (C.n_states * C.n_states >= 64 * 1024) ? 1024 : 512;
+        wp_span_begin(B, FAM_DASM, s);
+        k_direct_assemble2<<<std::min(n_pos, 148 * per_sm), threads, smem2, s>>>(b);
+        wp_span_end(B, s, 1);
+        WP_CUDA(cudaGetLastError());
+        return 0;
+    }
     dim3 grid(n_pos, (C.n_states * C.n_states + 255) / 256);
     wp_span_begin(B, FAM_DASM, s);
     k_direct_assemble<<<grid, 256, 0, s>>>(a);

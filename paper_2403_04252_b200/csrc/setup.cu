@@ -110,6 +110,17 @@ int fill_centre_host(CentreTab &C, const wpccc_centre &in, int lambda_max) {
     }
     for (int lam = lambda_max + 1; lam < WP_MAX_LAMBDA + 2; ++lam) C.lam_off[lam] = (int)C.ent_a.size();
     C.E = (int)C.ent_a.size();
+    // pair-major slots of the entries (direct assembly stages F in this order): pair (a' <= a), then lambda ascending
+    C.pair_off.assign(C.n_pairs + 1, 0);
+    for (int e = 0; e < C.E; ++e) C.pair_off[C.ent_pair[e] + 1]++;
+    for (int q = 0; q < C.n_pairs; ++q) C.pair_off[q + 1] += C.pair_off[q];
+    C.ent_perm.assign(C.E, 0);
+    for (int e = 0; e < C.E; ++e) {
+        const int l1 = C.l[C.ent_a1[e]], l = C.l[C.ent_a[e]];
+        C.ent_perm[e] = C.pair_off[C.ent_pair[e]] + (C.ent_lam[e] - std::abs(l1 - l)) / 2;
+    }
+    C.st_pack.resize(C.n_states);
+    for (int i = 0; i < C.n_states; ++i) C.st_pack[i] = C.st_rad[i] | (C.st_l[i] << 16) | (lm_index(C.st_l[i], C.st_m[i]) << 20);
     // transfer columns (a, q >= 0) grouped by q
     C.col_rad.clear(); C.col_q.clear(); C.q_off.clear();
     for (int q = 0; q <= C.l_max; ++q) {
@@ -145,6 +156,7 @@ size_t layout(wpccc_basis &B, char *base) {
         C.d_ent_pair = bump.take<int>(C.E);
         C.d_ent_lookup = bump.take<int>((size_t)L1 * C.n_rad * C.n_rad);
         C.d_G = bump.take<double>((size_t)nlm * nlm * L1);
+        C.d_pair_off = bump.take<int>(C.n_pairs + 1); C.d_ent_perm = bump.take<int>(C.E); C.d_st_pack = bump.take<int>(C.n_states);
         C.d_Ut = bump.take<double>((size_t)(B.Nr + 1) * C.nf_pad);
         C.d_st_rad = bump.take<int>(C.n_states); C.d_st_l = bump.take<int>(C.n_states); C.d_st_m = bump.take<int>(C.n_states);
         C.d_eps = bump.take<double>(C.n_rad); C.d_l = bump.take<int>(C.n_rad); C.d_rad_first = bump.take<int>(C.n_rad);
@@ -168,7 +180,7 @@ int describe(wpccc_basis &B, int n_centres, const wpccc_centre *centres, int Nr,
     }
     B.n_tot = 0; B.E_tot = 0; B.tiles.clear();
     for (int ci = 0; ci < n_centres; ++ci) {
-        if (centres[ci].n_rad < 1 || !centres[ci].l || !centres[ci].eps || !centres[ci].u) { wp_set_error("centre %d: missing arrays", ci); return WPCCC_EINVAL; }
+        if (centres[ci].n_rad < 1 || centres[ci].n_rad > 60000 || !centres[ci].l || !centres[ci].eps || !centres[ci].u) { wp_set_error("centre %d: missing arrays", ci); return WPCCC_EINVAL; }
         if (fill_centre_host(B.c[ci], centres[ci], lambda_max)) { wp_set_error("centre %d: l out of range 0..%d", ci, WP_MAX_L); return WPCCC_EINVAL; }
         B.n_tot += B.c[ci].n_states; B.E_tot += B.c[ci].E;
         for (int lam = 0; lam <= lambda_max; ++lam) {
@@ -269,6 +281,7 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
         for (int e = 0; e < C.E; ++e) look[((size_t)C.ent_lam[e] * C.n_rad + C.ent_a1[e]) * C.n_rad + C.ent_a[e]] = e;
         chk(upload(C.d_ent_lookup, look, s));
         chk(upload(C.d_ent_pair, C.ent_pair, s));
+        chk(upload(C.d_pair_off, C.pair_off, s)); chk(upload(C.d_ent_perm, C.ent_perm, s)); chk(upload(C.d_st_pack, C.st_pack, s));
         chk(upload(C.d_st_rad, C.st_rad, s)); chk(upload(C.d_st_l, C.st_l, s)); chk(upload(C.d_st_m, C.st_m, s));
         chk(upload(C.d_eps, C.eps, s)); chk(upload(C.d_l, C.l, s)); chk(upload(C.d_rad_first, C.rad_first, s));
         keep_i.emplace_back(C.col_rad); keep_i.back().resize(C.nqc_pad, -1); chk(upload(C.d_col_rad, keep_i.back(), s));
