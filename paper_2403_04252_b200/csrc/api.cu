@@ -157,7 +157,7 @@ PropPlan plan_propagate(const wpccc_basis *B, int n_traj, int n_groups, int n_un
         P.tws = 0;
         P.fixed = 64 * 1024 + (size_t)n_traj * 64 + (size_t)n_units * sizeof(SweepUnit);
         P.per_idx_single = (size_t)n_groups * (6 * 8 + (size_t)B->E_tot * 8) + 4096;
-        P.per_idx_double = (size_t)n_groups * N * N * 8 + 4096;                                                       // real D^T
+        P.per_idx_double = (size_t)n_groups * N * (size_t)wp_sweep1_ld((int)N) * 8 + 4096;                                      // real D^T (even row stride)
     }
     return P;
 }
@@ -271,6 +271,8 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
     // one-centre: trajectories with the same b share every matrix (D^T depends on (b, z) only)
     std::vector<double> ub; std::vector<int> group_of(n_traj);
     std::vector<SweepUnit> units;
+    int nv = 1, rows_per_chunk = 1, ring_stages = 2;
+    const int ldD = wp_sweep1_ld(N);
     if (!two) {
         std::map<double, int> idx;
         std::vector<std::vector<int>> members;
@@ -280,8 +282,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
             group_of[t] = it->second; members[it->second].push_back(t);
         }
         // units of up to nv trajectories; nv limited by the sweep kernel's shared memory
-        int nv = SWEEP_NV;
-        while (nv > 1 && ((size_t)4 * nv * N + (size_t)nv * B->c[0].n_rad) * 16 > 200 * 1024) --nv;
+        wp_sweep1_plan(N, B->c[0].n_rad, &nv, &rows_per_chunk, &ring_stages);
         for (size_t g = 0; g < members.size(); ++g)
             for (size_t k = 0; k < members[g].size(); k += nv) {
                 SweepUnit u{}; u.group = (int)g; u.n = (int)std::min<size_t>(nv, members[g].size() - k);
@@ -309,7 +310,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         if (two) {
             d_H[k] = cv.take<double>(npos_max * N * N * 2); d_K[k] = cv.take<double>(npos_max * NP * NT * 2);
             d_LU[k] = cv.take<double>(npos_max * NP * NP * 2);
-        } else d_D[k] = cv.take<double>(npos_max * N * N);
+        } else d_D[k] = cv.take<double>(npos_max * N * ldD);
     }
     if (!cv.ok) WP_FAIL(WPCCC_ENOMEM, "workspace too small (internal plan mismatch)");
 
@@ -343,7 +344,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
             if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], e);
         } else {
             rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, e);
-            if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_D[buf], N, (long long)N * N, 0, e);
+            if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_D[buf], ldD, (long long)N * ldD, 0, e);
         }
         if (rc) break;
         WP_CUDA(cudaEventRecord(ev_elem[buf], e));
@@ -357,7 +358,7 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         } else {
             Sweep1Args a{};
             a.units = d_units; a.D = d_D[buf]; a.st_rad = B->c[0].d_st_rad; a.eps = B->c[0].d_eps; a.v = d_v; a.C = dC; a.drift = d_norm_drift;
-            a.N = N; a.n_rad = B->c[0].n_rad; a.n_idx = n_idx; a.steps = steps; a.i0 = i0; a.z_min = z_min; a.h = h;
+            a.N = N; a.n_rad = B->c[0].n_rad; a.n_idx = n_idx; a.ldD = ldD; a.nv = nv; a.rows_per_chunk = rows_per_chunk; a.ring_stages = ring_stages; a.steps = steps; a.i0 = i0; a.z_min = z_min; a.h = h;
             rc = wp_sweep_one_centre(B, (int)units.size(), a, sw);
         }
         if (rc) break;

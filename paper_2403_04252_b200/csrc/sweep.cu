@@ -30,98 +30,159 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 __device__ __forceinline__ double zpos(double z_min, double h, long long i) { return __dadd_rn(z_min, __dmul_rn(0.5 * (double)i, h)); }
 
-// ------------------------------------------------------------------ one-centre sweep
-// grid = units; block = 256.  Dynamic smem: C, A, X, Knew [nv][N] complex, ph [nv][n_rad] complex, red[8].
-__global__ void __launch_bounds__(256) k_sweep1(const Sweep1Args a) {
-    extern __shared__ __align__(16) double sm[];
-    const SweepUnit u = a.units[blockIdx.x];
-    const int N = a.N, nv = u.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
-    cplx *C = reinterpret_cast<cplx *>(sm);
-    cplx *Acc = C + SWEEP_NV * N;
-    cplx *X = Acc + SWEEP_NV * N;
-    cplx *Kn = X + SWEEP_NV * N;
-    cplx *ph = Kn + SWEEP_NV * N;               // [nv][n_rad]
-    __shared__ double red[SWEEP_NV][8];
-    double vel[SWEEP_NV];
-    for (int q = 0; q < SWEEP_NV; ++q) vel[q] = (q < nv) ? a.v[u.traj[q]] : 1.0;
+// ------------------------------------------------------------------ TMA / mbarrier helpers (both sweeps)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
+        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
 
+constexpr int SW_STAGES = 4;
+constexpr int SW_CONSUMERS = 256;
+
+// ------------------------------------------------------------------ one-centre sweep
+// grid = units (up to nv trajectories that share b, hence D); block = 8 consumer warps + 1 producer warp.
+// The real matrices D(z) do not depend on the amplitudes: the producer warp streams their rows through a
+// shared-memory ring with TMA bulk copies (running ahead across stages), the consumer warps do the GEMV for the nv
+// stage vectors at once.  Dynamic smem: ring, then C, Acc, X, Kn [nv][N] complex, ph [nv][n_rad] complex.
+__global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep1(const Sweep1Args a) {
+    extern __shared__ __align__(128) unsigned char smraw1[];
+    const SweepUnit u = a.units[blockIdx.x];
+    const int N = a.N, ld = a.ldD, nvm = a.nv, nv = u.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int rpc = a.rows_per_chunk, n_chunks = (N + rpc - 1) / rpc;
+    const size_t chunk_bytes = (size_t)rpc * ld * 8;
+    const int NS = a.ring_stages;
+    unsigned char *ring = smraw1;
+    cplx *C = reinterpret_cast<cplx *>(smraw1 + (size_t)NS * chunk_bytes);
+    cplx *Acc = C + nvm * N, *X = Acc + nvm * N, *Kn = X + nvm * N, *ph = Kn + nvm * N;   // ph [nv][n_rad]
+    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
+    __shared__ double red[SWEEP_NV][8];
+    if (tid == 0) {
+        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+    }
+    __syncthreads();
+    if (warp == SW_CONSUMERS / 32) {
+        if (lane != 0) return;
+        const long long total = (long long)a.steps * 4 * n_chunks;
+        for (long long g = 0; g < total; ++g) {
+            const int slot = (int)(g % NS); const long long use = g / NS;
+            if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
+            const int sst = (int)(g / n_chunks), q = (int)(g - (long long)sst * n_chunks), s = sst >> 2, st = sst & 3;
+            const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));
+            const int r0 = q * rpc, rows = min(rpc, N - r0);
+            const double *src = a.D + ((size_t)u.group * a.n_idx + li) * (size_t)N * ld + (size_t)r0 * ld;
+            const unsigned bytes = (unsigned)rows * ld * 8u;
+            mbar_expect_tx(&full[slot], bytes);
+            tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
+        }
+        return;
+    }
+    double vel[SWEEP_NV];
+    #pragma unroll
+    for (int q = 0; q < SWEEP_NV; ++q) vel[q] = (q < nv) ? a.v[u.traj[q]] : 1.0;
     for (int q = 0; q < nv; ++q)
-        for (int j = tid; j < N; j += blockDim.x) {
+        for (int j = tid; j < N; j += SW_CONSUMERS) {
             const double *src = a.C + ((size_t)u.traj[q] * N + j) * 2;
-            C[q * N + j] = {src[0], src[1]};
+            C[q * N + j] = {src[0], src[1]}; Acc[q * N + j] = {0.0, 0.0}; Kn[q * N + j] = {0.0, 0.0};
         }
     double drift[SWEEP_NV];
+    #pragma unroll
     for (int q = 0; q < SWEEP_NV; ++q) drift[q] = (a.drift && q < nv) ? a.drift[u.traj[q]] : 0.0;
-    __syncthreads();
-
+    consumer_sync();
     const double h = a.h;
+    long long g = 0;
     for (int s = 0; s < a.steps; ++s) {
-        for (int j = tid; j < nv * N; j += blockDim.x) { Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
-        __syncthreads();
         #pragma unroll 1
         for (int st = 0; st < 4; ++st) {
             const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));       // local half-step index of this stage
             const double alpha = (st == 0) ? 0.0 : (st == 3 ? h : 0.5 * h);
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
             const double z = zpos(a.z_min, h, a.i0 + li);
-            for (int j = tid; j < nv * a.n_rad; j += blockDim.x) {
-                int q = j / a.n_rad, r = j % a.n_rad;
+            for (int j = tid; j < nv * a.n_rad; j += SW_CONSUMERS) {
+                const int q = j / a.n_rad, r = j - q * a.n_rad;
                 double sn, cs; sincos(a.eps[r] * z / vel[q], &sn, &cs);
                 ph[j] = {cs, sn};
             }
-            __syncthreads();
+            consumer_sync();
             // X = P^H (C + alpha * Kn)
-            for (int j = tid; j < nv * N; j += blockDim.x) {
-                int q = j / N, col = j % N;
-                cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
+            for (int j = tid; j < nv * N; j += SW_CONSUMERS) {
+                const int q = j / N, col = j - q * N;
+                const cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
                 X[j] = cmulc(x, ph[q * a.n_rad + a.st_rad[col]]);
             }
-            __syncthreads();
-            const double *D = a.D + ((size_t)u.group * a.n_idx + li) * (size_t)N * N;
-            for (int row = warp; row < N; row += nw) {
-                const double *Dr = D + (size_t)row * N;
-                double sr[SWEEP_NV], si[SWEEP_NV];
-                #pragma unroll
-                for (int q = 0; q < SWEEP_NV; ++q) { sr[q] = 0.0; si[q] = 0.0; }
-                for (int col = lane; col < N; col += 32) {
-                    const double d = Dr[col];
+            consumer_sync();
+            for (int c = 0; c < n_chunks; ++c) {
+                const int slot = (int)(g % NS);
+                mbar_wait(&full[slot], (unsigned)((g / NS) & 1));
+                const double *buf = reinterpret_cast<const double *>(ring + (size_t)slot * chunk_bytes);
+                const int r0 = c * rpc, rows = min(rpc, N - r0);
+                for (int r = warp; r < rows; r += 8) {
+                    const double *Dr = buf + (size_t)r * ld;
+                    const int row = r0 + r;
+                    double sr[SWEEP_NV], si[SWEEP_NV];
                     #pragma unroll
-                    for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) { cplx x = X[q * N + col]; sr[q] += d * x.x; si[q] += d * x.y; }
-                }
-                #pragma unroll
-                for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) {
-                    double yr = warp_sum(sr[q]), yi = warp_sum(si[q]);
-                    if (lane == 0) {
-                        // k = -(i/v) P y
-                        cplx y = cmul({yr, yi}, ph[q * a.n_rad + a.st_rad[row]]);
-                        cplx k = {y.y / vel[q], -y.x / vel[q]};
-                        Kn[q * N + row] = k;
-                        Acc[q * N + row].x += wgt * k.x; Acc[q * N + row].y += wgt * k.y;
+                    for (int q = 0; q < SWEEP_NV; ++q) { sr[q] = 0.0; si[q] = 0.0; }
+                    for (int col = lane; col < N; col += 32) {
+                        const double d = Dr[col];
+                        #pragma unroll
+                        for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) { const cplx x = X[q * N + col]; sr[q] += d * x.x; si[q] += d * x.y; }
+                    }
+                    #pragma unroll
+                    for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) {
+                        const double yr = warp_sum(sr[q]), yi = warp_sum(si[q]);
+                        if (lane == 0) Kn[q * N + row] = {yr, yi};          // raw y = D x; finished below
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[slot]);
+                ++g;
             }
-            __syncthreads();
+            consumer_sync();
+            // k = -(i/v) P y, accumulate; after the fourth stage the RK4 combination
+            for (int j = tid; j < nv * N; j += SW_CONSUMERS) {
+                const int q = j / N, row = j - q * N;
+                const cplx y = cmul(Kn[j], ph[q * a.n_rad + a.st_rad[row]]);
+                const cplx k = {y.y / vel[q], -y.x / vel[q]};
+                Kn[j] = k;
+                Acc[j].x += wgt * k.x; Acc[j].y += wgt * k.y;
+                if (st == 3) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
+            }
+            consumer_sync();
         }
-        for (int j = tid; j < nv * N; j += blockDim.x) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; }
-        __syncthreads();
         if (a.drift) {
             for (int q = 0; q < nv; ++q) {
                 double part = 0.0;
-                for (int j = tid; j < N; j += blockDim.x) part += C[q * N + j].x * C[q * N + j].x + C[q * N + j].y * C[q * N + j].y;
+                for (int j = tid; j < N; j += SW_CONSUMERS) part += C[q * N + j].x * C[q * N + j].x + C[q * N + j].y * C[q * N + j].y;
                 part = warp_sum(part);
                 if (lane == 0) red[q][warp] = part;
             }
-            __syncthreads();
+            consumer_sync();
             for (int q = 0; q < nv; ++q) {
                 double tot = 0.0;
-                for (int w = 0; w < nw; ++w) tot += red[q][w];
+                for (int w = 0; w < 8; ++w) tot += red[q][w];
                 drift[q] = fmax(drift[q], fabs(tot - 1.0));
             }
-            __syncthreads();
+            consumer_sync();
         }
     }
     for (int q = 0; q < nv; ++q) {
-        for (int j = tid; j < N; j += blockDim.x) {
+        for (int j = tid; j < N; j += SW_CONSUMERS) {
             double *dst = a.C + ((size_t)u.traj[q] * N + j) * 2;
             dst[0] = C[q * N + j].x; dst[1] = C[q * N + j].y;
         }
@@ -234,30 +295,6 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
 //     y = H0 x;   y_P -= K y_T;   w_P = Ainv y_P;   w_T = y_T - K^H w_P;   k = -(i/v) P w.
 // The matrices do not depend on the amplitudes, so the producer warp streams them (rows of H0, K, Ainv, K again)
 // through a shared-memory ring with TMA bulk copies, running ahead of the consumers across stage boundaries.
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
-    asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
-        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
-
-constexpr int SW_STAGES = 4;
-constexpr int SW_CONSUMERS = 256;
-
 // Chunk schedule of one RK4 step: stages 0..3 each [H rows | K rows | Ainv rows | K rows], then (drift only) K rows.
 struct SweepSched {
     int N, NT, NP, rH, rK, rA, nH, nK, nA, per_stage, per_step;
@@ -447,13 +484,29 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
 }
 }  // namespace
 
+void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages) {
+    // ring of `stages` chunks of whole rows + 4 nv N + nv n_rad complex numbers within the 227 KB of a CTA;
+    // preferred: 8 rows per chunk (one per consumer warp), 3-4 stages, as many trajectories per unit as fit
+    const int ld = wp_sweep1_ld(N);
+    const size_t cap = 226 * 1024;
+    auto bytes = [&](int vv, int rr, int ss) { return (size_t)ss * rr * ld * 8 + ((size_t)4 * vv * N + (size_t)vv * n_rad) * 16; };
+    for (int v = SWEEP_NV; v >= 1; --v)
+        for (int rr : {16, 8})
+            for (int ss : {4, 3})
+                if (bytes(v, rr, ss) <= cap && (v >= 3 || rr == 8)) { *nv = v; *rows_per_chunk = rr; *stages = ss; return; }
+    int v = 1, rr = 8, ss = 2;
+    while (rr > 1 && bytes(v, rr, ss) > cap) --rr;
+    *nv = v; *rows_per_chunk = rr; *stages = ss;
+}
+
 int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s) {
     if (n_units <= 0 || a.steps <= 0) return 0;
-    const size_t smem = ((size_t)4 * SWEEP_NV * a.N + (size_t)SWEEP_NV * a.n_rad) * 16;
-    if (smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
-    WP_CUDA(cudaFuncSetAttribute(k_sweep1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + ((size_t)4 * a.nv * a.N + (size_t)a.nv * a.n_rad) * 16;
+    if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
+    static size_t attr = 0;
+    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_sweep1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     wp_span_begin(B, FAM_SWEEP, s);
-    k_sweep1<<<n_units, 256, smem, s>>>(a);
+    k_sweep1<<<n_units, SW_CONSUMERS + 32, smem, s>>>(a);
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;
