@@ -14,7 +14,7 @@
 namespace {
 
 constexpr int BM = 128, BN = 128, BK = 32, LDS_ = BK + 4;   // row stride 36 doubles: conflict-free fragment reads
-constexpr int GEMM_THREADS = 256;
+constexpr int GEMM_THREADS = 256, NSTG = 3;    // three k-chunks in flight, one block-wide barrier per chunk
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -42,8 +42,8 @@ struct GemmArgs {
 // grid: (m tiles, n tiles).  256 threads = 8 warps as 2 (M) x 4 (N); warp tile 64 x 32 -> 32 DMMA per k4 step.
 __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs a) {
     extern __shared__ __align__(16) double smem[];
-    double *As = smem;                         // [2][BM][LDS_]
-    double *Bs = smem + 2 * BM * LDS_;         // [2][BN][LDS_]
+    double *As = smem;                         // [NSTG][BM][LDS_]
+    double *Bs = smem + NSTG * BM * LDS_;      // [NSTG][BN][LDS_]
     __shared__ double sR[BM], sRp[BM], sRm[BM];
     __shared__ int sPair[BN];
 
@@ -101,13 +101,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs 
     const bool warp_active = (wn < t.cnt);
     const int fr = lane >> 2, fk = lane & 3;
 
-    load_B(0, 0); cp_async_commit();
-    gen_A(0, 0);
+    load_B(0, 0); cp_async_commit(); gen_A(0, 0);
+    if (nk > 1) { load_B(1, 1); gen_A(1, 1); }
+    cp_async_commit();
     for (int kc = 0; kc < nk; ++kc) {
-        const int buf = kc & 1;
-        if (kc + 1 < nk) { load_B(buf ^ 1, kc + 1); cp_async_commit(); gen_A(buf ^ 1, kc + 1); cp_async_wait<1>(); }
-        else cp_async_wait<0>();
-        __syncthreads();
+        const int buf = kc % NSTG;
+        cp_async_wait<1>();                    // this thread's copies of chunk kc have landed
+        __syncthreads();                       // chunk kc complete for everyone; buffer of chunk kc - 1 is free again
+        if (kc + 2 < nk) { load_B((kc + 2) % NSTG, kc + 2); gen_A((kc + 2) % NSTG, kc + 2); }
+        cp_async_commit();
         if (warp_active) {
             const double *Ab = As + buf * BM * LDS_ + (wm + fr) * LDS_ + fk;
             const double *Bb = Bs + buf * BN * LDS_ + (wn + fr) * LDS_ + fk;
@@ -124,7 +126,6 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs 
                     for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
             }
         }
-        __syncthreads();
     }
     if (!warp_active) return;
     const int colbase = a.cen_off[t.c] + a.lam_off[t.c][lam] + t.n0;
@@ -280,7 +281,7 @@ int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, in
         a.cen_off[c] = off; off += B->c[c].E;
     }
     a.rp = B->d_rp; a.rm = B->d_rm; a.rk = B->d_rk; a.R = d_R; a.F = d_F; a.ldF = ldF; a.n_pos = n_pos; a.Kpad = B->Kpad;
-    const size_t smem = (size_t)2 * (BM + BN) * LDS_ * sizeof(double);
+    const size_t smem = (size_t)NSTG * (BM + BN) * LDS_ * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         WP_CUDA(cudaFuncSetAttribute(k_direct_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
