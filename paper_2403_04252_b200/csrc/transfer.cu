@@ -426,12 +426,17 @@ struct TrotArgs {
 };
 
 // Wigner d^l_{m' m}(beta) = <l m'| e^{-i beta J_y} |l m>, Wigner's sum formula; cb = cos(beta/2), sb = sin(beta/2).
+__device__ __forceinline__ double ipow(double x, int n) {        // x^n, n >= 0, by repeated squaring
+    double r = 1.0;
+    while (n) { if (n & 1) r *= x; x *= x; n >>= 1; }
+    return r;
+}
 __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
     double tot = 0.0;
     const double num = sqrt(c_fact[l + m] * c_fact[l - m] * c_fact[l + mp] * c_fact[l - mp]);
     for (int k = max(0, m - mp); k <= min(l + m, l - mp); ++k) {
         const double den = c_fact[l + m - k] * c_fact[k] * c_fact[l - k - mp] * c_fact[k - m + mp];
-        double term = num / den * pow(cb, 2 * l - 2 * k + m - mp) * pow(sb, 2 * k - m + mp);
+        double term = num / den * ipow(cb, 2 * l - 2 * k + m - mp) * ipow(sb, 2 * k - m + mp);
         tot += ((k - m + mp) & 1) ? -term : term;
     }
     return tot;
@@ -460,19 +465,19 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
         }
     }
     // stage the rows (b, q'), b in [b0, b1), q' = 0..l_b: local row = rowbase[b] + q'
-    const double2 *part = reinterpret_cast<const double2 *>(a.part) + (size_t)p * a.n_split * 6 * blk;
+    __shared__ int s_rowsrc[256];                    // body row (column index of centre P) of each local row
+    for (int b = ch.b0 + tid; b < ch.b1; b += blockDim.x)
+        for (int r = 0; r <= a.lradP[b]; ++r) s_rowsrc[a.rowbase[b] + r] = a.colP[b * (WP_MAX_L + 1) + r];
+    __syncthreads();
     {
-        // rows are enumerated per radial function; each row is nq8T contiguous complex numbers in each family
-        const int *cP = a.colP;
-        for (int b = ch.b0; b < ch.b1; ++b) {
-            const int nrow_b = a.lradP[b] + 1;
-            for (int e = tid; e < 2 * nrow_b * nq8T; e += blockDim.x) {
-                const int fam = e / (nrow_b * nq8T), r = (e / nq8T) % nrow_b, c = e % nq8T;
-                const double2 *src = part + ((size_t)fam * 3 + prod) * blk + (size_t)cP[b * (WP_MAX_L + 1) + r] * nq8T + c;
-                double2 v = {0.0, 0.0};
-                for (int sp = 0; sp < a.n_split; ++sp) { const double2 x = src[(size_t)sp * 6 * blk]; v.x += x.x; v.y += x.y; }
-                body[fam * fam_stride + (size_t)(a.rowbase[b] + r) * nq8T + c] = v;
-            }
+        const double2 *part = reinterpret_cast<const double2 *>(a.part) + (size_t)p * a.n_split * 6 * blk;
+        const int per_fam = ch.nrows * nq8T;
+        for (int e = tid; e < 2 * per_fam; e += blockDim.x) {
+            const int fam = e >= per_fam, r2 = e - fam * per_fam, r = r2 / nq8T, c = r2 - r * nq8T;
+            const double2 *src = part + ((size_t)fam * 3 + prod) * blk + (size_t)s_rowsrc[r] * nq8T + c;
+            double2 v = {0.0, 0.0};
+            for (int sp = 0; sp < a.n_split; ++sp) { const double2 x = src[(size_t)sp * 6 * blk]; v.x += x.x; v.y += x.y; }
+            body[fam * fam_stride + (size_t)r * nq8T + c] = v;
         }
     }
     __syncthreads();
@@ -601,7 +606,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     int rot_max_rows = 0;
     {
         const CentreTab &C = B->c[1];
-        const int cap = std::max(C.l_max + 1, (int)((100 * 1024 - rot_nd) / (2 * (size_t)P.nq8[0] * 16)));
+        const int cap = std::min(256, std::max(C.l_max + 1, (int)((100 * 1024 - rot_nd) / (2 * (size_t)P.nq8[0] * 16))));
         TrotChunk cur{0, 0, 0, 0, 0};
         for (int b = 0; b < C.n_rad; ++b) {
             if (cur.nrows + C.l[b] + 1 > cap) { rchunks.push_back(cur); cur = TrotChunk{b, b, C.rad_first[b], 0, 0}; }
