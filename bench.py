@@ -123,7 +123,8 @@ def family_work(prob, b_local, n_steps):
         nqc = [int(sum(int(x) + 1 for x in c.l)) for c in prob.centres]
         nrad = [len(c.l) for c in prob.centres]
         out["transfer_contraction"] = ("tensor", 3 * 4.0 * nqc[0] * nqc[1] * nodes * n_pos, "flop")
-        out["transfer_tables"] = ("alu", (20.0 * (nrad[0] + nrad[1]) + 4.0 * (nqc[0] + nqc[1])) * nodes * n_pos, "flop")
+        # node tables: bound by the HBM write of X and Xh for every (column, node) of both sides
+        out["transfer_tables"] = ("hbm", 8.0 * 2 * (nqc[0] + nqc[1]) * nodes * n_pos, "byte")
         out["rotation"] = ("hbm", 16.0 * (3 * Nc[0] * Nc[1] + 6 * nqc[0] * nqc[1]) * n_pos, "byte")
         out["direct_assemble"] = ("hbm", 16.0 * (Nc[0] ** 2 + Nc[1] ** 2) * n_pos, "byte")
         out["factor"] = ("alu", (8.0 * Nc[1] ** 2 * Nc[0] + 8.0 / 3.0 * Nc[1] ** 3) * n_pos, "flop")
