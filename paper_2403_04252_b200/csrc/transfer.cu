@@ -455,8 +455,10 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     const TrotChunk ch = a.chunks[blockIdx.x];
     const int nd = ((L + 1) * W * W + 1) & ~1;
     double2 *body = reinterpret_cast<double2 *>(sd + nd);
-    const int nq8T = a.nq8T;
+    const int nq8T = a.nq8T, NT = a.NT;
     const size_t blk = (size_t)a.nq8P * nq8T, fam_stride = (size_t)a.max_rows * nq8T;
+    double2 *Ep = body + 2 * fam_stride, *Em = Ep + (size_t)a.max_rows * NT;      // [rows][NT] each
+    int *s_colT = reinterpret_cast<int *>(Em + (size_t)a.max_rows * NT);          // [NT][L+1] column of (a, q) per target state
     {
         double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
         for (int e = tid; e < (L + 1) * W * W; e += blockDim.x) {
@@ -465,9 +467,13 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
         }
     }
     // stage the rows (b, q'), b in [b0, b1), q' = 0..l_b: local row = rowbase[b] + q'
-    __shared__ int s_rowsrc[256];                    // body row (column index of centre P) of each local row
+    __shared__ int s_rowsrc[256], s_rowp[256];       // body row (column index of centre P) and q' of each local row
     for (int b = ch.b0 + tid; b < ch.b1; b += blockDim.x)
-        for (int r = 0; r <= a.lradP[b]; ++r) s_rowsrc[a.rowbase[b] + r] = a.colP[b * (WP_MAX_L + 1) + r];
+        for (int r = 0; r <= a.lradP[b]; ++r) { s_rowsrc[a.rowbase[b] + r] = a.colP[b * (WP_MAX_L + 1) + r]; s_rowp[a.rowbase[b] + r] = r; }
+    for (int e = tid; e < NT * (L + 1); e += blockDim.x) {
+        const int ia = e / (L + 1), q = e - ia * (L + 1);
+        s_colT[e] = (q <= a.lT_st[ia]) ? a.colT[a.radT[ia] * (WP_MAX_L + 1) + q] : 0;
+    }
     __syncthreads();
     {
         const double2 *part = reinterpret_cast<const double2 *>(a.part) + (size_t)p * a.n_split * 6 * blk;
@@ -481,30 +487,45 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
         }
     }
     __syncthreads();
-    const int NT = a.NT, NP = a.NP, N = NT + NP;
+    // stage 1: contract the target-side index.  For body row (b, p = |q'|) and target state alpha = (a, m_a):
+    //   P0 = sum_{q>=0} d^{l_a}_{m_a,q} F0[q],  M0 = sum_{q>0} (-1)^q d_{m_a,-q} F0[q],  P1, M1 the same with family (+),
+    //   E+ = P0 + (p == 0 ? M0 : M1)            (q' = +p),      E- = (-1)^p (d_{m_a,0} F0[0] + P1 + M0)   (q' = -p < 0)
+    for (int e = tid; e < ch.nrows * NT; e += blockDim.x) {
+        const int r = e / NT, ia = e - r * NT, pq = s_rowp[r];
+        const int la = a.lT_st[ia], ma = a.mT_st[ia];
+        const double *dA = sd + (la * W + ma + L) * W + L;
+        const double2 *f0 = body + (size_t)r * nq8T, *f1 = f0 + fam_stride;
+        const int *ct = s_colT + ia * (L + 1);
+        const double2 x00 = f0[ct[0]];
+        const double d0 = dA[0];
+        double2 P0 = {d0 * x00.x, d0 * x00.y}, M0 = {0.0, 0.0}, P1 = {0.0, 0.0}, M1 = {0.0, 0.0};
+        const double2 Z0 = P0;
+        for (int q = 1; q <= la; ++q) {
+            const int c = ct[q];
+            const double dp = dA[q], dm = (q & 1) ? -dA[-q] : dA[-q];
+            const double2 x0 = f0[c], x1 = f1[c];
+            P0.x += dp * x0.x; P0.y += dp * x0.y; M0.x += dm * x0.x; M0.y += dm * x0.y;
+            P1.x += dp * x1.x; P1.y += dp * x1.y; M1.x += dm * x1.x; M1.y += dm * x1.y;
+        }
+        const double2 mm = (pq == 0) ? M0 : M1;
+        const double sg = (pq & 1) ? -1.0 : 1.0;
+        Ep[e] = {P0.x + mm.x, P0.y + mm.y};
+        Em[e] = {sg * (Z0.x + P1.x + M0.x), sg * (Z0.y + P1.y + M0.y)};
+    }
+    __syncthreads();
+    // stage 2: contract the projectile-side index
+    const int NP = a.NP, N = NT + NP;
     for (int e = tid; e < ch.nst * NT; e += blockDim.x) {
         // products 0, 1 are written row-major in (beta, alpha); product 2 (H_TP) in (alpha, beta): coalesced stores
         const int ibl = (prod < 2) ? e / NT : e % ch.nst, ia = (prod < 2) ? e % NT : e / ch.nst;
         const int ib = ch.st0 + ibl;
         const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
-        const int ra = a.radT[ia], la = a.lT_st[ia], ma = a.mT_st[ia];
-        const double *dB = sd + (lb * W + mb + L) * W + L, *dA = sd + (la * W + ma + L) * W + L;
-        const int *cT = a.colT + ra * (WP_MAX_L + 1);
-        const int row0 = a.rowbase[rb];
-        double sr = 0.0, si = 0.0;
-        for (int qp = -lb; qp <= lb; ++qp) {
-            const int aqp = abs(qp);
-            const size_t rowoff = (size_t)(row0 + aqp) * nq8T;
-            double tr = 0.0, ti = 0.0;
-            for (int q = -la; q <= la; ++q) {
-                const int aq = abs(q);
-                const int fam = ((q >= 0) == (qp >= 0) || aq == 0 || aqp == 0) ? 0 : 1;
-                const double2 x = body[fam * fam_stride + rowoff + cT[aq]];
-                const int sg = (q < 0 ? aq : 0) + (qp < 0 ? aqp : 0);
-                const double dav = (sg & 1) ? -dA[q] : dA[q];
-                tr += dav * x.x; ti += dav * x.y;
-            }
-            sr += dB[qp] * tr; si += dB[qp] * ti;
+        const double *dB = sd + (lb * W + mb + L) * W + L;
+        const double2 *ep = Ep + (size_t)a.rowbase[rb] * NT + ia, *em = Em + (size_t)a.rowbase[rb] * NT + ia;
+        double sr = dB[0] * ep[0].x, si = dB[0] * ep[0].y;
+        for (int pq = 1; pq <= lb; ++pq) {
+            const double2 xp = ep[pq * NT], xm = em[pq * NT];
+            sr += dB[pq] * xp.x + dB[-pq] * xm.x; si += dB[pq] * xp.y + dB[-pq] * xm.y;
         }
         double *o;
         if (prod == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
@@ -606,7 +627,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     int rot_max_rows = 0;
     {
         const CentreTab &C = B->c[1];
-        const int cap = std::min(256, std::max(C.l_max + 1, (int)((100 * 1024 - rot_nd) / (2 * (size_t)P.nq8[0] * 16))));
+        const size_t rot_fixed = rot_nd + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
+        const int cap = std::min(256, std::max(C.l_max + 1, (int)((100 * 1024 - rot_fixed) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
         TrotChunk cur{0, 0, 0, 0, 0};
         for (int b = 0; b < C.n_rad; ++b) {
             if (cur.nrows + C.l[b] + 1 > cap) { rchunks.push_back(cur); cur = TrotChunk{b, b, C.rad_first[b], 0, 0}; }
@@ -620,7 +642,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     if (off > ws_bytes) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small");
     WP_CUDA(cudaMemcpyAsync(d_rchunks, rchunks.data(), rchunks.size() * sizeof(TrotChunk), cudaMemcpyHostToDevice, s));
     WP_CUDA(cudaMemcpyAsync(d_rowbase, rowbase.data(), rowbase.size() * sizeof(int), cudaMemcpyHostToDevice, s));
-    const size_t rot_smem = rot_nd + 2 * (size_t)rot_max_rows * P.nq8[0] * 16;
+    const size_t rot_smem = rot_nd + 2 * (size_t)rot_max_rows * ((size_t)P.nq8[0] + B->c[0].n_states) * 16 + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
     if (rot_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the rotation kernel's shared memory");
     static size_t rot_attr = 0;
     if (rot_smem > rot_attr) { WP_CUDA(cudaFuncSetAttribute(k_trot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem)); rot_attr = rot_smem; }
