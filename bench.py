@@ -153,8 +153,14 @@ def run_ours(args):
     b_all, v_all, vg_all = run["b"], run["v"], run["vgroup"]
     b, v = b_all[mine], v_all[mine]
     n_steps, z0, z1 = run["n_steps"], run["z_min"], run["z_max"]
+    if args.window_steps:                                                  # not the headline: a window of the configured step size around z = 0
+        hz = (z1 - z0) / n_steps
+        n_steps = int(args.window_steps)
+        z0, z1 = -0.5 * n_steps * hz, 0.5 * n_steps * hz
     n_vg = int(vg_all.max()) + 1
     basis = wp.setup_basis(prob)
+    if args.direct_tables:
+        basis.enable_direct_tables(True)
     N = basis.n_tot
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
@@ -234,6 +240,8 @@ def run_ours(args):
     pk = measured_peaks()
     dmma, dfma = wp.fp64_peak(1), wp.fp64_peak(0)
     work = family_work(prob, b, n_steps)
+    if args.direct_tables:                                                 # NEXT-1: 16 B read + 8 B written per entry and position
+        work["direct_gemm"] = ("hbm", work["direct_gemm"][1] / (2.0 * prob.Nr) * 24.0, "byte")
     fams = {}
     for k, (ms, n) in fam_ms.items():
         if n == 0 or k not in work:
@@ -264,9 +272,10 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": "BASELINE.json configs[%d]: %s, N_tot=%d states, %d trajectories x %d RK4 steps per step%s" % (
                        args.config, "two-centre p+H with electron transfer, quadrature %dx%dx%d" % (prob.quad["n_rho"], prob.quad["n_phi"], prob.quad["n_z"]) if prob.quad else "one-centre",
-                       N, len(b_all), n_steps, " (%d per rank)" % len(b) if world > 1 else ""),
+                       N, len(b_all), n_steps, (" (%d per rank)" % len(b) if world > 1 else "") + (" [window of the configured step size around z = 0, not the full z-range]" if args.window_steps else "")),
                    "l2": "512 MiB buffer written between timed iterations (L2 flush); window buffers of one step are several GB >> L2",
-                   "parallelism": "dp%d over impact parameters" % world},
+                   "parallelism": "dp%d over impact parameters" % world,
+                   "direct": "prefix/suffix tables (NEXT-1)" if args.direct_tables else "DMMA GEMM"},
         "matrix_elements_per_s": round(elems_per_pos * len(b_all) * (2 * n_steps + 1) / (ms_step * 1e-3), 1),
         "clocks": clocks,
         "e2e": {"value": round(e2e_val, 3), "unit": "trajectory*steps/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
@@ -337,8 +346,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--cpu-steps", type=int, default=5, help="RK4 steps of the cpu_baseline sample")
+    ap.add_argument("--cpu-steps", type=int, default=16, help="RK4 steps of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--direct-tables", action="store_true", help="SURVEY.md 8(f) NEXT-1: radial sums from prefix/suffix tables instead of the DMMA GEMM (family direct_gemm then counts HBM bytes)")
+    ap.add_argument("--window-steps", type=int, default=0, help="propagate only this many RK4 steps (configured step size) around z = 0; for configs whose full run takes many minutes")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -104,6 +104,19 @@ int wpccc_radial_entry(const wpccc_basis *basis, int c, int e, int *a_prime, int
  * windows); what = 2: the minimum wpccc_propagate accepts. */
 size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, int what);
 
+/* ---- a2 alternative: tabulated direct couplings (the paper's own route, in exact form)
+ * V_lambda(r, R) = min^lambda / max^(lambda+1) separates at r = R, so the grid sum of eq. (7) is
+ *   F^c_lambda(a', a; R) = R^-(lambda+1) P_e[g] + R^lambda Q_e[g],   g = #{k : r_k < R},
+ *   P_e[g] = sum_{k <= g} w_k u_a' u_a r_k^lambda,   Q_e[g] = sum_{k > g} w_k u_a' u_a r_k^-(lambda+1):
+ * the same discrete sum as the GEMM of wpccc_matrix_elements / wpccc_propagate (up to rounding order), at 24 bytes of
+ * HBM traffic per entry and position instead of 2 N_r flops.
+ * wpccc_direct_table_bytes: bytes of the table [g = 0..N_r][entry] of (P, Q) pairs for this basis.
+ * wpccc_enable_direct_tables: builds the tables in `dev_tables` [device, 256-byte aligned, caller-owned, must stay
+ *   valid while enabled] and makes every later call on this handle use them instead of the GEMM; dev_tables == NULL
+ *   switches back to the GEMM.  Synchronises `stream`.  Errors: WPCCC_EINVAL, WPCCC_ENOMEM (bytes too small). */
+size_t wpccc_direct_table_bytes(const wpccc_basis *basis);
+int wpccc_enable_direct_tables(wpccc_basis *basis, void *dev_tables /*[device] or NULL*/, size_t bytes, void *stream);
+
 /* ---- a1-a6: matrix elements at given positions ------------------------------------------------
  * For each position p (b[p], z[p], v[p]) [host arrays] computes
  *   S = [[I, S_PT^H], [S_PT, I]],  H = [[D^T, H_TP], [H_PT, D^P]]            (eq. (1); A1)

@@ -73,13 +73,17 @@ _lib.wpccc_last_timing.restype = C.c_int
 _lib.wpccc_last_timing.argtypes = [_vp, _dp, C.POINTER(C.c_longlong)]
 _lib.wpccc_fp64_peak.restype = C.c_double
 _lib.wpccc_fp64_peak.argtypes = [C.c_int, _vp]
+_lib.wpccc_direct_table_bytes.restype = C.c_size_t
+_lib.wpccc_direct_table_bytes.argtypes = [_vp]
+_lib.wpccc_enable_direct_tables.restype = C.c_int
+_lib.wpccc_enable_direct_tables.argtypes = [_vp, _vp, C.c_size_t, _vp]
 _lib.wpccc_last_error.restype = C.c_char_p
 _lib.wpccc_version.restype = C.c_char_p
 
 EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
            "wpccc_matrix_elements", "wpccc_propagate", "wpccc_probabilities", "wpccc_last_timing", "wpccc_fp64_peak",
-           "wpccc_last_error", "wpccc_version")
+           "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
 
 
 def version() -> str:
@@ -167,6 +171,19 @@ class Basis:
             self.close()
         except Exception:
             pass
+
+    def enable_direct_tables(self, on: bool = True):
+        """wpccc_enable_direct_tables: evaluate the radial sums of eq. (7) from prefix/suffix tables
+        instead of the DMMA GEMM; the table tensor is owned by this handle.  on=False switches back to the GEMM."""
+        torch = _torch()
+        if not on:
+            _check(_lib.wpccc_enable_direct_tables(self._h, None, 0, _stream(torch)))
+            self._dtab = None
+            return
+        nbytes = _lib.wpccc_direct_table_bytes(self._h)
+        self._dtab = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        base = (self._dtab.data_ptr() + 255) & ~255
+        _check(_lib.wpccc_enable_direct_tables(self._h, C.c_void_p(base), nbytes, _stream(torch)))
 
     def radial_entries(self, c):
         """[(a', a, lambda)] of the radial entries F^c_lambda(a', a) in output order."""

@@ -69,6 +69,8 @@ struct wpccc_basis {
     double *d_rm = nullptr;    // [lambda_max+1][Kpad] r_k^-(lambda+1)
     double *d_rk = nullptr;    // [Kpad] r_k (0 in the padding)
     GemmTile *d_tiles = nullptr;
+    int *d_ent_lam = nullptr;   // [E_tot] multipole of every radial entry (both centres)
+    double2 *d_dtab = nullptr;  // [Nr+1][E_tot] (P_e[g], Q_e[g]) prefix/suffix sums of eq. (7), caller-owned; nullptr: GEMM
     double *d_gl_rho = nullptr, *d_gl_phi = nullptr, *d_gl_zq = nullptr, *d_gl_zh = nullptr;  // GL x,w on [-1,1]: [2][n]
     int    *d_status = nullptr; // [4] device status word (0 ok; 1 zero pivot; 2 |S_PT| >= 1), position index
     char *arena = nullptr; size_t arena_bytes = 0;

@@ -268,10 +268,85 @@ __global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
     }
 }
 
+// ---- a2 alternative: prefix / suffix tables of the grid sum of eq. (7)
+// T[g][e] = (P_e[g], Q_e[g]),  P_e[g] = sum_{k=1..g} PP_e[k] r_k^lambda,  Q_e[g] = sum_{k=g+1..Nr} PP_e[k] r_k^-(lambda+1).
+struct TabBuildArgs {
+    const double *PP[2]; const int *ent_pair[2]; const int *ent_lam; const double *rp, *rm;
+    int E[2], E_tot, Nr, Kpad; double2 *T;
+};
+__global__ void __launch_bounds__(128) k_direct_tables_build(const TabBuildArgs a) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= a.E_tot) return;
+    const int c = (e >= a.E[0]) ? 1 : 0, el = e - (c ? a.E[0] : 0), lam = a.ent_lam[e];
+    const double *pp = a.PP[c] + (size_t)a.ent_pair[c][el] * a.Kpad;
+    const double *rp = a.rp + (size_t)lam * a.Kpad, *rm = a.rm + (size_t)lam * a.Kpad;
+    double acc = 0.0;
+    a.T[e].x = 0.0;
+    for (int k = 1; k <= a.Nr; ++k) { acc += pp[k - 1] * rp[k - 1]; a.T[(size_t)k * a.E_tot + e].x = acc; }
+    acc = 0.0;
+    a.T[(size_t)a.Nr * a.E_tot + e].y = 0.0;
+    for (int k = a.Nr; k >= 1; --k) { acc += pp[k - 1] * rm[k - 1]; a.T[(size_t)(k - 1) * a.E_tot + e].y = acc; }
+}
+
+struct TabEvalArgs { const double2 *T; const int *ent_lam; const double *rk, *R; double *F; int E_tot, Nr, ldF, lambda_max; double h; };
+// grid = (positions, entry blocks of 256)
+__global__ void __launch_bounds__(256) k_direct_tables_eval(const TabEvalArgs a) {
+    __shared__ double sRp[WP_MAX_LAMBDA + 1], sRm[WP_MAX_LAMBDA + 1];
+    __shared__ int s_g;
+    const int p = blockIdx.x;
+    const double R = a.R[p];
+    if (threadIdx.x == 0) {
+        // g = number of grid points r_k = rk[k-1] (k = 1..Nr) with r_k < R: the same comparison as the GEMM's operand
+        int g = (int)floor(R / a.h);
+        g = max(0, min(a.Nr, g));
+        while (g < a.Nr && a.rk[g] < R) ++g;
+        while (g > 0 && !(a.rk[g - 1] < R)) --g;
+        s_g = g;
+        double Rp = 1.0;
+        for (int lam = 0; lam <= a.lambda_max; ++lam) { sRp[lam] = Rp; sRm[lam] = 1.0 / (Rp * R); Rp *= R; }
+    }
+    __syncthreads();
+    const int e = blockIdx.y * blockDim.x + threadIdx.x;
+    if (e >= a.E_tot) return;
+    const double2 t = a.T[(size_t)s_g * a.E_tot + e];
+    const int lam = a.ent_lam[e];
+    a.F[(size_t)p * a.ldF + e] = sRm[lam] * t.x + sRp[lam] * t.y;
+}
+
 }  // namespace
+
+extern "C" size_t wpccc_direct_table_bytes(const wpccc_basis *B) {
+    return B ? (size_t)(B->Nr + 1) * B->E_tot * sizeof(double2) : 0;
+}
+
+extern "C" int wpccc_enable_direct_tables(wpccc_basis *B, void *dev_tables, size_t bytes, void *stream) {
+    if (!B) WP_FAIL(WPCCC_EINVAL, "basis is NULL");
+    if (!dev_tables) { B->d_dtab = nullptr; return 0; }
+    if ((uintptr_t)dev_tables & 255) WP_FAIL(WPCCC_EINVAL, "dev_tables must be 256-byte aligned");
+    if (bytes < wpccc_direct_table_bytes(B)) WP_FAIL(WPCCC_ENOMEM, "direct tables need %zu bytes", wpccc_direct_table_bytes(B));
+    cudaStream_t s = (cudaStream_t)stream;
+    TabBuildArgs a{};
+    for (int c = 0; c < B->n_centres; ++c) { a.PP[c] = B->c[c].d_PP; a.ent_pair[c] = B->c[c].d_ent_pair; a.E[c] = B->c[c].E; }
+    a.ent_lam = B->d_ent_lam; a.rp = B->d_rp; a.rm = B->d_rm; a.E_tot = B->E_tot; a.Nr = B->Nr; a.Kpad = B->Kpad; a.T = (double2 *)dev_tables;
+    k_direct_tables_build<<<(B->E_tot + 127) / 128, 128, 0, s>>>(a);
+    WP_CUDA(cudaGetLastError());
+    WP_CUDA(cudaStreamSynchronize(s));
+    B->d_dtab = (double2 *)dev_tables;
+    return 0;
+}
 
 int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s) {
     if (n_pos <= 0) return 0;
+    if (B->d_dtab) {
+        TabEvalArgs t{};
+        t.T = B->d_dtab; t.ent_lam = B->d_ent_lam; t.rk = B->d_rk; t.R = d_R; t.F = d_F; t.E_tot = B->E_tot; t.Nr = B->Nr; t.ldF = ldF;
+        t.lambda_max = B->lambda_max; t.h = B->h;
+        wp_span_begin(B, FAM_GEMM, s);
+        k_direct_tables_eval<<<dim3(n_pos, (B->E_tot + 255) / 256), 256, 0, s>>>(t);
+        wp_span_end(B, s, 1);
+        WP_CUDA(cudaGetLastError());
+        return 0;
+    }
     GemmArgs a{};
     a.tiles = B->d_tiles;
     int off = 0;

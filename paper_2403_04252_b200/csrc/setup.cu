@@ -142,6 +142,7 @@ size_t layout(wpccc_basis &B, char *base) {
     B.d_rm = bump.take<double>((size_t)L1 * B.Kpad);
     B.d_rk = bump.take<double>(B.Kpad);
     B.d_tiles = bump.take<GemmTile>(B.tiles.size());
+    B.d_ent_lam = bump.take<int>(B.E_tot);
     B.d_status = bump.take<int>(64);
     if (B.has_quad) {
         B.d_gl_rho = bump.take<double>(2 * (size_t)B.quad.n_rho);
@@ -252,6 +253,9 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     auto chk = [&](int r_) { if (r_ && !rc) rc = r_; };
     chk(upload(B->d_rp, rp, s)); chk(upload(B->d_rm, rm, s)); chk(upload(B->d_rk, rk, s));
     chk(upload(B->d_tiles, B->tiles, s));
+    std::vector<int> all_lam;
+    for (int ci = 0; ci < n_centres; ++ci) all_lam.insert(all_lam.end(), B->c[ci].ent_lam.begin(), B->c[ci].ent_lam.end());
+    chk(upload(B->d_ent_lam, all_lam, s));
     if (!rc && cudaMemsetAsync(B->d_status, 0, 64 * sizeof(int), s) != cudaSuccess) rc = WPCCC_ECUDA;
     if (!rc && cudaMemcpyAsync(d_w, w, (size_t)(Nr + 1) * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = WPCCC_ECUDA;
     std::vector<std::vector<double>> keep_d; std::vector<std::vector<int>> keep_i;   // host staging must outlive the async copies

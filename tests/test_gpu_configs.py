@@ -140,3 +140,35 @@ def test_T3_timed_configuration_invariants(lib):
     assert np.abs(out["P_class"].cpu().numpy() - Pc).max() < 1e-13
     sig = observables.cross_sections(b, np.zeros(len(b), np.int32), Pnl, 1)
     assert np.abs(out["sigma_nl"].cpu().numpy() - sig).max() < 1e-12 * max(1.0, np.abs(sig).max())
+
+
+def test_NEXT1_direct_tables_match_oracle_and_gemm(lib):
+    """the prefix/suffix-table route gives the same grid sums of eq. (7) as the definition
+    (oracle) and as the DMMA GEMM, at configs[2] size, including R below the first and beyond the last grid point."""
+    prob, basis = config(lib, 2)
+    run = run_of(2)
+    rng = np.random.default_rng(9)
+    n = 200
+    b, z = rng.choice(run["b"], n), rng.uniform(-99.0, 99.0, n)
+    b[:4] = [0.004, 0.0125, 0.05, 15.0]; z[:4] = [0.003, 0.0, 0.0, 99.5]       # R < r_1, R = r_1 exactly, ..., R > r_max
+    _, Hg, Fg = lib.matrix_elements(basis, b, z, np.ones(n), phases=False, want_S=False, want_F=True)
+    Fg = Fg.cpu().numpy()
+    basis.enable_direct_tables(True)
+    try:
+        _, Ht, Ft = lib.matrix_elements(basis, b, z, np.ones(n), phases=False, want_S=False, want_F=True)
+        Ft, Ht = Ft.cpu().numpy(), Ht.cpu().numpy()
+        ent = basis.radial_entries(0)
+        r = prob.h * np.arange(prob.Nr + 1)
+        for p in (0, 1, 2, 3, 57, 199):
+            Fo = direct.radial_F_all(prob.centres[0], prob.w, r, float(np.hypot(b[p], z[p])), prob.lambda_max)
+            assert_elements(Ft[p], np.array([Fo[lam, a1, a] for (a1, a, lam) in ent]), "table F at position %d" % p)
+        assert_elements(Ft, Fg, "table F vs GEMM F")
+        So, Ho = assemble.S_and_H(prob, b[57], z[57], 1.0, time_phase=False)
+        assert_elements(Ht[57], Ho, "D^T from the table route")
+        # propagation through the table route (configs[4] pick, window of 2 steps)
+        h = (run["z_max"] - run["z_min"]) / run["n_steps"]
+        Cg = lib.propagate(basis, [run["b"][40]], [2.0], -h, h, 2).cpu().numpy()[0]
+        co = oprop.propagate(prob, run["b"][40], 2.0, -h, h, 2)
+        assert np.abs(Cg - co).max() < PTOL
+    finally:
+        basis.enable_direct_tables(False)

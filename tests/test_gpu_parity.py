@@ -75,6 +75,25 @@ def test_direct_many_positions_span_tiles(lib, one_centre):
         assert_elements(F[p], np.array([Fo[lam, a1, a] for (a1, a, lam) in ent]), "F at position %d" % p)
 
 
+def test_direct_tables_route(lib, one_centre):
+    """prefix/suffix tables instead of the GEMM, ragged Nr, all positions against the oracle."""
+    prob, basis = one_centre
+    b, z, v = map(np.array, zip(*POS1))
+    basis.enable_direct_tables(True)
+    try:
+        S, H, F = lib.matrix_elements(basis, b, z, v, phases=True, want_F=True)
+        H, F = H.cpu().numpy(), F.cpu().numpy()
+        ent = basis.radial_entries(0)
+        r = prob.h * np.arange(prob.Nr + 1)
+        for p in range(len(b)):
+            Fo = direct.radial_F_all(prob.centres[0], prob.w, r, float(np.hypot(b[p], z[p])), prob.lambda_max)
+            assert_elements(F[p], np.array([Fo[lam, a1, a] for (a1, a, lam) in ent]), "table F at position %d" % p)
+            So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
+            assert_elements(H[p], Ho, "D^T (tables) at position %d" % p)
+    finally:
+        basis.enable_direct_tables(False)
+
+
 def test_one_centre_propagation_and_probabilities(lib, one_centre):
     prob, basis = one_centre
     b = np.array([0.6, 0.6, 2.0, 0.6, 1.1])          # repeated b: trajectories share matrices
