@@ -13,6 +13,7 @@
 // A^{-1} explicitly: the four solves of an RK4 step then have no sequential dependency chain,
 //     y_P' = y_P - K y_T;  w_P = A^{-1} y_P';  w_T = y_T - K^H w_P.
 #include <algorithm>
+#include <cstdlib>
 
 #include "sweep.cuh"
 
@@ -190,6 +191,83 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep1(const Sweep1Args a
     }
 }
 
+// ------------------------------------------------------------------ a7, large N_P: blocked Gauss-Jordan in global memory
+// In-place inversion of the n x n matrix G (row-major, global / L2) in panels of FJ_NB columns.  A panel is
+// eliminated in shared memory exactly as the unblocked algorithm does it (partial pivoting over the rows not yet
+// used); its row interchanges are then applied to the other columns, and with W = the (interchanged) pivot rows
+// the rest of the matrix is updated in ONE pass,  G[i][c] = (i in panel ? 0 : G[i][c]) + sum_t Pn[i][t] W[t][c],
+// which is the block form of the same FJ_NB elimination steps (traffic over G: once per panel, not once per step).
+constexpr int FJ_NB = 8;
+
+__device__ void gauss_jordan_blocked(cplx *G, int n, cplx *Pn /*[n][FJ_NB]*/, cplx *W /*[FJ_NB][n]*/, cplx *col /*[n]*/,
+                                     int *piv /*[n]*/, int *s_piv, int *s_flag) {
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ cplx rowv[FJ_NB];
+    for (int j0 = 0; j0 < n; j0 += FJ_NB) {
+        const int w = min(FJ_NB, n - j0);
+        for (int e = tid; e < n * w; e += nt) { const int i = e / w, t = e - i * w; Pn[i * FJ_NB + t] = G[(size_t)i * n + j0 + t]; }
+        __syncthreads();
+        for (int t = 0; t < w; ++t) {
+            const int j = j0 + t;
+            if (warp == 0) {
+                double best = -1.0; int bi = j;
+                for (int i = j + lane; i < n; i += 32) { const cplx x = Pn[i * FJ_NB + t]; const double m = x.x * x.x + x.y * x.y; if (m > best) { best = m; bi = i; } }
+                #pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const double m2 = __shfl_xor_sync(0xffffffffu, best, o); const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+                    if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
+                }
+                if (lane == 0) { *s_piv = bi; piv[j] = bi; if (!(best > 0.0)) *s_flag = 1; }
+            }
+            __syncthreads();
+            const int pr = *s_piv;
+            if (pr != j) {
+                if (tid < w) { const cplx x = Pn[j * FJ_NB + tid]; Pn[j * FJ_NB + tid] = Pn[pr * FJ_NB + tid]; Pn[pr * FJ_NB + tid] = x; }
+                __syncthreads();
+            }
+            const cplx d = Pn[j * FJ_NB + t];
+            const double dn = d.x * d.x + d.y * d.y;
+            const cplx dinv = (dn > 0.0) ? cplx{d.x / dn, -d.y / dn} : cplx{0.0, 0.0};
+            for (int i = tid; i < n; i += nt) col[i] = Pn[i * FJ_NB + t];
+            if (tid < w) rowv[tid] = (tid == t) ? dinv : cmul(Pn[j * FJ_NB + tid], dinv);
+            __syncthreads();
+            for (int e = tid; e < n * w; e += nt) {
+                const int i = e / w, tt = e - i * w;
+                cplx v = Pn[i * FJ_NB + tt];
+                if (tt == t) v = {0.0, 0.0};
+                Pn[i * FJ_NB + tt] = (i == j) ? rowv[tt] : csub(v, cmul(col[i], rowv[tt]));
+            }
+            __syncthreads();
+        }
+        // the panel's row interchanges on the other columns, in order
+        for (int t = 0; t < w; ++t) {
+            const int j = j0 + t, pr = piv[j];
+            if (pr != j) {
+                for (int c = tid; c < n; c += nt)
+                    if (c < j0 || c >= j0 + w) { const cplx x = G[(size_t)j * n + c]; G[(size_t)j * n + c] = G[(size_t)pr * n + c]; G[(size_t)pr * n + c] = x; }
+                __syncthreads();
+            }
+        }
+        for (int e = tid; e < w * n; e += nt) { const int t = e / n, c = e - t * n; W[e] = G[(size_t)(j0 + t) * n + c]; }
+        __syncthreads();
+        {
+            int i = tid / n, c = tid - i * n;
+            const int di = nt / n, dc = nt - di * n;
+            for (int e = tid; e < n * n; e += nt) {
+                if (c >= j0 && c < j0 + w) G[e] = Pn[i * FJ_NB + (c - j0)];
+                else {
+                    const cplx *pn = Pn + i * FJ_NB;
+                    cplx acc = (i >= j0 && i < j0 + w) ? cplx{0.0, 0.0} : G[e];
+                    for (int t = 0; t < w; ++t) { const cplx x = pn[t], y = W[t * n + c]; acc.x += x.x * y.x - x.y * y.y; acc.y += x.x * y.y + x.y * y.x; }
+                    G[e] = acc;
+                }
+                i += di; c += dc; if (c >= n) { c -= n; ++i; }
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // ------------------------------------------------------------------ a7: Schur complement + inverse
 // grid = positions; block = 512.  A = I - K K^H (row-major, ld = NP) lives in shared memory when it fits, else in
 // the output buffer (global).  K is staged through shared memory in column chunks of odd width cw (conflict-free).
@@ -232,6 +310,21 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
         __syncthreads();
     }
     if (bad) s_flag = 2;
+    if (!a.use_smem) {
+        // large N_P: the shared memory that staged K now holds the panel, the pivot rows and the column vector
+        cplx *Pn = smc, *Wr = Pn + (size_t)n * FJ_NB, *colv = Wr + (size_t)n * FJ_NB;
+        int *pivg = reinterpret_cast<int *>(colv + n);
+        gauss_jordan_blocked(G, n, Pn, Wr, colv, pivg, &s_piv, &s_flag);
+        for (int j = n - 1; j >= 0; --j) {
+            const int q = pivg[j];
+            if (q != j) {
+                for (int r = tid; r < n; r += nt) { const cplx t = G[(size_t)r * n + j]; G[(size_t)r * n + j] = G[(size_t)r * n + q]; G[(size_t)r * n + q] = t; }
+                __syncthreads();
+            }
+        }
+        if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
+        return;
+    }
     for (int j = 0; j < n; ++j) {
         if (warp == 0) {                                       // pivot search in column j, rows j..n-1
             double best = -1.0; int bi = j;
@@ -538,13 +631,18 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     a.K = d_K; a.Ainv = d_Ainv; a.status = B->d_status; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states;
     const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
     const size_t budget = 200 * 1024;
-    a.use_smem = n * n * 16 + n * 9 * 16 + small <= budget;
+    static const bool force_blocked = []() { const char *e = getenv("WPCCC_FACTOR_BLOCKED"); return e && e[0] == '1'; }();   // tests
+    a.use_smem = !force_blocked && n * n * 16 + n * 9 * 16 + small <= budget;
     const size_t fixed = (a.use_smem ? n * n * 16 : 0) + small;
-    int cw = (int)std::min<size_t>((budget - fixed) / (n * 16), (size_t)a.NT);
+    // large N_P (blocked path): two CTAs per SM; the K staging area is reused by the panel buffers (2 FJ_NB + 1 columns)
+    const size_t blocked_need = (2 * FJ_NB + 1) * n * 16 + n * 4 + 64;
+    const size_t kbudget = a.use_smem ? budget : std::max<size_t>(blocked_need, 100 * 1024);
+    if (!a.use_smem && blocked_need > budget) WP_FAIL(WPCCC_EINVAL, "factorisation: N_P = %d too large", a.NP);
+    int cw = (int)std::min<size_t>((kbudget - fixed) / (n * 16), (size_t)a.NT);
     if (cw > 1 && (cw & 1) == 0) --cw;                        // odd width: conflict-free column reads
     if (cw < 1) WP_FAIL(WPCCC_EINVAL, "factorisation: N_P = %d too large", a.NP);
     a.cw = cw;
-    const size_t smem = fixed + n * cw * 16;
+    const size_t smem = a.use_smem ? fixed + n * cw * 16 : std::max(fixed + n * cw * 16, blocked_need);
     static size_t attr = 0;
     if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     wp_span_begin(B, FAM_FACT, s);
