@@ -325,43 +325,9 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
         if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
         return;
     }
-    for (int j = 0; j < n; ++j) {
-        if (warp == 0) {                                       // pivot search in column j, rows j..n-1
-            double best = -1.0; int bi = j;
-            for (int i = j + lane; i < n; i += 32) { const cplx x = A[(size_t)i * n + j]; const double m = x.x * x.x + x.y * x.y; if (m > best) { best = m; bi = i; } }
-            #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double m2 = __shfl_xor_sync(0xffffffffu, best, o); const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
-            }
-            if (lane == 0) { s_piv = bi; piv[j] = bi; if (!(best > 0.0)) s_flag = 1; }
-        }
-        __syncthreads();
-        const int pr = s_piv;
-        if (pr != j) {
-            for (int c = tid; c < n; c += nt) { const cplx t = A[(size_t)j * n + c]; A[(size_t)j * n + c] = A[(size_t)pr * n + c]; A[(size_t)pr * n + c] = t; }
-            __syncthreads();
-        }
-        const cplx d = A[(size_t)j * n + j];
-        const double dn = d.x * d.x + d.y * d.y;
-        const cplx dinv = (dn > 0.0) ? cplx{d.x / dn, -d.y / dn} : cplx{0.0, 0.0};
-        for (int i = tid; i < n; i += nt) {
-            col[i] = A[(size_t)i * n + j];
-            rowj[i] = (i == j) ? dinv : cmul(A[(size_t)j * n + i], dinv);
-        }
-        __syncthreads();
-        {   // A[i][c] = (i == j) ? rowj[c] : (c == j ? 0 : A[i][c]) - col[i] rowj[c]
-            int i = tid / n, c = tid - i * n;
-            const int di = nt / n, dc = nt - di * n;
-            for (int e = tid; e < n * n; e += nt) {
-                const cplx rj = rowj[c];
-                cplx v = A[e];
-                if (c == j) v = {0.0, 0.0};
-                A[e] = (i == j) ? rj : csub(v, cmul(col[i], rj));
-                i += di; c += dc; if (c >= n) { c -= n; ++i; }
-            }
-        }
-        __syncthreads();
+    {   // shared-memory A: the same blocked elimination, panel buffers in the area that staged K (piv, idx lie behind it)
+        cplx *Pn = Kc, *Wr = Pn + (size_t)n * FJ_NB, *colv = Wr + (size_t)n * FJ_NB;
+        gauss_jordan_blocked(A, n, Pn, Wr, colv, piv, &s_piv, &s_flag);
     }
     if (a.use_smem) {
         if (tid == 0) {
@@ -632,7 +598,7 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
     const size_t budget = 200 * 1024;
     static const bool force_blocked = []() { const char *e = getenv("WPCCC_FACTOR_BLOCKED"); return e && e[0] == '1'; }();   // tests
-    a.use_smem = !force_blocked && n * n * 16 + n * 9 * 16 + small <= budget;
+    a.use_smem = !force_blocked && n * n * 16 + n * (2 * FJ_NB + 1) * 16 + small <= budget;   // K chunk area doubles as the panel buffers
     const size_t fixed = (a.use_smem ? n * n * 16 : 0) + small;
     // large N_P (blocked path): two CTAs per SM; the K staging area is reused by the panel buffers (2 FJ_NB + 1 columns)
     const size_t blocked_need = (2 * FJ_NB + 1) * n * 16 + n * 4 + 64;
