@@ -22,6 +22,17 @@ void wp_set_error(const char *fmt, ...);
 #define WP_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
     wp_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); return WPCCC_ECUDA; } } while (0)
 
+// Row of a buffer for position p of a launch: p = g * n + li  ->  g * ld + fold(off + li), where fold(i) = i for
+// i <= mid and mid2 - i beyond (the mirror position (b, -z) of a z-grid symmetric about 0); n == 0: identity.
+struct PosMap { int n, ld, off, mid2; };    // mid2 < 0: no folding
+__host__ __device__ inline size_t pos_row(const PosMap &m, int p) {
+    if (m.n == 0) return (size_t)p;
+    const int g = p / m.n;
+    int i = m.off + (p - g * m.n);
+    if (m.mid2 >= 0 && 2 * i > m.mid2) i = m.mid2 - i;
+    return (size_t)g * m.ld + i;
+}
+
 // One n-tile of the grouped direct GEMM: columns [n0, n0+cnt) of multipole `lam` of centre `c`.
 struct GemmTile { int c, lam, n0, cnt; };
 
@@ -97,10 +108,13 @@ void wp_timing_reset(wpccc_basis *B);
 
 // ---- direct.cu ----
 // F[p][off_c + e] for all entries of all centres; R = |R_p|.
-int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s);
+// Optional maps: R is read at row pos_row(rmap, p), F written at row pos_row(fmap, p).
+int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s,
+                   const PosMap *rmap = nullptr, const PosMap *fmap = nullptr);
 // Real direct blocks without time phase: Dre[p][N_c][N_c] = -charge * sum_lambda sgn^lambda G P_lambda^mu(cos) F.
 int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, const double *d_F, int ldF,
-                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s);
+                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s,
+                       const PosMap *fmap = nullptr);   // F of position p is row pos_row(fmap, p)
 
 // ---- transfer.cu ----
 size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk);

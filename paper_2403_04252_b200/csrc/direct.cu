@@ -37,6 +37,7 @@ struct GemmArgs {
     const double *R;
     double *F;
     int ldF, n_pos, Kpad;
+    PosMap rmap, fmap;
 };
 
 // grid: (m tiles, n tiles).  256 threads = 8 warps as 2 (M) x 4 (N); warp tile 64 x 32 -> 32 DMMA per k4 step.
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs 
 
     if (tid < BM) {
         int p = m0 + tid;
-        double R = (p < a.n_pos) ? a.R[p] : 1.0;
+        double R = (p < a.n_pos) ? a.R[pos_row(a.rmap, p)] : 1.0;
         double Rp = 1.0;
         for (int i = 0; i < lam; ++i) Rp *= R;
         sR[tid] = R; sRp[tid] = Rp; sRm[tid] = 1.0 / (Rp * R);
@@ -133,7 +134,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs 
     for (int i = 0; i < 8; ++i) {
         int p = m0 + wm + 8 * i + fr;
         if (p >= a.n_pos) continue;
-        double *Frow = a.F + (size_t)p * a.ldF + colbase;
+        double *Frow = a.F + pos_row(a.fmap, p) * a.ldF + colbase;
         #pragma unroll
         for (int j = 0; j < 4; ++j) {
             int n = wn + 8 * j + 2 * fk;
@@ -173,6 +174,7 @@ struct AsmArgs {
     int n_rad, N, Lc, lambda_max, ldF, f_off, ld_out, complex_out;
     long long pos_stride;
     double charge; int alt_sign;
+    PosMap fmap;
 };
 
 // grid: (n_pos, ceil(N*N/256)).  out[p*pos_stride + i*ld_out + j] (real, or complex with zero imaginary part).
@@ -189,7 +191,7 @@ __global__ void __launch_bounds__(256) k_direct_assemble(const AsmArgs a) {
     const int mu = mp - m, nlm = (a.Lc + 1) * (a.Lc + 1);
     const int alo = min(ap, aa), ahi = max(ap, aa);
     const double *Gp = a.G + ((size_t)lm_index(lp, mp) * nlm + lm_index(l, m)) * (L + 1);
-    const double *Fp = a.F + (size_t)p * a.ldF + a.f_off;
+    const double *Fp = a.F + pos_row(a.fmap, p) * a.ldF + a.f_off;
     double acc = 0.0;
     int lam0 = abs(lp - l);
     for (int lam = lam0; lam <= min(lp + l, L); lam += 2) {
@@ -215,6 +217,7 @@ struct Asm2Args {
     int n_rad, n_pairs, E, N, Lc, lambda_max, ldF, f_off, ld_out, complex_out, n_pos;
     long long pos_stride;
     double charge; int alt_sign;
+    PosMap fmap;
 };
 
 __global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
@@ -231,7 +234,7 @@ __global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
     for (int p = blockIdx.x; p < a.n_pos; p += gridDim.x) {
         __syncthreads();                                 // previous position done with sF / sAng
         if (tid == 0) assoc_legendre_all(L, a.cosT[p], sP, ldp);
-        const double *Fp = a.F + (size_t)p * a.ldF + a.f_off;
+        const double *Fp = a.F + pos_row(a.fmap, p) * a.ldF + a.f_off;
         for (int e = tid; e < a.E; e += nt) sF[a.ent_perm[e]] = Fp[e];
         __syncthreads();
         for (int e = tid; e < (L + 1) * nlm * nlm; e += nt) {
@@ -288,13 +291,13 @@ __global__ void __launch_bounds__(128) k_direct_tables_build(const TabBuildArgs 
     for (int k = a.Nr; k >= 1; --k) { acc += pp[k - 1] * rm[k - 1]; a.T[(size_t)(k - 1) * a.E_tot + e].y = acc; }
 }
 
-struct TabEvalArgs { const double2 *T; const int *ent_lam; const double *rk, *R; double *F; int E_tot, Nr, ldF, lambda_max; double h; };
+struct TabEvalArgs { const double2 *T; const int *ent_lam; const double *rk, *R; double *F; int E_tot, Nr, ldF, lambda_max; double h; PosMap rmap, fmap; };
 // grid = (positions, entry blocks of 256)
 __global__ void __launch_bounds__(256) k_direct_tables_eval(const TabEvalArgs a) {
     __shared__ double sRp[WP_MAX_LAMBDA + 1], sRm[WP_MAX_LAMBDA + 1];
     __shared__ int s_g;
     const int p = blockIdx.x;
-    const double R = a.R[p];
+    const double R = a.R[pos_row(a.rmap, p)];
     if (threadIdx.x == 0) {
         // g = number of grid points r_k = rk[k-1] (k = 1..Nr) with r_k < R: the same comparison as the GEMM's operand
         int g = (int)floor(R / a.h);
@@ -310,7 +313,7 @@ __global__ void __launch_bounds__(256) k_direct_tables_eval(const TabEvalArgs a)
     if (e >= a.E_tot) return;
     const double2 t = a.T[(size_t)s_g * a.E_tot + e];
     const int lam = a.ent_lam[e];
-    a.F[(size_t)p * a.ldF + e] = sRm[lam] * t.x + sRp[lam] * t.y;
+    a.F[pos_row(a.fmap, p) * a.ldF + e] = sRm[lam] * t.x + sRp[lam] * t.y;
 }
 
 }  // namespace
@@ -335,10 +338,13 @@ extern "C" int wpccc_enable_direct_tables(wpccc_basis *B, void *dev_tables, size
     return 0;
 }
 
-int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s) {
+int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, int ldF, cudaStream_t s,
+                   const PosMap *rmap, const PosMap *fmap) {
     if (n_pos <= 0) return 0;
+    const PosMap ident{0, 0, 0, -1};
     if (B->d_dtab) {
         TabEvalArgs t{};
+        t.rmap = rmap ? *rmap : ident; t.fmap = fmap ? *fmap : ident;
         t.T = B->d_dtab; t.ent_lam = B->d_ent_lam; t.rk = B->d_rk; t.R = d_R; t.F = d_F; t.E_tot = B->E_tot; t.Nr = B->Nr; t.ldF = ldF;
         t.lambda_max = B->lambda_max; t.h = B->h;
         wp_span_begin(B, FAM_GEMM, s);
@@ -356,6 +362,7 @@ int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, in
         a.cen_off[c] = off; off += B->c[c].E;
     }
     a.rp = B->d_rp; a.rm = B->d_rm; a.rk = B->d_rk; a.R = d_R; a.F = d_F; a.ldF = ldF; a.n_pos = n_pos; a.Kpad = B->Kpad;
+    a.rmap = rmap ? *rmap : ident; a.fmap = fmap ? *fmap : ident;
     const size_t smem = (size_t)NSTG * (BM + BN) * LDS_ * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
@@ -371,10 +378,11 @@ int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, in
 }
 
 int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, const double *d_F, int ldF,
-                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s) {
+                       double *d_out, int ld_out, long long pos_stride, int complex_out, cudaStream_t s, const PosMap *fmap) {
     if (n_pos <= 0) return 0;
     const CentreTab &C = B->c[c];
     AsmArgs a{};
+    a.fmap = fmap ? *fmap : PosMap{0, 0, 0, -1};
     a.G = C.d_G; a.ent_lookup = C.d_ent_lookup; a.st_rad = C.d_st_rad; a.st_l = C.d_st_l; a.st_m = C.d_st_m;
     a.cosT = d_cos; a.F = d_F; a.out = d_out;
     a.n_rad = C.n_rad; a.N = C.n_states; a.Lc = C.l_max; a.lambda_max = B->lambda_max; a.ldF = ldF;
@@ -392,7 +400,7 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
         b.cosT = d_cos; b.F = d_F; b.out = d_out;
         b.n_rad = C.n_rad; b.n_pairs = C.n_pairs; b.E = C.E; b.N = C.n_states; b.Lc = C.l_max; b.lambda_max = B->lambda_max; b.ldF = ldF;
         b.f_off = a.f_off; b.ld_out = ld_out; b.complex_out = complex_out; b.n_pos = n_pos; b.pos_stride = pos_stride;
-        b.charge = a.charge; b.alt_sign = a.alt_sign;
+        b.charge = a.charge; b.alt_sign = a.alt_sign; b.fmap = a.fmap;
         static size_t attr2 = 0;
         if (smem2 > attr2) { WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2)); attr2 = smem2; }
         const int per_sm = smem2 <= 100 * 1024 ? 2 : 1;
