@@ -100,9 +100,11 @@ def workload(cfg_idx, world, rank):
     return prob, run, shard_indices(len(run["b"]), rank, world)
 
 
-def family_work(prob, b_local, n_steps):
+def family_work(prob, b_local, n_steps, units=None):
     """Algorithmic work of each kernel family for ONE step of the bench.
-    Returns {family: (bound, work, unit)} with work in flops (tensor / alu) or bytes (hbm)."""
+    Returns {family: (bound, work, unit)} with work in flops (tensor / alu) or bytes (hbm).
+    units: positions per step each family actually processed (wpccc_last_units): on a symmetric z-grid the node
+    tables and the contraction run once per mirror pair (b, -z), (b, +z), and only that work is counted."""
     two = len(prob.centres) == 2
     n_traj_local = len(b_local)
     groups = len(set(np.asarray(b_local).tolist()))       # one-centre: trajectories with equal b share every matrix
@@ -122,9 +124,11 @@ def family_work(prob, b_local, n_steps):
         nodes = q["n_rho"] * q["n_z"]
         nqc = [int(sum(int(x) + 1 for x in c.l)) for c in prob.centres]
         nrad = [len(c.l) for c in prob.centres]
-        out["transfer_contraction"] = ("tensor", 3 * 4.0 * nqc[0] * nqc[1] * nodes * n_pos, "flop")
+        n_con = (units or {}).get("transfer_contraction") or n_pos
+        n_tab = (units or {}).get("transfer_tables") or n_pos
+        out["transfer_contraction"] = ("tensor", 3 * 4.0 * nqc[0] * nqc[1] * nodes * n_con, "flop")
         # node tables: bound by the HBM write of X and Xh for every (column, node) of both sides
-        out["transfer_tables"] = ("hbm", 8.0 * 2 * (nqc[0] + nqc[1]) * nodes * n_pos, "byte")
+        out["transfer_tables"] = ("hbm", 8.0 * 2 * (nqc[0] + nqc[1]) * nodes * n_tab, "byte")
         out["rotation"] = ("hbm", 16.0 * (3 * Nc[0] * Nc[1] + 6 * nqc[0] * nqc[1]) * n_pos, "byte")
         out["direct_assemble"] = ("hbm", 16.0 * (Nc[0] ** 2 + Nc[1] ** 2) * n_pos, "byte")
         out["factor"] = ("alu", (8.0 * Nc[1] ** 2 * Nc[0] + 8.0 / 3.0 * Nc[1] ** 3) * n_pos, "flop")
@@ -180,7 +184,7 @@ def run_ours(args):
         step()
     barrier()
     m0 = sampler.mark() if sampler else 0
-    evs, launches, fam_ms = [], 0, {}
+    evs, launches, fam_ms, units_step = [], 0, {}, {}
     for _ in range(args.steps):
         flush.fill_(1)                                                     # L2 flush between timed iterations
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -190,6 +194,7 @@ def run_ours(args):
         evs.append((e0, e1))
         tm = wp.last_timing(basis)                                         # synchronises; per-family event times of this step
         launches += sum(n for _, n in tm.values()) + 4                     # + init amplitudes, probabilities, 2 x cross sections
+        units_step = wp.last_units(basis)                                  # positions per family of this step (same every step)
         for k, (ms, n) in tm.items():
             a = fam_ms.setdefault(k, [0.0, 0])
             a[0] += ms; a[1] += n
@@ -239,7 +244,7 @@ def run_ours(args):
     # stream each kernel was launched on, during the timed steps above)
     pk = measured_peaks()
     dmma, dfma = wp.fp64_peak(1), wp.fp64_peak(0)
-    work = family_work(prob, b, n_steps)
+    work = family_work(prob, b, n_steps, units_step)
     if args.direct_tables:                                                 # NEXT-1: 16 B read + 8 B written per entry and position
         work["direct_gemm"] = ("hbm", work["direct_gemm"][1] / (2.0 * prob.Nr) * 24.0, "byte")
     fams = {}
@@ -275,7 +280,9 @@ def run_ours(args):
                        N, len(b_all), n_steps, (" (%d per rank)" % len(b) if world > 1 else "") + (" [window of the configured step size around z = 0, not the full z-range]" if args.window_steps else "")),
                    "l2": "512 MiB buffer written between timed iterations (L2 flush); window buffers of one step are several GB >> L2",
                    "parallelism": "dp%d over impact parameters" % world,
-                   "direct": "prefix/suffix tables (NEXT-1)" if args.direct_tables else "DMMA GEMM"},
+                   "direct": "prefix/suffix tables (NEXT-1)" if args.direct_tables else "DMMA GEMM",
+                   "mirror_pairs": "body-frame integrals of (b,-z),(b,+z) evaluated together: %d of %d positions per step run the node tables and the contraction; roofline work counts those only" % (
+                       units_step.get("transfer_contraction", 0), units_step.get("rotation", 0)) if prob.quad else "n/a"},
         "matrix_elements_per_s": round(elems_per_pos * len(b_all) * (2 * n_steps + 1) / (ms_step * 1e-3), 1),
         "clocks": clocks,
         "e2e": {"value": round(e2e_val, 3), "unit": "trajectory*steps/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},

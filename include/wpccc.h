@@ -179,6 +179,16 @@ int wpccc_probabilities(const wpccc_basis *basis, int n_traj, const double *dC /
  * 7 other.  Synchronises the device.  Returns the number of families (8). */
 int wpccc_last_timing(const wpccc_basis *basis, double *ms /*[host][8]*/, long long *launches /*[host][8]*/);
 
+/* Positions processed by each family (same order) in the last wpccc_propagate / wpccc_matrix_elements
+ * call, for the families that count them (2 node tables, 3 contraction, 4 rotation; 0 otherwise).
+ * wpccc_propagate on a z-grid symmetric about 0 (z_min = -z_max) evaluates the body-frame integrals of
+ * eq. (9) once per mirror pair (b, -z), (b, +z) -- they differ only by the complex conjugation of the
+ * axial phase -- as far as the workspace beyond wpccc_workspace_bytes(.., 2) can hold the second
+ * member's integrals until the sweep reaches it; units[3] is then smaller
+ * than the number of positions.  The environment variable WPCCC_NO_MIRROR disables this.
+ * Returns the number of families (8) or WPCCC_EINVAL. */
+int wpccc_last_units(const wpccc_basis *basis, long long *units /*[host][8]*/);
+
 /* Measures the device's FP64 peak with a register-resident micro-benchmark on `stream`:
  * kind 0 = DFMA (plain FP64 FMA pipe), kind 1 = DMMA (mma.sync.m8n8k4.f64).  Returns TFLOP/s
  * (negative WPCCC_E* as a double on error).  Used by bench.py for the roofline denominator. */

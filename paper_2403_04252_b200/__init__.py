@@ -7,7 +7,7 @@ compute call raises ``WpcccError`` when the library cannot run on a CUDA device,
 ``ImportError`` when ``libwpccc.so`` has not been built (``python paper_2403_04252_b200/build.py`` or ``__graft_entry__.build()``).
 
 The function names mirror the C entry points: ``setup_basis`` (wpccc_setup_basis), ``matrix_elements``,
-``propagate``, ``probabilities``, ``fp64_peak``, ``last_timing``.
+``propagate``, ``probabilities``, ``fp64_peak``, ``last_timing``, ``last_units``.
 """
 from __future__ import annotations
 
@@ -71,6 +71,8 @@ _lib.wpccc_probabilities.restype = C.c_int
 _lib.wpccc_probabilities.argtypes = [_vp, C.c_int, _vp, _dp, _ip, C.c_int, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.wpccc_last_timing.restype = C.c_int
 _lib.wpccc_last_timing.argtypes = [_vp, _dp, C.POINTER(C.c_longlong)]
+_lib.wpccc_last_units.restype = C.c_int
+_lib.wpccc_last_units.argtypes = [_vp, C.POINTER(C.c_longlong)]
 _lib.wpccc_fp64_peak.restype = C.c_double
 _lib.wpccc_fp64_peak.argtypes = [C.c_int, _vp]
 _lib.wpccc_direct_table_bytes.restype = C.c_size_t
@@ -82,7 +84,7 @@ _lib.wpccc_version.restype = C.c_char_p
 
 EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
-           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_probabilities", "wpccc_last_timing", "wpccc_fp64_peak",
+           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
            "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
 
 
@@ -265,6 +267,13 @@ def last_timing(basis: Basis):
     ln = (C.c_longlong * 8)()
     _lib.wpccc_last_timing(basis._h, ms, ln)
     return {f: (ms[i], ln[i]) for i, f in enumerate(FAMILIES)}
+
+
+def last_units(basis: Basis):
+    """wpccc_last_units: {family: positions processed} of the last propagate / matrix_elements call (0: not counted)."""
+    un = (C.c_longlong * 8)()
+    _lib.wpccc_last_units(basis._h, un)
+    return {f: un[i] for i, f in enumerate(FAMILIES)}
 
 
 def fp64_peak(kind: int) -> float:

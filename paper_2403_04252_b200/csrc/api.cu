@@ -2,6 +2,7 @@
 // wpccc_fp64_peak: argument checking, workspace carving and launch orchestration only (include/wpccc.h).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <map>
 
 #include "common.cuh"
@@ -129,12 +130,12 @@ GeomOut carve_geom(Carver &cv, size_t n) {
 
 // elements of one block of positions (geometry already on the device): F, then H0 / K (two-centre) or Dre (one-centre)
 int elements_two_centre(wpccc_basis *B, int n_pos, const GeomOut &g, double *d_F, double *d_K, double *d_H, void *tws, size_t tws_bytes,
-                        int chunk, cudaStream_t s) {
+                        int chunk, cudaStream_t s, const TransferSel *sel = nullptr) {
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
     int rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, s); if (rc) return rc;
     rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_H, N, (long long)N * N, 1, s); if (rc) return rc;
     rc = wp_direct_assemble(B, 1, n_pos, g.cosT, d_F, B->E_tot, d_H + ((size_t)NT * N + NT) * 2, N, (long long)N * N, 1, s); if (rc) return rc;
-    return wp_transfer(B, n_pos, g.R, g.cosT, g.sinT, g.theta, g.v, d_K, d_H, tws, tws_bytes, chunk, s);
+    return wp_transfer(B, n_pos, g.R, g.cosT, g.sinT, g.theta, g.v, d_K, d_H, tws, tws_bytes, chunk, s, sel);
 }
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -180,7 +181,10 @@ extern "C" size_t wpccc_workspace_bytes(const wpccc_basis *B, int n_traj, int n_
     if (what == 2) return plan_bytes(P, 1);
     int W = std::max(1, std::min(n_steps, 64));
     while (W > 1 && plan_bytes(P, W) > ((size_t)48 << 30)) W = W / 2;
-    return plan_bytes(P, W);
+    size_t tot = plan_bytes(P, W);
+    if (P.two && W == std::min(std::max(n_steps, 1), 64) && wp_transfer_mirror_ok(B))     // mirror stash, at most 32 GB
+        tot += std::min((size_t)n_traj * (size_t)std::max(n_steps, 1) * wp_transfer_stash_doubles(B) * 8, (size_t)32 << 30) + 4096;
+    return tot;
 }
 
 extern "C" int wpccc_matrix_elements(const wpccc_basis *Bc, int n_pos, const double *b, const double *z, const double *v, int flags,
@@ -313,6 +317,18 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         } else d_D[k] = cv.take<double>(npos_max * N * ldD);
     }
     if (!cv.ok) WP_FAIL(WPCCC_ENOMEM, "workspace too small (internal plan mismatch)");
+    // Mirror stash: on a z-grid symmetric about 0 the body-frame two-centre integrals at (b, +z) are written by the
+    // launch that evaluates (b, -z) (TransferSel, common.cuh); whatever the workspace has left beyond the window
+    // buffers holds the n_st half-step positions per trajectory that follow z = 0.
+    TransferSel sel{}; bool mirror = false;
+    if (two && std::fabs(z_min + z_max) <= 1e-14 * std::fabs(z_max) && wp_transfer_mirror_ok(B) && !getenv("WPCCC_NO_MIRROR")) {
+        const size_t slot = wp_transfer_stash_doubles(B) * 8, left = ws_bytes > cv.off + 4096 ? ws_bytes - cv.off - 4096 : 0;
+        const size_t n_st = std::min<size_t>((size_t)n_steps, left / ((size_t)n_traj * slot));
+        if (n_st > 0) {
+            sel.stash = cv.take<double>((size_t)n_traj * n_st * (slot / 8));
+            sel.n_st = (int)n_st; sel.n_groups = n_traj; sel.i_mid = n_steps; mirror = cv.ok;
+        }
+    }
 
     if (two) WP_CUDA(cudaMemcpyAsync(d_b, b, n_traj * sizeof(double), cudaMemcpyHostToDevice, s));
     else WP_CUDA(cudaMemcpyAsync(d_b, ub.data(), ub.size() * sizeof(double), cudaMemcpyHostToDevice, s));
@@ -340,7 +356,12 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         wp_span_end(B, e, 1);
         if (two) {
             WP_CUDA(cudaMemsetAsync(d_H[buf], 0, (size_t)n_pos * N * N * 16, e));
-            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e);
+            if (mirror) {
+                sel.n_idx = n_idx; sel.i0 = i0;
+                sel.n_pre = (int)std::max<long long>(0, std::min<long long>(n_idx, sel.i_mid + 1 - i0));
+                sel.suf0 = (int)std::max<long long>(sel.n_pre, std::min<long long>(n_idx, sel.i_mid + sel.n_st + 1 - i0));
+            }
+            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e, mirror ? &sel : nullptr);
             if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], e);
         } else {
             rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, e);

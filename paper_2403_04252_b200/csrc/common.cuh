@@ -33,6 +33,20 @@ __host__ __device__ inline size_t pos_row(const PosMap &m, int p) {
     return (size_t)g * m.ld + i;
 }
 
+// Mirror pairs of a z-grid symmetric about 0 (two-centre propagation).  The body-frame integrals of eq. (9) at (b, -z)
+// and (b, +z) share R, the quadrature nodes, the node tables and the ring weights Phi_Delta(v rho' sinTheta); only the
+// axial phase e^{-i v cosTheta (z' - R/2)} is complex-conjugated.  A window of wpccc_propagate therefore evaluates
+// the integrals only at the positions selected here and, for those with a free stash slot, also writes the
+// integrals of the mirror position, which a later window fetches instead of recomputing them.
+// Window position p = g * n_idx + li (half-step index i = i0 + li); evaluated li: [0, n_pre) and [suf0, n_idx),
+// fetched li: [n_pre, suf0), i.e. the indices in (i_mid, i_mid + n_st].  Stash slot of (g, i): g * n_st + i - i_mid - 1.
+struct TransferSel {
+    int n_groups, n_idx, n_pre, suf0;
+    long long i0, i_mid;
+    int n_st;                    // stash depth (half-step indices per group)
+    double *stash;               // [n_groups * n_st] slots of wp_transfer_stash_doubles(B) doubles
+};
+
 // One n-tile of the grouped direct GEMM: columns [n0, n0+cnt) of multipole `lam` of centre `c`.
 struct GemmTile { int c, lam, n0, cnt; };
 
@@ -98,6 +112,7 @@ struct wpccc_basis {
     long long last_launches[WP_NFAM] = {0};
     long long launches[WP_NFAM] = {0};
     long long groups[WP_NFAM] = {0};
+    long long units[WP_NFAM] = {0};       // positions processed per family in the last call (wpccc_last_units)
     int cur_fam = 0; bool cur_sampled = false;
 };
 
@@ -121,8 +136,13 @@ size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk);
 int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes);
 // Lab-frame S_PT -> d_K [p][N_P][N_T]; H_PT -> d_H rows N_T.., cols 0..; H_TP -> d_H rows 0.., cols N_T..  (no time phases).
 // `chunk` positions are processed per launch group (node tables of a chunk should stay L2-resident).
+// With `sel` (n_pos = sel->n_groups * sel->n_idx) only the selected positions are evaluated (ring splits off) and the
+// others come from sel->stash.
 int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
-                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s);
+                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s,
+                const TransferSel *sel = nullptr);
+size_t wp_transfer_stash_doubles(const wpccc_basis *B);   // doubles per stash slot
+bool wp_transfer_mirror_ok(const wpccc_basis *B);         // the mirror-pair contraction kernel fits shared memory
 int wp_transfer_default_chunk(const wpccc_basis *B);
 
 // ---- sweep.cu ----

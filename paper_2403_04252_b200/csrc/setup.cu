@@ -350,11 +350,11 @@ static cudaEvent_t take_event(wpccc_basis *B) {
 }
 void wp_timing_reset(wpccc_basis *B) {
     B->spans.clear(); B->ev_used = 0;
-    for (int k = 0; k < WP_NFAM; ++k) { B->launches[k] = 0; B->groups[k] = 0; }
+    for (int k = 0; k < WP_NFAM; ++k) { B->launches[k] = 0; B->groups[k] = 0; B->units[k] = 0; }
 }
 // Spans are sampled: families launched once per chunk of positions (thousands of launches per call) record an
 // event pair on every 8th launch group only; the family total is the sampled mean times the number of groups.
-static const int k_sample_every[WP_NFAM] = {1, 1, 8, 8, 8, 1, 1, 1};
+static const int k_sample_every[WP_NFAM] = {1, 1, 8, 8, 1, 1, 1, 1};
 void wp_span_begin(wpccc_basis *B, int fam, cudaStream_t s) {
     B->cur_fam = fam;
     B->cur_sampled = (B->groups[fam]++ % k_sample_every[fam]) == 0;
@@ -380,5 +380,10 @@ extern "C" int wpccc_last_timing(const wpccc_basis *Bc, double *ms, long long *l
         if (ms) ms[k] = B->last_ms[k];
         if (launches) launches[k] = B->launches[k];
     }
+    return WP_NFAM;
+}
+extern "C" int wpccc_last_units(const wpccc_basis *B, long long *units) {
+    if (!B || !units) return WPCCC_EINVAL;
+    for (int k = 0; k < WP_NFAM; ++k) units[k] = B->units[k];
     return WP_NFAM;
 }

@@ -38,6 +38,14 @@ __host__ __device__ inline int lq_index(int l, int q) { return l * (l + 1) / 2 +
 __constant__ double c_fact[2 * WP_MAX_L + 2];
 __constant__ double c_thnorm[NLQ];          // sqrt((2l+1)/2 (l-q)!/(l+q)!)
 
+// Evaluated positions of a launch group (TransferSel in common.cuh): compact index q -> window position p.
+struct SelDev { int n_c, n_idx, n_pre, suf0; };          // n_idx == 0: identity
+__device__ __forceinline__ int sel_pos(const SelDev &s, int q) {
+    if (s.n_idx == 0) return q;
+    const int g = q / s.n_c, lj = q - g * s.n_c;
+    return g * s.n_idx + (lj < s.n_pre ? lj : lj - s.n_pre + s.suf0);
+}
+
 // ------------------------------------------------------------------------------------------------ per-position tables
 struct PosTabs {      // layout of the small per-position table block (doubles), filled by k_tpos
     int n_rho, n_z, n_phi, dmax;
@@ -51,14 +59,15 @@ struct PosTabs {      // layout of the small per-position table block (doubles),
 struct TposArgs {
     PosTabs L; const double *R, *cosT, *sinT, *v; const double *gl_rho, *gl_phi, *gl_zq, *gl_zh;
     double rho_max, z_pad; int phi_rule; double *out;
+    SelDev sel; int q0;                      // block x evaluates window position sel_pos(sel, q0 + x)
 };
 
 // grid = positions, block = 128
 __global__ void __launch_bounds__(128) k_tpos(const TposArgs a) {
-    const int p = blockIdx.x, tid = threadIdx.x;
+    const int p = blockIdx.x, tid = threadIdx.x, gp = sel_pos(a.sel, a.q0 + p);
     const PosTabs &L = a.L;
     double *o = a.out + (size_t)p * L.size();
-    const double R = a.R[p], cT = a.cosT[p], sT = a.sinT[p], v = a.v[p];
+    const double R = a.R[gp], cT = a.cosT[gp], sT = a.sinT[gp], v = a.v[gp];
     const int nq = L.n_z / 4, nh = L.n_z / 2;
     for (int k = tid; k < L.n_z; k += blockDim.x) {
         double lo, hi, x, w;
@@ -112,6 +121,7 @@ struct TtabArgs {
     double h; int Nr, KC;                    // KC: z' nodes per CTA (multiple of 4)
     double *out[2]; size_t pos_stride[2];    // doubles per position for each side
     int lmax[2];
+    SelDev sel; int q0;
 };
 
 // grid = (ring * n_kchunks, side, position), block = 256, dynamic smem (per-node quantities only).
@@ -129,7 +139,7 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     double *sTh = sPot + KC;                             // [nlq][KC]
     int *sJ = reinterpret_cast<int *>(sTh + (size_t)nlq * KC);   // [KC] stencil centre, -1 beyond r_max
     const double *pt = a.pos + (size_t)p * a.L.size();
-    const double R = a.R[p];
+    const double R = a.R[sel_pos(a.sel, a.q0 + p)];
     const int nkc = a.L.n_z / 4;
     const int tile_stride = a.L.n_rho * nkc * 256;
 
@@ -221,8 +231,13 @@ __device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigne
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int TC_STAGES = 3, TC_KCS = 16;     // stage = 16 k4-groups = 64 z' nodes per operand
-constexpr int TC_STAGE_DOUBLES = TC_KCS * 256;                  // per operand
+// TMA ring of the contraction: stage = KCS k4-groups of z' nodes per operand (256 doubles each).
+// Plain kernel: 3 stages of 16 groups (192 KB).  Mirror-pair kernel (DUAL): the accumulators of the mirror position
+// take 128 KB of shared memory, so the ring is 5 stages of 4 groups (80 KB).
+template <bool DUAL> struct TcRing {
+    static constexpr int STAGES = DUAL ? 5 : 3, KCS = DUAL ? 4 : 16, STAGE_DOUBLES = KCS * 256;
+    static constexpr size_t ACC_DOUBLES = DUAL ? 64 * 256 : 0;      // [32 double2][256 threads] (NJ = 4 only)
+};
 
 struct TconArgs {
     PosTabs L; const double *pos;
@@ -232,12 +247,14 @@ struct TconArgs {
     const int2 *tiles; int n_tiles;                              // (row tile over [B|Bh], col tile over [A|Ah])
     int n_split;                                                 // ring splits
     double *part;                                                // [p][split][fam 2][prod 3][nq8P][nq8T] complex
+    // DUAL: block z = compact position q0 + z; its mirror's integrals go to the stash slot (n_split == 1)
+    SelDev sel; int q0, n_st; long long i0, i_mid; double *stash;
 };
 
 // One stage (nk k4-groups of z' nodes) of a warp's 16 x 8 NJ complex tile: C += (B ck)^T A with the complex weight
 // ck = w_z e^{..} folded into the B fragments.  ALL: every 8 x 8 sub-tile is needed (no predicates in the loop);
 // FULL: nk == TC_KCS (fully unrolled, fragments of the next k4-group loaded while the current DMMAs issue).
-template <int NJ, bool ALL, bool FULL>
+template <int NJ, bool ALL, bool FULL, int TC_KCS>
 __device__ __forceinline__ void tcon_stage(const double *Ab, const double *Bb, const double *ck, int nk, const bool (&need)[2][NJ],
                                            double (&Cre)[2][NJ][2], double (&Cim)[2][NJ][2]) {
     double af[2][NJ], bb[2][2], cc[2][2];
@@ -281,13 +298,16 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
 // grid = (tile, ring split, position); block = 4 (rows) x 8/NJ (cols) warps; warp tile 16 x 8 NJ complex
 // (NJ = 4: 8 warps, NJ = 2: 16 warps).  Stages are released per warp through `empty` mbarriers (no block-wide
 // barrier in the main loop); thread 0 refills the buffer of stage st - 1 once it has finished stage st itself.
-template <int NJ>
+template <int NJ, bool DUAL>
 __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     constexpr int WC = 8 / NJ, NW = 4 * WC, TC_THREADS = 32 * NW;
+    constexpr int TC_STAGES = TcRing<DUAL>::STAGES, TC_KCS = TcRing<DUAL>::KCS, TC_STAGE_DOUBLES = TcRing<DUAL>::STAGE_DOUBLES;
+    static_assert(!DUAL || NJ == 4, "mirror-pair kernel: 256 threads");
     extern __shared__ __align__(128) double sm[];
     double *sA = sm;                                          // [STAGES][TC_STAGE_DOUBLES]  A-side (mma "B" operand)
     double *sB = sA + TC_STAGES * TC_STAGE_DOUBLES;           // [STAGES][TC_STAGE_DOUBLES]  B-side (mma "A" operand)
-    double *sCk = sB + TC_STAGES * TC_STAGE_DOUBLES;          // [n_z][2]
+    double2 *sAcc = reinterpret_cast<double2 *>(sB + TC_STAGES * TC_STAGE_DOUBLES);   // DUAL: [32][256] mirror accumulators
+    double *sCk = sB + TC_STAGES * TC_STAGE_DOUBLES + TcRing<DUAL>::ACC_DOUBLES;      // [n_z][2]
     double *sRw = sCk + 2 * a.L.n_z;                          // [dmax+2][n_rho][2], last row zero (weight of unused elements)
     __shared__ __align__(8) unsigned long long bar[TC_STAGES], empty[TC_STAGES];
 
@@ -304,6 +324,10 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     for (int i = tid; i < 2 * n_z; i += TC_THREADS) sCk[i] = pt[a.L.off_ck() + i];
     for (int i = tid; i < 2 * (a.L.dmax + 1) * n_rho; i += TC_THREADS) sRw[i] = pt[a.L.off_rw() + i];
     for (int i = tid; i < 2 * n_rho; i += TC_THREADS) sRw[2 * (a.L.dmax + 1) * n_rho + i] = 0.0;
+    if (DUAL) {
+        #pragma unroll
+        for (int k = 0; k < 32; ++k) sAcc[k * 256 + tid] = make_double2(0.0, 0.0);
+    }
     if (tid == 0) { for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&bar[s], 1); mbar_init(&empty[s], NW); } asm volatile("fence.mbarrier_init.release.cluster;\n" ::); }
     __syncthreads();
 
@@ -364,9 +388,9 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
             const double *Ab = sA + buf * TC_STAGE_DOUBLES + (NJ * wc) * 32 + lane;
             const double *Bb = sB + buf * TC_STAGE_DOUBLES + (2 * wr) * 32 + lane;
             const double *ck = sCk + 2 * (kc0 * 4 + fk);
-            if (all_need && nk == TC_KCS) tcon_stage<NJ, true, true>(Ab, Bb, ck, nk, need, Cre, Cim);
-            else if (all_need) tcon_stage<NJ, true, false>(Ab, Bb, ck, nk, need, Cre, Cim);
-            else tcon_stage<NJ, false, false>(Ab, Bb, ck, nk, need, Cre, Cim);
+            if (all_need && nk == TC_KCS) tcon_stage<NJ, true, true, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
+            else if (all_need) tcon_stage<NJ, true, false, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
+            else tcon_stage<NJ, false, false, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[buf]);           // this warp is done with the buffer
@@ -387,6 +411,13 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
                         const double2 wm = rw[dm[i][j][e] >> 1], wp = rw[dp[i][j][e] >> 1];
                         Mre[i][j][e] += wm.x * cr - wm.y * ci; Mim[i][j][e] += wm.x * ci + wm.y * cr;
                         Pre[i][j][e] += wp.x * cr - wp.y * ci; Pim[i][j][e] += wp.x * ci + wp.y * cr;
+                        if (DUAL) {      // mirror position: same ring weight, conjugate z'-sum  w (cr - i ci)
+                            const int t = ((i * NJ + j) * 2 + e) * 2;
+                            double2 m = sAcc[t * 256 + tid], q = sAcc[(t + 1) * 256 + tid];
+                            m.x += wm.x * cr + wm.y * ci; m.y += wm.y * cr - wm.x * ci;
+                            q.x += wp.x * cr + wp.y * ci; q.y += wp.y * cr - wp.x * ci;
+                            sAcc[t * 256 + tid] = m; sAcc[(t + 1) * 256 + tid] = q;
+                        }
                         Cre[i][j][e] = 0.0; Cim[i][j][e] = 0.0;
                     }
         }
@@ -394,6 +425,12 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     // write partial sums
     const size_t blk = (size_t)a.nq8P * a.nq8T;
     double *o = a.part + ((size_t)p * a.n_split + split) * 6 * blk * 2;
+    double *om = nullptr;                                   // stash slot of the mirror position
+    if (DUAL && a.stash) {
+        const int q = a.q0 + p, g = a.sel.n_idx ? q / a.sel.n_c : 0;
+        const long long i = a.i0 + (sel_pos(a.sel, q) - g * a.sel.n_idx);
+        if (i < a.i_mid && i >= a.i_mid - a.n_st) om = a.stash + ((size_t)g * a.n_st + (size_t)(a.i_mid - i - 1)) * 6 * blk * 2;
+    }
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
@@ -408,6 +445,12 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
                 o[idx] = Mre[i][j][e]; o[idx + 1] = Mim[i][j][e];
                 double *op = o + 3 * blk * 2;
                 op[idx] = Pre[i][j][e]; op[idx + 1] = Pim[i][j][e];
+                if (DUAL && om) {
+                    const int t = ((i * NJ + j) * 2 + e) * 2;
+                    const double2 m = sAcc[t * 256 + tid], q = sAcc[(t + 1) * 256 + tid];
+                    om[idx] = m.x; om[idx + 1] = m.y;
+                    om[3 * blk * 2 + idx] = q.x; om[3 * blk * 2 + idx + 1] = q.y;
+                }
             }
 }
 
@@ -422,7 +465,11 @@ struct TrotArgs {
     const int *lradP;                        // [n_rad_P] l of each projectile radial function
     const TrotChunk *chunks; const int *rowbase;   // rowbase[b]: first local body row of radial function b inside its chunk
     int NT, NP, lmax, max_rows;
-    double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex
+    double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex (p: window position)
+    // block z: evaluated position (fetch == 0): window position sel_pos(sel, q0 + z), integrals part[z];
+    //          fetched position (fetch == 1): z = g * n_fetch + lf -> window position g * n_idx + n_pre + lf,
+    //          integrals in stash slot g * n_st + slot0 + lf
+    SelDev sel; int q0, fetch, n_fetch, n_st, slot0; const double *stash;
 };
 
 // Wigner d^l_{m' m}(beta) = <l m'| e^{-i beta J_y} |l m>, Wigner's sum formula; cb = cos(beta/2), sb = sin(beta/2).
@@ -451,8 +498,18 @@ __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
 //   times (-1)^q for q < 0 and (-1)^q' for q' < 0.
 __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     extern __shared__ __align__(16) double sd[];     // [lmax+1][W][W] Wigner d, W = 2 lmax + 1; then body rows [2][max_rows][nq8T] complex
-    const int p = blockIdx.z, prod = blockIdx.y, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
+    const int prod = blockIdx.y, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
     const TrotChunk ch = a.chunks[blockIdx.x];
+    int p; const double2 *part;              // window position (geometry, outputs) and its body-frame integrals
+    {
+        const size_t per_pos = (size_t)a.n_split * 6 * a.nq8P * a.nq8T;
+        if (!a.fetch) { p = sel_pos(a.sel, a.q0 + blockIdx.z); part = reinterpret_cast<const double2 *>(a.part) + blockIdx.z * per_pos; }
+        else {
+            const int zz = a.q0 + blockIdx.z, g = zz / a.n_fetch, lf = zz - g * a.n_fetch;
+            p = g * a.sel.n_idx + a.sel.n_pre + lf;
+            part = reinterpret_cast<const double2 *>(a.stash) + ((size_t)g * a.n_st + a.slot0 + lf) * per_pos;
+        }
+    }
     const int nd = ((L + 1) * W * W + 1) & ~1;
     double2 *body = reinterpret_cast<double2 *>(sd + nd);
     const int nq8T = a.nq8T, NT = a.NT;
@@ -476,7 +533,6 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     }
     __syncthreads();
     {
-        const double2 *part = reinterpret_cast<const double2 *>(a.part) + (size_t)p * a.n_split * 6 * blk;
         const int per_fam = ch.nrows * nq8T;
         for (int e = tid; e < 2 * per_fam; e += blockDim.x) {
             const int fam = e >= per_fam, r2 = e - fam * per_fam, r = r2 / nq8T, c = r2 - r * nq8T;
@@ -592,9 +648,24 @@ int wp_transfer_default_chunk(const wpccc_basis *B) {
     return c;
 }
 
+size_t wp_transfer_stash_doubles(const wpccc_basis *B) { return make_plan(B, 1).part_per_pos; }
+static size_t dual_smem_bytes(const TransferPlan &P) {
+    return ((size_t)2 * TcRing<true>::STAGES * TcRing<true>::STAGE_DOUBLES + TcRing<true>::ACC_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho) * 8;
+}
+bool wp_transfer_mirror_ok(const wpccc_basis *B) { return dual_smem_bytes(make_plan(B, 1)) <= 226 * 1024; }
+
 int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
-                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s) {
+                const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s,
+                const TransferSel *sel) {
     if (n_pos <= 0) return 0;
+    SelDev sd{0, 0, 0, 0};
+    int n_eval = n_pos, n_fetch = 0;                 // evaluated positions of this call; fetched indices per group
+    if (sel) {
+        if (n_pos != sel->n_groups * sel->n_idx) WP_FAIL(WPCCC_EINVAL, "transfer: selection does not match the window");
+        n_fetch = sel->suf0 - sel->n_pre;
+        sd = SelDev{sel->n_idx - n_fetch, sel->n_idx, sel->n_pre, sel->suf0};
+        n_eval = sel->n_groups * sd.n_c;
+    }
     static bool consts = false;
     if (!consts) {
         double f[2 * WP_MAX_L + 2]; f[0] = 1.0;
@@ -607,8 +678,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     }
     const int max_chunk = wp_transfer_chunk_positions(B, ws_bytes);
     if (max_chunk < 1) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small (%zu bytes)", ws_bytes);
-    chunk = std::max(1, std::min(std::min(chunk, max_chunk), n_pos));
-    const int n_split = pick_split(B, chunk);
+    chunk = std::max(1, std::min(std::min(chunk, max_chunk), std::max(n_eval, 1)));
+    const int n_split = sel ? 1 : pick_split(B, chunk);
     TransferPlan P = make_plan(B, n_split);
 
     // carve the workspace
@@ -669,24 +740,41 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     const int KC = (P.L.n_z % 64 == 0) ? 64 : ((P.L.n_z % 32 == 0) ? 32 : 16);
     const size_t tab_smem = (size_t)(7 + nlq) * KC * 8 + (size_t)KC * 4 + 64;
     static size_t con_attr = 0;
-    const size_t con_smem = ((size_t)2 * TC_STAGES * TC_STAGE_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho) * 8;
+    const size_t con_tabs = 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho;
+    const size_t con_smem = ((size_t)2 * TcRing<false>::STAGES * TcRing<false>::STAGE_DOUBLES + con_tabs) * 8;
+    const size_t dual_smem = dual_smem_bytes(P);
     if (con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
+    // mirror-pair kernel: whenever some evaluated position of this window has a stash slot
+    const bool dual = sel && sel->stash && sel->n_st > 0 && sel->i0 < sel->i_mid && sel->i0 + sel->n_pre > sel->i_mid - sel->n_st;
+    if (dual && dual_smem > 226 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: mirror stash requested but the pair kernel does not fit shared memory");
     static const int tcon_nj = []() { const char *e = getenv("WPCCC_TCON_NJ"); return (e && atoi(e) == 2) ? 2 : 4; }();
     if (con_smem > con_attr) {
-        WP_CUDA(cudaFuncSetAttribute(k_tcon<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
-        WP_CUDA(cudaFuncSetAttribute(k_tcon<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+        WP_CUDA(cudaFuncSetAttribute(k_tcon<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+        WP_CUDA(cudaFuncSetAttribute(k_tcon<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
         con_attr = con_smem;
+    }
+    static size_t dual_attr = 0;
+    if (dual && dual_smem > dual_attr) {
+        WP_CUDA(cudaFuncSetAttribute(k_tcon<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dual_smem));
+        dual_attr = dual_smem;
     }
 
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
-    for (int p0 = 0; p0 < n_pos; p0 += chunk) {
-        const int np = std::min(chunk, n_pos - p0);
-        TposArgs ta{}; ta.L = P.L; ta.R = d_R + p0; ta.cosT = d_cos + p0; ta.sinT = d_sin + p0; ta.v = d_v + p0;
+    TrotArgs tr{}; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta;
+    tr.radT = B->c[0].d_st_rad; tr.lT_st = B->c[0].d_st_l; tr.mT_st = B->c[0].d_st_m;
+    tr.radP = B->c[1].d_st_rad; tr.lP_st = B->c[1].d_st_l; tr.mP_st = B->c[1].d_st_m;
+    tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
+    tr.lmax = lmx; tr.K = d_K; tr.H = d_H;
+    tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
+    tr.sel = sd;
+    for (int p0 = 0; p0 < n_eval; p0 += chunk) {
+        const int np = std::min(chunk, n_eval - p0);
+        TposArgs ta{}; ta.L = P.L; ta.R = d_R; ta.cosT = d_cos; ta.sinT = d_sin; ta.v = d_v; ta.sel = sd; ta.q0 = p0;
         ta.gl_rho = B->d_gl_rho; ta.gl_phi = B->d_gl_phi; ta.gl_zq = B->d_gl_zq; ta.gl_zh = B->d_gl_zh;
         ta.rho_max = B->quad.rho_max; ta.z_pad = B->quad.z_pad; ta.phi_rule = B->quad.phi_rule; ta.out = d_pos;
         wp_span_begin(B, FAM_TTAB, s);
         k_tpos<<<np, 128, 0, s>>>(ta);
-        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R + p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC;
+        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R; tb.sel = sd; tb.q0 = p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC;
         for (int c = 0; c < 2; ++c) {
             tb.Ut[c] = B->c[c].d_Ut; tb.lrad[c] = B->c[c].d_l; tb.n_rad[c] = B->c[c].n_rad; tb.nf_pad[c] = B->c[c].nf_pad;
             tb.nq8[c] = P.nq8[c]; tb.ntile[c] = P.ntile[c]; tb.colidx[c] = d_colidx[c]; tb.out[c] = d_tab[c]; tb.pos_stride[c] = P.stride[c];
@@ -696,27 +784,42 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         dim3 gt(P.L.n_rho * (P.L.n_z / KC), 2, np);
         k_ttab<<<gt, 256, tab_smem, s>>>(tb);
         wp_span_end(B, s, 2);
+        B->units[FAM_TTAB] += np;
         WP_CUDA(cudaGetLastError());
 
         TconArgs tc{}; tc.L = P.L; tc.pos = d_pos; tc.tabT = d_tab[0]; tc.tabP = d_tab[1]; tc.strideT = P.stride[0]; tc.strideP = P.stride[1];
         tc.nq8T = P.nq8[0]; tc.nq8P = P.nq8[1]; tc.ntT = P.ntile[0]; tc.ntP = P.ntile[1]; tc.qT = d_qcol[0]; tc.qP = d_qcol[1];
         tc.tiles = d_tiles; tc.n_tiles = (int)P.tiles.size(); tc.n_split = n_split; tc.part = d_part;
+        tc.sel = sd; tc.q0 = p0;
+        if (dual) { tc.n_st = sel->n_st; tc.i0 = sel->i0; tc.i_mid = sel->i_mid; tc.stash = sel->stash; }
         dim3 gc((unsigned)P.tiles.size(), n_split, np);
         wp_span_begin(B, FAM_TCON, s);
-        if (tcon_nj == 4) k_tcon<4><<<gc, 256, con_smem, s>>>(tc); else k_tcon<2><<<gc, 512, con_smem, s>>>(tc);
+        if (dual) k_tcon<4, true><<<gc, 256, dual_smem, s>>>(tc);
+        else if (tcon_nj == 4) k_tcon<4, false><<<gc, 256, con_smem, s>>>(tc);
+        else k_tcon<2, false><<<gc, 512, con_smem, s>>>(tc);
         wp_span_end(B, s, 1);
+        B->units[FAM_TCON] += np;
         WP_CUDA(cudaGetLastError());
 
-        TrotArgs tr{}; tr.part = d_part; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta + p0;
-        tr.radT = B->c[0].d_st_rad; tr.lT_st = B->c[0].d_st_l; tr.mT_st = B->c[0].d_st_m;
-        tr.radP = B->c[1].d_st_rad; tr.lP_st = B->c[1].d_st_l; tr.mP_st = B->c[1].d_st_m;
-        tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
-        tr.lmax = lmx; tr.K = d_K + (size_t)p0 * NP * NT * 2; tr.H = d_H + (size_t)p0 * N * N * 2;
+        tr.part = d_part; tr.q0 = p0; tr.fetch = 0;
         wp_span_begin(B, FAM_ROT, s);
-        tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
         k_trot<<<dim3((unsigned)rchunks.size(), 3, np), 256, rot_smem, s>>>(tr);
         wp_span_end(B, s, 1);
+        B->units[FAM_ROT] += np;
         WP_CUDA(cudaGetLastError());
+    }
+    if (n_fetch > 0) {       // positions whose integrals an earlier window left in the stash
+        tr.part = nullptr; tr.q0 = 0; tr.fetch = 1; tr.n_fetch = n_fetch; tr.n_st = sel->n_st; tr.stash = sel->stash;
+        tr.slot0 = (int)(sel->i0 + sel->n_pre - sel->i_mid - 1);
+        const int total = sel->n_groups * n_fetch;
+        for (int z0 = 0; z0 < total; z0 += 32768) {
+            tr.q0 = z0;                      // fetch mode: first (g, lf) pair of this launch
+            wp_span_begin(B, FAM_ROT, s);
+            k_trot<<<dim3((unsigned)rchunks.size(), 3, (unsigned)std::min(32768, total - z0)), 256, rot_smem, s>>>(tr);
+            wp_span_end(B, s, 1);
+            WP_CUDA(cudaGetLastError());
+        }
+        B->units[FAM_ROT] += total;
     }
     return 0;
 }

@@ -188,6 +188,33 @@ def test_two_centre_propagation(lib, two_centre):
     assert np.abs(Cs - Cg).max() < 1e-13
 
 
+def test_two_centre_mirror_pairs(lib, two_centre, monkeypatch):
+    """On a z-grid symmetric about 0 the body-frame integrals of (b, -z) and (b, +z) are evaluated together (wpccc.h,
+    wpccc_last_units).  Several windows (150 steps > 64), full and partial stash, against the run with the pairing
+    switched off; and an asymmetric grid, where pairing must switch itself off, against the oracle."""
+    prob, basis = two_centre
+    b, v = np.array([0.7, 1.9, 0.4]), np.array([1.0, 1.3, 1.6])
+    n_steps = 150
+    n_pos = 3 * (2 * n_steps + 3)          # windows of 64, 64, 22 steps; consecutive windows share their boundary position
+    Cm = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
+    um = lib.last_units(basis)
+    assert um["transfer_contraction"] == 3 * (n_steps + 2) and um["rotation"] == n_pos, um       # z <= 0 evaluated, z > 0 fetched
+    base = lib._lib.wpccc_workspace_bytes(basis._h, 3, n_steps, 1)
+    part = lib._lib.wpccc_workspace_bytes(basis._h, 3, 64, 1)                                   # room for 64 of the 150 mirror indices
+    Cp = lib.propagate(basis, b, v, -9.0, 9.0, n_steps, ws_bytes=part).cpu().numpy()
+    up = lib.last_units(basis)
+    assert 3 * (n_steps + 2) < up["transfer_contraction"] < n_pos and part < base, (up, part, base)
+    monkeypatch.setenv("WPCCC_NO_MIRROR", "1")
+    C0 = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
+    assert lib.last_units(basis)["transfer_contraction"] == n_pos
+    monkeypatch.delenv("WPCCC_NO_MIRROR")
+    assert np.abs(Cm - C0).max() < 1e-12 and np.abs(Cp - C0).max() < 1e-12, (np.abs(Cm - C0).max(), np.abs(Cp - C0).max())
+    Ca = lib.propagate(basis, b[:1], v[:1], -6.0, 4.0, 25).cpu().numpy()
+    assert lib.last_units(basis)["transfer_contraction"] == 51
+    co = oprop.propagate(prob, b[0], v[0], -6.0, 4.0, 25)
+    assert np.abs(Ca[0] - co).max() < PTOL
+
+
 def test_argument_errors(lib, one_centre):
     prob, basis = one_centre
     with pytest.raises(lib.WpcccError):
