@@ -231,13 +231,36 @@ __device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigne
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// TMA ring of the contraction: stage = KCS k4-groups of z' nodes per operand (256 doubles each).
-// Plain kernel: 3 stages of 16 groups (192 KB).  Mirror-pair kernel (DUAL): the accumulators of the mirror position
-// take 128 KB of shared memory, so the ring is 5 stages of 4 groups (80 KB).
+// TMA ring of the contraction: 3 stages of 16 k4-groups of z' nodes per operand (256 doubles each), 192 KB.
+// Mirror-pair kernel (DUAL): the 64 accumulators per thread of the mirror position (128 KB per CTA; the register file
+// holds the 96 of the position itself) live in tensor memory, 256 of the SM's 512 TMEM columns, moved with
+// tcgen05.ld / tcgen05.st in the per-ring epilogue: neither registers nor shared-memory bandwidth are spent on them.
 template <bool DUAL> struct TcRing {
-    static constexpr int STAGES = DUAL ? 5 : 3, KCS = DUAL ? 4 : 16, STAGE_DOUBLES = KCS * 256;
-    static constexpr size_t ACC_DOUBLES = DUAL ? 64 * 256 : 0;      // [32 double2][256 threads] (NJ = 4 only)
+    static constexpr int STAGES = 3, KCS = 16, STAGE_DOUBLES = KCS * 256;
+    static constexpr size_t ACC_DOUBLES = 0;
+    static constexpr int TMEM_COLS = 256;
 };
+
+// 16 consecutive 32-bit TMEM columns of this thread's lane (shape 32x32b: lane = 32 (warp % 4) + laneid) <-> 8 doubles
+__device__ __forceinline__ void tmem_ld8(unsigned taddr, double (&d)[8]) {
+    unsigned r[16];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) d[k] = __hiloint2double((int)r[2 * k + 1], (int)r[2 * k]);
+}
+__device__ __forceinline__ void tmem_st8(unsigned taddr, const double (&d)[8]) {
+    unsigned r[16];
+    #pragma unroll
+    for (int k = 0; k < 8; ++k) { r[2 * k] = (unsigned)__double2loint(d[k]); r[2 * k + 1] = (unsigned)__double2hiint(d[k]); }
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};\n"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                    "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
 
 struct TconArgs {
     PosTabs L; const double *pos;
@@ -306,7 +329,7 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     extern __shared__ __align__(128) double sm[];
     double *sA = sm;                                          // [STAGES][TC_STAGE_DOUBLES]  A-side (mma "B" operand)
     double *sB = sA + TC_STAGES * TC_STAGE_DOUBLES;           // [STAGES][TC_STAGE_DOUBLES]  B-side (mma "A" operand)
-    double2 *sAcc = reinterpret_cast<double2 *>(sB + TC_STAGES * TC_STAGE_DOUBLES);   // DUAL: [32][256] mirror accumulators
+    __shared__ unsigned s_tmem;                               // DUAL: base address of the allocated TMEM columns
     double *sCk = sB + TC_STAGES * TC_STAGE_DOUBLES + TcRing<DUAL>::ACC_DOUBLES;      // [n_z][2]
     double *sRw = sCk + 2 * a.L.n_z;                          // [dmax+2][n_rho][2], last row zero (weight of unused elements)
     __shared__ __align__(8) unsigned long long bar[TC_STAGES], empty[TC_STAGES];
@@ -324,12 +347,22 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     for (int i = tid; i < 2 * n_z; i += TC_THREADS) sCk[i] = pt[a.L.off_ck() + i];
     for (int i = tid; i < 2 * (a.L.dmax + 1) * n_rho; i += TC_THREADS) sRw[i] = pt[a.L.off_rw() + i];
     for (int i = tid; i < 2 * n_rho; i += TC_THREADS) sRw[2 * (a.L.dmax + 1) * n_rho + i] = 0.0;
-    if (DUAL) {
-        #pragma unroll
-        for (int k = 0; k < 32; ++k) sAcc[k * 256 + tid] = make_double2(0.0, 0.0);
+    if (DUAL && tid < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&s_tmem)), "n"(TcRing<DUAL>::TMEM_COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::);
     }
     if (tid == 0) { for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&bar[s], 1); mbar_init(&empty[s], NW); } asm volatile("fence.mbarrier_init.release.cluster;\n" ::); }
+    if (DUAL) asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
+    unsigned tacc = 0;            // DUAL: this thread's 128 TMEM columns: lane 32 (warp % 4) + laneid, columns 128 (warp / 4) ..
+    if (DUAL) {
+        asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        tacc = s_tmem + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)(128 * (warp >> 2));
+        const double zero[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        #pragma unroll
+        for (int k = 0; k < 2 * NJ; ++k) tmem_st8(tacc + 16 * k, zero);
+        tmem_wait_st();
+    }
 
     const double *gA = a.tabT + (size_t)p * a.strideT + (size_t)ct * n_rho * nkc * 256;
     const double *gB = a.tabP + (size_t)p * a.strideP + (size_t)rt * n_rho * nkc * 256;
@@ -404,7 +437,9 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
             #pragma unroll
             for (int i = 0; i < 2; ++i)
                 #pragma unroll
-                for (int j = 0; j < NJ; ++j)
+                for (int j = 0; j < NJ; ++j) {
+                    double mir[8];       // DUAL, per e: (M'.re, M'.im, P'.re, P'.im) of the mirror position
+                    if (DUAL) tmem_ld8(tacc + 16 * (i * NJ + j), mir);
                     #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const double cr = Cre[i][j][e], ci = Cim[i][j][e];
@@ -412,14 +447,14 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
                         Mre[i][j][e] += wm.x * cr - wm.y * ci; Mim[i][j][e] += wm.x * ci + wm.y * cr;
                         Pre[i][j][e] += wp.x * cr - wp.y * ci; Pim[i][j][e] += wp.x * ci + wp.y * cr;
                         if (DUAL) {      // mirror position: same ring weight, conjugate z'-sum  w (cr - i ci)
-                            const int t = ((i * NJ + j) * 2 + e) * 2;
-                            double2 m = sAcc[t * 256 + tid], q = sAcc[(t + 1) * 256 + tid];
-                            m.x += wm.x * cr + wm.y * ci; m.y += wm.y * cr - wm.x * ci;
-                            q.x += wp.x * cr + wp.y * ci; q.y += wp.y * cr - wp.x * ci;
-                            sAcc[t * 256 + tid] = m; sAcc[(t + 1) * 256 + tid] = q;
+                            mir[4 * e + 0] += wm.x * cr + wm.y * ci; mir[4 * e + 1] += wm.y * cr - wm.x * ci;
+                            mir[4 * e + 2] += wp.x * cr + wp.y * ci; mir[4 * e + 3] += wp.y * cr - wp.x * ci;
                         }
                         Cre[i][j][e] = 0.0; Cim[i][j][e] = 0.0;
                     }
+                    if (DUAL) tmem_st8(tacc + 16 * (i * NJ + j), mir);
+                }
+            if (DUAL) tmem_wait_st();
         }
     }
     // write partial sums
@@ -434,7 +469,9 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
     #pragma unroll
     for (int i = 0; i < 2; ++i)
         #pragma unroll
-        for (int j = 0; j < NJ; ++j)
+        for (int j = 0; j < NJ; ++j) {
+            double mir[8];
+            if (DUAL) tmem_ld8(tacc + 16 * (i * NJ + j), mir);       // warp-uniform: outside the per-element predicate
             #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 if (!((okmask >> ((i * NJ + j) * 2 + e)) & 1u)) continue;
@@ -446,12 +483,16 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
                 double *op = o + 3 * blk * 2;
                 op[idx] = Pre[i][j][e]; op[idx + 1] = Pim[i][j][e];
                 if (DUAL && om) {
-                    const int t = ((i * NJ + j) * 2 + e) * 2;
-                    const double2 m = sAcc[t * 256 + tid], q = sAcc[(t + 1) * 256 + tid];
-                    om[idx] = m.x; om[idx + 1] = m.y;
-                    om[3 * blk * 2 + idx] = q.x; om[3 * blk * 2 + idx + 1] = q.y;
+                    om[idx] = mir[4 * e]; om[idx + 1] = mir[4 * e + 1];
+                    om[3 * blk * 2 + idx] = mir[4 * e + 2]; om[3 * blk * 2 + idx + 1] = mir[4 * e + 3];
                 }
             }
+        }
+    if (DUAL) {
+        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+        __syncthreads();
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(s_tmem), "n"(TcRing<DUAL>::TMEM_COLS));
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ rotation (a6)
