@@ -348,6 +348,225 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
     if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
 }
 
+// ------------------------------------------------------------------ a7, N_P <= 90: A and the elimination in registers
+// grid = positions; block = 15 worker warps + 1 panel warp.  Worker (ty = warp, tx = lane) owns the elements
+// A[ty + 15 r][tx + 32 s], r < 6, s < 3, in registers for the whole kernel: the Schur complement is accumulated there
+// (K staged in shared memory, row stride odd), and the blocked Gauss-Jordan elimination (panels of FR_NB columns)
+// updates them in place.  Rows are never interchanged: the pivot of column j is the largest entry among the rows not
+// yet used (the same candidates, by row identity, as partial pivoting with interchanges; first maximal row wins), and
+// with piv[j] = that row the inverse is  Ainv[pinv[r]][piv[k]] = G[r][k],  pinv[piv[j]] = j.
+// The panel warp (lane owns rows lane, lane + 32, lane + 64) eliminates the FR_NB columns of a panel in registers
+// with shuffles only; it works one panel ahead: the workers update and hand over the columns of panel p + 1 first,
+// then finish the update of panel p while the panel warp eliminates panel p + 1.
+constexpr int FR_WW = 15, FR_RN = 6, FR_CN = 3, FR_NMAX = FR_WW * FR_RN, FR_WORKERS = 32 * FR_WW, FR_THREADS = FR_WORKERS + 32;
+constexpr int FR_NB = 4;                                              // panel width (the panel warp holds 3 rows of it per lane)
+constexpr int FR_BAR_DONE = 1, FR_BAR_WORK = 2, FR_BAR_PANEL = 3;      // named barriers (0 is unused here)
+
+__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
+
+// Gauss-Jordan steps j0 .. j0 + w - 1 on the panel Pn [n][FR_NB] (shared), by one warp, in registers.
+__device__ __forceinline__ void fr_panel(cplx *Pn, const int n, const int w, const int j0, const int pid, bool (&used)[3],
+                                         int *piv, int *rowpid, int *rowslot, int *s_flag, const int lane) {
+    cplx p[3][FR_NB];
+    #pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const int row = lane + 32 * q;
+        #pragma unroll
+        for (int t = 0; t < FR_NB; ++t) p[q][t] = (row < n) ? Pn[row * FR_NB + t] : cplx{0.0, 0.0};
+    }
+    #pragma unroll
+    for (int t = 0; t < FR_NB; ++t) {
+        if (t < w) {
+            double best = -1.0; int bi = 0x7fffffff;
+            #pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const int row = lane + 32 * q;
+                if (row < n && !used[q]) {
+                    double m = p[q][t].x * p[q][t].x + p[q][t].y * p[q][t].y;
+                    if (!(m == m)) m = 0.0;                       // NaN: flagged below as a zero pivot
+                    if (m > best) { best = m; bi = row; }
+                }
+            }
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double m2 = __shfl_xor_sync(0xffffffffu, best, o); const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
+            }
+            const int pr = bi, ol = pr & 31, oq = pr >> 5;
+            cplx rowv[FR_NB];
+            #pragma unroll
+            for (int tt = 0; tt < FR_NB; ++tt) {
+                const cplx v = (oq == 0) ? p[0][tt] : ((oq == 1) ? p[1][tt] : p[2][tt]);
+                rowv[tt].x = __shfl_sync(0xffffffffu, v.x, ol); rowv[tt].y = __shfl_sync(0xffffffffu, v.y, ol);
+            }
+            const cplx d = rowv[t];
+            const double dn = d.x * d.x + d.y * d.y;
+            const cplx dinv = (dn > 0.0) ? cplx{d.x / dn, -d.y / dn} : cplx{0.0, 0.0};
+            #pragma unroll
+            for (int tt = 0; tt < FR_NB; ++tt) rowv[tt] = (tt == t) ? dinv : cmul(rowv[tt], dinv);
+            #pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const bool isp = (lane + 32 * q == pr);
+                const cplx col = p[q][t];
+                #pragma unroll
+                for (int tt = 0; tt < FR_NB; ++tt) {
+                    const cplx v = (tt == t) ? cplx{0.0, 0.0} : p[q][tt];
+                    p[q][tt] = isp ? rowv[tt] : csub(v, cmul(col, rowv[tt]));
+                }
+                if (isp) used[q] = true;
+            }
+            if (lane == 0) { piv[j0 + t] = pr; rowpid[pr] = pid; rowslot[pr] = t; if (!(best > 0.0)) *s_flag = 1; }
+        }
+    }
+    #pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const int row = lane + 32 * q;
+        if (row < n) {
+            #pragma unroll
+            for (int t = 0; t < FR_NB; ++t) Pn[row * FR_NB + t] = (t < w) ? p[q][t] : cplx{0.0, 0.0};
+        }
+    }
+}
+
+__global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a) {
+    extern __shared__ __align__(16) double sm[];
+    const int n = a.NP, NT = a.NT, cw = a.cw, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const size_t pos = blockIdx.x;
+    cplx *Ks = reinterpret_cast<cplx *>(sm);                          // [n][cw] K chunk; later [n][n] output staging
+    cplx *Pn = Ks + (size_t)n * max(cw, n);                           // [2][FR_NMAX][FR_NB]
+    cplx *W = Pn + 2 * FR_NMAX * FR_NB;                               // [FR_NB][FR_NMAX]
+    int *piv = reinterpret_cast<int *>(W + FR_NB * FR_NMAX), *pinv = piv + FR_NMAX, *rowpid = pinv + FR_NMAX, *rowslot = rowpid + FR_NMAX;
+    __shared__ int s_flag;
+    const int np = (n + FR_NB - 1) / FR_NB;
+
+    if (warp == FR_WORKERS / 32) {                                    // ---- panel warp
+        bool used[3] = {false, false, false};
+        for (int p = 0; p < np; ++p) {
+            bar_sync(FR_BAR_PANEL, FR_THREADS);
+            fr_panel(Pn + (p & 1) * FR_NMAX * FR_NB, n, min(FR_NB, n - p * FR_NB), p * FR_NB, p, used, piv, rowpid, rowslot, &s_flag, lane);
+            bar_sync(FR_BAR_DONE, FR_THREADS);
+        }
+        return;
+    }
+    // ---- workers
+    const int ty = warp, tx = lane;
+    const cplx *K = reinterpret_cast<const cplx *>(a.K) + pos * (size_t)n * NT;
+    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + pos * (size_t)n * n;
+    int rc[FR_RN], cc[FR_CN];                                         // clamped: out-of-range copies are computed, never stored
+    #pragma unroll
+    for (int r = 0; r < FR_RN; ++r) rc[r] = min(ty + FR_WW * r, n - 1);
+    #pragma unroll
+    for (int s = 0; s < FR_CN; ++s) cc[s] = min(tx + 32 * s, n - 1);
+    if (tid == 0) s_flag = 0;
+    if (tid < FR_NMAX) rowpid[tid] = -1;
+    cplx acc[FR_RN][FR_CN];
+    #pragma unroll
+    for (int r = 0; r < FR_RN; ++r)
+        #pragma unroll
+        for (int s = 0; s < FR_CN; ++s) acc[r][s] = cplx{(rc[r] == cc[s]) ? 1.0 : 0.0, 0.0};
+    // A[r][s] = delta_rs - sum_i K[r][i] conj(K[s][i]), i ascending (the elimination order)
+    int bad = 0;
+    for (int i0 = 0; i0 < NT; i0 += cw) {
+        const int w = min(cw, NT - i0);
+        if (i0) bar_sync(FR_BAR_WORK, FR_WORKERS);
+        for (int e = tid; e < n * w; e += FR_WORKERS) {
+            const int r = e / w, ii = e - r * w;
+            const cplx k = K[(size_t)r * NT + i0 + ii];
+            Ks[r * cw + ii] = k;
+            if (!(k.x * k.x + k.y * k.y < 1.0)) bad = 1;              // pivot-order precondition |K_ij| < 1
+        }
+        bar_sync(FR_BAR_WORK, FR_WORKERS);
+        #pragma unroll 2
+        for (int ii = 0; ii < w; ++ii) {
+            cplx kr[FR_RN], ks[FR_CN];
+            #pragma unroll
+            for (int r = 0; r < FR_RN; ++r) kr[r] = Ks[rc[r] * cw + ii];
+            #pragma unroll
+            for (int s = 0; s < FR_CN; ++s) ks[s] = Ks[cc[s] * cw + ii];
+            #pragma unroll
+            for (int r = 0; r < FR_RN; ++r)
+                #pragma unroll
+                for (int s = 0; s < FR_CN; ++s) {
+                    acc[r][s].x -= kr[r].x * ks[s].x + kr[r].y * ks[s].y;
+                    acc[r][s].y -= kr[r].y * ks[s].x - kr[r].x * ks[s].y;
+                }
+        }
+    }
+    if (bad) s_flag = 2;
+
+    // hand the columns of panel q to the panel warp
+    auto write_panel = [&](const int q) {
+        const int j0 = q * FR_NB, wq = min(FR_NB, n - j0);
+        cplx *P = Pn + (q & 1) * FR_NMAX * FR_NB;
+        #pragma unroll
+        for (int s = 0; s < FR_CN; ++s) {
+            const int t = tx + 32 * s - j0;
+            if (t >= 0 && t < wq) {
+                #pragma unroll
+                for (int r = 0; r < FR_RN; ++r) if (ty + FR_WW * r < n) P[(ty + FR_WW * r) * FR_NB + t] = acc[r][s];
+            }
+        }
+        __threadfence_block();
+        bar_arrive(FR_BAR_PANEL, FR_THREADS);
+    };
+    write_panel(0);
+    bool pivrow[FR_RN];
+    for (int p = 0; p < np; ++p) {
+        const int j0 = p * FR_NB, w = min(FR_NB, n - j0);
+        const cplx *P = Pn + (p & 1) * FR_NMAX * FR_NB;
+        bar_sync(FR_BAR_DONE, FR_THREADS);                            // panel p eliminated: P, piv, rowpid
+        #pragma unroll
+        for (int r = 0; r < FR_RN; ++r) {                             // W[t][:] = row piv[j0 + t] before the update
+            const int row = ty + FR_WW * r;
+            pivrow[r] = row < n && rowpid[rc[r]] == p;
+            if (pivrow[r]) {
+                const int t = rowslot[row];
+                #pragma unroll
+                for (int s = 0; s < FR_CN; ++s) if (tx + 32 * s < n) W[t * FR_NMAX + tx + 32 * s] = acc[r][s];
+            }
+        }
+        bar_sync(FR_BAR_WORK, FR_WORKERS);
+        #pragma unroll
+        for (int r = 0; r < FR_RN; ++r)
+            if (pivrow[r]) {                                          // pivot rows of this panel start from zero
+                #pragma unroll
+                for (int s = 0; s < FR_CN; ++s) acc[r][s] = cplx{0.0, 0.0};
+            }
+        auto update_col = [&](const int s) {
+            for (int t = 0; t < w; ++t) {
+                const cplx y = W[t * FR_NMAX + cc[s]];
+                #pragma unroll
+                for (int r = 0; r < FR_RN; ++r) {
+                    const cplx x = P[rc[r] * FR_NB + t];
+                    acc[r][s].x += x.x * y.x - x.y * y.y; acc[r][s].y += x.x * y.y + x.y * y.x;
+                }
+            }
+            const int t = tx + 32 * s - j0;
+            if (t >= 0 && t < w) {                                    // the panel's own columns
+                #pragma unroll
+                for (int r = 0; r < FR_RN; ++r) acc[r][s] = P[rc[r] * FR_NB + t];
+            }
+        };
+        // the column slab that holds the next panel goes first (three copies: register indices stay static)
+        const int sn = (p + 1 < np) ? (j0 + FR_NB) >> 5 : -1;
+        if (sn == 1)      { update_col(1); write_panel(p + 1); update_col(0); update_col(2); }
+        else if (sn == 2) { update_col(2); write_panel(p + 1); update_col(0); update_col(1); }
+        else              { update_col(0); if (sn == 0) write_panel(p + 1); update_col(1); update_col(2); }
+    }
+    // Ainv[pinv[r]][piv[k]] = G[r][k], through shared memory for whole-row stores
+    if (tid < n) pinv[piv[tid]] = tid;
+    bar_sync(FR_BAR_WORK, FR_WORKERS);
+    #pragma unroll
+    for (int r = 0; r < FR_RN; ++r)
+        #pragma unroll
+        for (int s = 0; s < FR_CN; ++s)
+            if (ty + FR_WW * r < n && tx + 32 * s < n) Ks[pinv[ty + FR_WW * r] * n + piv[tx + 32 * s]] = acc[r][s];
+    bar_sync(FR_BAR_WORK, FR_WORKERS);
+    for (int e = tid; e < n * n; e += FR_WORKERS) G[e] = Ks[e];
+    if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)pos + 1); }
+}
+
 // ------------------------------------------------------------------ two-centre sweep
 // grid = trajectories; block = 8 consumer warps + 1 producer warp.  Per RK4 stage, with phase-free H0, K and
 // Ainv = (I - K K^H)^{-1} of the stage's position:
@@ -598,6 +817,22 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
     const size_t budget = 200 * 1024;
     static const bool force_blocked = []() { const char *e = getenv("WPCCC_FACTOR_BLOCKED"); return e && e[0] == '1'; }();   // tests
+    static const bool no_reg = []() { const char *e = getenv("WPCCC_FACTOR_NOREG"); return e && e[0] == '1'; }();            // tests, A/B timing
+    if (n <= (size_t)FR_NMAX && !force_blocked && !no_reg) {                    // A in registers
+        const size_t tail = (2 * FR_NMAX * FR_NB + FR_NB * FR_NMAX) * 16 + 4 * FR_NMAX * 4;
+        size_t cwr = (size_t)a.NT | 1;                                        // odd row stride: conflict-free column reads
+        const size_t cw_max = ((160 * 1024 - tail) / (n * 16) - 1) | 1;
+        if (cwr > cw_max) cwr = cw_max;
+        a.cw = (int)cwr;
+        const size_t smem = n * std::max(cwr, n) * 16 + tail;
+        static size_t attr_r = 0;
+        if (smem > attr_r) { WP_CUDA(cudaFuncSetAttribute(k_factor_reg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_r = smem; }
+        wp_span_begin(B, FAM_FACT, s);
+        k_factor_reg<<<n_pos, FR_THREADS, smem, s>>>(a);
+        wp_span_end(B, s, 1);
+        WP_CUDA(cudaGetLastError());
+        return 0;
+    }
     a.use_smem = !force_blocked && n * n * 16 + n * (2 * FJ_NB + 1) * 16 + small <= budget;   // K chunk area doubles as the panel buffers
     const size_t fixed = (a.use_smem ? n * n * 16 : 0) + small;
     // large N_P (blocked path): two CTAs per SM; the K staging area is reused by the panel buffers (2 FJ_NB + 1 columns)
