@@ -365,58 +365,72 @@ constexpr int FR_BAR_DONE = 1, FR_BAR_WORK = 2, FR_BAR_PANEL = 3;      // named 
 __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
 
-// Gauss-Jordan steps j0 .. j0 + w - 1 on the panel Pn [n][FR_NB] (shared), by one warp, in registers.
-__device__ __forceinline__ void fr_panel(cplx *Pn, const int n, const int w, const int j0, const int pid, bool (&used)[3],
-                                         int *piv, int *rowpid, int *rowslot, int *s_flag, const int lane) {
+// Gauss-Jordan steps j0 .. j0 + w - 1 on the panel Pn [n][FR_NB] (shared), by one warp, in registers.  The warp is
+// alone on the critical path of the whole kernel, so a step is kept short: branch-free pivot search on integer
+// keys (bit pattern of |x|^2 + 1 for a free row, 0 for a used one: the order of non-negative doubles) with three
+// warp reductions, the pivot row passed through shared memory, one reciprocal, one update formula for every row
+// and a fix-up of the pivot row by its owner.  usedmask: bit q = row lane + 32 q already used as a pivot.
+__device__ __forceinline__ void fr_panel(cplx *Pn, const int n, const int w, const int j0, const int pid, unsigned &usedmask,
+                                         int *piv, int *rowpid, int *rowslot, int *s_flag, cplx *rowbuf /*[2][FR_NB]*/, const int lane) {
     cplx p[3][FR_NB];
     #pragma unroll
     for (int q = 0; q < 3; ++q) {
-        const int row = lane + 32 * q;
+        const int row = min(lane + 32 * q, n - 1);                    // rows >= n: copies, marked used by the caller
         #pragma unroll
-        for (int t = 0; t < FR_NB; ++t) p[q][t] = (row < n) ? Pn[row * FR_NB + t] : cplx{0.0, 0.0};
+        for (int t = 0; t < FR_NB; ++t) p[q][t] = Pn[row * FR_NB + t];
     }
     #pragma unroll
     for (int t = 0; t < FR_NB; ++t) {
         if (t < w) {
-            double best = -1.0; int bi = 0x7fffffff;
+            unsigned long long best = 0; int brow = lane;
             #pragma unroll
             for (int q = 0; q < 3; ++q) {
-                const int row = lane + 32 * q;
-                if (row < n && !used[q]) {
-                    double m = p[q][t].x * p[q][t].x + p[q][t].y * p[q][t].y;
-                    if (!(m == m)) m = 0.0;                       // NaN: flagged below as a zero pivot
-                    if (m > best) { best = m; bi = row; }
-                }
+                const double m = p[q][t].x * p[q][t].x + p[q][t].y * p[q][t].y;
+                const unsigned long long key = ((usedmask >> q) & 1u) ? 0ull : (unsigned long long)__double_as_longlong(m) + 1ull;
+                const bool gt = key > best;                           // first maximal row wins within the lane
+                best = gt ? key : best; brow = gt ? lane + 32 * q : brow;
             }
-            #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double m2 = __shfl_xor_sync(0xffffffffu, best, o); const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
+            const unsigned hi = (unsigned)(best >> 32), lo = (unsigned)best;
+            const unsigned H = __reduce_max_sync(0xffffffffu, hi);
+            const unsigned L = __reduce_max_sync(0xffffffffu, hi == H ? lo : 0u);
+            const int pr = (int)__reduce_min_sync(0xffffffffu, (hi == H && lo == L) ? (unsigned)brow : 0x7fffffffu);
+            const int ol = pr & 31, oq = pr >> 5;
+            cplx *rb = rowbuf + (t & 1) * FR_NB;
+            if (lane == ol) {
+                #pragma unroll
+                for (int tt = 0; tt < FR_NB; ++tt) rb[tt] = (oq == 0) ? p[0][tt] : ((oq == 1) ? p[1][tt] : p[2][tt]);
             }
-            const int pr = bi, ol = pr & 31, oq = pr >> 5;
+            __syncwarp();
             cplx rowv[FR_NB];
             #pragma unroll
-            for (int tt = 0; tt < FR_NB; ++tt) {
-                const cplx v = (oq == 0) ? p[0][tt] : ((oq == 1) ? p[1][tt] : p[2][tt]);
-                rowv[tt].x = __shfl_sync(0xffffffffu, v.x, ol); rowv[tt].y = __shfl_sync(0xffffffffu, v.y, ol);
-            }
+            for (int tt = 0; tt < FR_NB; ++tt) rowv[tt] = rb[tt];
             const cplx d = rowv[t];
             const double dn = d.x * d.x + d.y * d.y;
-            const cplx dinv = (dn > 0.0) ? cplx{d.x / dn, -d.y / dn} : cplx{0.0, 0.0};
+            const double inv = (dn > 0.0) ? __drcp_rn(dn) : 0.0;
+            const cplx dinv = {d.x * inv, -d.y * inv};
             #pragma unroll
             for (int tt = 0; tt < FR_NB; ++tt) rowv[tt] = (tt == t) ? dinv : cmul(rowv[tt], dinv);
             #pragma unroll
             for (int q = 0; q < 3; ++q) {
-                const bool isp = (lane + 32 * q == pr);
                 const cplx col = p[q][t];
                 #pragma unroll
                 for (int tt = 0; tt < FR_NB; ++tt) {
                     const cplx v = (tt == t) ? cplx{0.0, 0.0} : p[q][tt];
-                    p[q][tt] = isp ? rowv[tt] : csub(v, cmul(col, rowv[tt]));
+                    p[q][tt] = csub(v, cmul(col, rowv[tt]));
                 }
-                if (isp) used[q] = true;
             }
-            if (lane == 0) { piv[j0 + t] = pr; rowpid[pr] = pid; rowslot[pr] = t; if (!(best > 0.0)) *s_flag = 1; }
+            if (lane == ol) {                                         // the pivot row itself
+                #pragma unroll
+                for (int tt = 0; tt < FR_NB; ++tt) {
+                    if (oq == 0) p[0][tt] = rowv[tt]; else if (oq == 1) p[1][tt] = rowv[tt]; else p[2][tt] = rowv[tt];
+                }
+                usedmask |= 1u << oq;
+            }
+            if (lane == 0) {
+                piv[j0 + t] = pr; rowpid[pr] = pid; rowslot[pr] = t;
+                const double mbest = __longlong_as_double((long long)((((unsigned long long)H << 32) | L) - 1ull));
+                if (!(mbest > 0.0) || H >= 0x7ff00000u) *s_flag = 1;   // zero, infinite or NaN pivot
+            }
         }
     }
     #pragma unroll
@@ -438,13 +452,16 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
     cplx *W = Pn + 2 * FR_NMAX * FR_NB;                               // [FR_NB][FR_NMAX]
     int *piv = reinterpret_cast<int *>(W + FR_NB * FR_NMAX), *pinv = piv + FR_NMAX, *rowpid = pinv + FR_NMAX, *rowslot = rowpid + FR_NMAX;
     __shared__ int s_flag;
+    __shared__ cplx rowbuf[2 * FR_NB];
     const int np = (n + FR_NB - 1) / FR_NB;
 
     if (warp == FR_WORKERS / 32) {                                    // ---- panel warp
-        bool used[3] = {false, false, false};
+        unsigned usedmask = 0;
+        #pragma unroll
+        for (int q = 0; q < 3; ++q) if (lane + 32 * q >= n) usedmask |= 1u << q;
         for (int p = 0; p < np; ++p) {
             bar_sync(FR_BAR_PANEL, FR_THREADS);
-            fr_panel(Pn + (p & 1) * FR_NMAX * FR_NB, n, min(FR_NB, n - p * FR_NB), p * FR_NB, p, used, piv, rowpid, rowslot, &s_flag, lane);
+            fr_panel(Pn + (p & 1) * FR_NMAX * FR_NB, n, min(FR_NB, n - p * FR_NB), p * FR_NB, p, usedmask, piv, rowpid, rowslot, &s_flag, rowbuf, lane);
             bar_sync(FR_BAR_DONE, FR_THREADS);
         }
         return;
@@ -507,8 +524,7 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
                 for (int r = 0; r < FR_RN; ++r) if (ty + FR_WW * r < n) P[(ty + FR_WW * r) * FR_NB + t] = acc[r][s];
             }
         }
-        __threadfence_block();
-        bar_arrive(FR_BAR_PANEL, FR_THREADS);
+        bar_arrive(FR_BAR_PANEL, FR_THREADS);                         // orders the stores above for the waiting panel warp
     };
     write_panel(0);
     bool pivrow[FR_RN];
