@@ -394,12 +394,13 @@ __device__ __forceinline__ void fr_panel(cplx *Pn, const int n, const int w, con
             const unsigned H = __reduce_max_sync(0xffffffffu, hi);
             const unsigned L = __reduce_max_sync(0xffffffffu, hi == H ? lo : 0u);
             const int pr = (int)__reduce_min_sync(0xffffffffu, (hi == H && lo == L) ? (unsigned)brow : 0x7fffffffu);
-            const int ol = pr & 31, oq = pr >> 5;
             cplx *rb = rowbuf + (t & 1) * FR_NB;
-            if (lane == ol) {
-                #pragma unroll
-                for (int tt = 0; tt < FR_NB; ++tt) rb[tt] = (oq == 0) ? p[0][tt] : ((oq == 1) ? p[1][tt] : p[2][tt]);
-            }
+            #pragma unroll
+            for (int q = 0; q < 3; ++q)
+                if (pr == lane + 32 * q) {                            // owner of the pivot row: predicated stores, no selects
+                    #pragma unroll
+                    for (int tt = 0; tt < FR_NB; ++tt) rb[tt] = p[q][tt];
+                }
             __syncwarp();
             cplx rowv[FR_NB];
             #pragma unroll
@@ -414,18 +415,19 @@ __device__ __forceinline__ void fr_panel(cplx *Pn, const int n, const int w, con
             for (int q = 0; q < 3; ++q) {
                 const cplx col = p[q][t];
                 #pragma unroll
-                for (int tt = 0; tt < FR_NB; ++tt) {
+                for (int tt = 0; tt < FR_NB; ++tt) {                  // v - col * rowv as two fma chains
                     const cplx v = (tt == t) ? cplx{0.0, 0.0} : p[q][tt];
-                    p[q][tt] = csub(v, cmul(col, rowv[tt]));
+                    p[q][tt].x = fma(col.y, rowv[tt].y, fma(-col.x, rowv[tt].x, v.x));
+                    p[q][tt].y = fma(-col.y, rowv[tt].x, fma(-col.x, rowv[tt].y, v.y));
                 }
             }
-            if (lane == ol) {                                         // the pivot row itself
-                #pragma unroll
-                for (int tt = 0; tt < FR_NB; ++tt) {
-                    if (oq == 0) p[0][tt] = rowv[tt]; else if (oq == 1) p[1][tt] = rowv[tt]; else p[2][tt] = rowv[tt];
+            #pragma unroll
+            for (int q = 0; q < 3; ++q)
+                if (pr == lane + 32 * q) {                            // the pivot row itself
+                    #pragma unroll
+                    for (int tt = 0; tt < FR_NB; ++tt) p[q][tt] = rowv[tt];
+                    usedmask |= 1u << q;
                 }
-                usedmask |= 1u << oq;
-            }
             if (lane == 0) {
                 piv[j0 + t] = pr; rowpid[pr] = pid; rowslot[pr] = t;
                 const double mbest = __longlong_as_double((long long)((((unsigned long long)H << 32) | L) - 1ull));
@@ -447,8 +449,8 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
     extern __shared__ __align__(16) double sm[];
     const int n = a.NP, NT = a.NT, cw = a.cw, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const size_t pos = blockIdx.x;
-    cplx *Ks = reinterpret_cast<cplx *>(sm);                          // [n][cw] K chunk; later [n][n] output staging
-    cplx *Pn = Ks + (size_t)n * max(cw, n);                           // [2][FR_NMAX][FR_NB]
+    cplx *Ks = reinterpret_cast<cplx *>(sm);                          // [n][cw] K chunk
+    cplx *Pn = Ks + (size_t)n * cw;                                  // [2][FR_NMAX][FR_NB]
     cplx *W = Pn + 2 * FR_NMAX * FR_NB;                               // [FR_NB][FR_NMAX]
     int *piv = reinterpret_cast<int *>(W + FR_NB * FR_NMAX), *pinv = piv + FR_NMAX, *rowpid = pinv + FR_NMAX, *rowslot = rowpid + FR_NMAX;
     __shared__ int s_flag;
@@ -570,16 +572,15 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
         else if (sn == 2) { update_col(2); write_panel(p + 1); update_col(0); update_col(1); }
         else              { update_col(0); if (sn == 0) write_panel(p + 1); update_col(1); update_col(2); }
     }
-    // Ainv[pinv[r]][piv[k]] = G[r][k], through shared memory for whole-row stores
+    // Ainv[pinv[r]][piv[k]] = G[r][k]: a lane's columns piv[tx + 32 s] are consecutive wherever the pivots stayed on
+    // the diagonal, so the stores are mostly whole 512-byte runs; they drain while the next CTA starts
     if (tid < n) pinv[piv[tid]] = tid;
     bar_sync(FR_BAR_WORK, FR_WORKERS);
     #pragma unroll
     for (int r = 0; r < FR_RN; ++r)
         #pragma unroll
         for (int s = 0; s < FR_CN; ++s)
-            if (ty + FR_WW * r < n && tx + 32 * s < n) Ks[pinv[ty + FR_WW * r] * n + piv[tx + 32 * s]] = acc[r][s];
-    bar_sync(FR_BAR_WORK, FR_WORKERS);
-    for (int e = tid; e < n * n; e += FR_WORKERS) G[e] = Ks[e];
+            if (ty + FR_WW * r < n && tx + 32 * s < n) G[(size_t)pinv[ty + FR_WW * r] * n + piv[tx + 32 * s]] = acc[r][s];
     if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)pos + 1); }
 }
 
@@ -840,7 +841,7 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
         const size_t cw_max = ((160 * 1024 - tail) / (n * 16) - 1) | 1;
         if (cwr > cw_max) cwr = cw_max;
         a.cw = (int)cwr;
-        const size_t smem = n * std::max(cwr, n) * 16 + tail;
+        const size_t smem = n * cwr * 16 + tail;
         static size_t attr_r = 0;
         if (smem > attr_r) { WP_CUDA(cudaFuncSetAttribute(k_factor_reg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_r = smem; }
         wp_span_begin(B, FAM_FACT, s);
