@@ -507,8 +507,8 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
             for (int r = 0; r < FR_RN; ++r)
                 #pragma unroll
                 for (int s = 0; s < FR_CN; ++s) {
-                    acc[r][s].x -= kr[r].x * ks[s].x + kr[r].y * ks[s].y;
-                    acc[r][s].y -= kr[r].y * ks[s].x - kr[r].x * ks[s].y;
+                    acc[r][s].x = fma(-kr[r].y, ks[s].y, fma(-kr[r].x, ks[s].x, acc[r][s].x));     // two fma per component
+                    acc[r][s].y = fma(kr[r].x, ks[s].y, fma(-kr[r].y, ks[s].x, acc[r][s].y));
                 }
         }
     }
@@ -557,7 +557,7 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
                 #pragma unroll
                 for (int r = 0; r < FR_RN; ++r) {
                     const cplx x = P[rc[r] * FR_NB + t];
-                    acc[r][s].x += x.x * y.x - x.y * y.y; acc[r][s].y += x.x * y.y + x.y * y.x;
+                    acc[r][s].x = fma(-x.y, y.y, fma(x.x, y.x, acc[r][s].x)); acc[r][s].y = fma(x.y, y.x, fma(x.x, y.y, acc[r][s].y));
                 }
             }
             const int t = tx + 32 * s - j0;
