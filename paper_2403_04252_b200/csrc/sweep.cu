@@ -496,7 +496,7 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
             if (!(k.x * k.x + k.y * k.y < 1.0)) bad = 1;              // pivot-order precondition |K_ij| < 1
         }
         bar_sync(FR_BAR_WORK, FR_WORKERS);
-        #pragma unroll 2
+        #pragma unroll 1
         for (int ii = 0; ii < w; ++ii) {
             cplx kr[FR_RN], ks[FR_CN];
             #pragma unroll
