@@ -833,8 +833,9 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     a.K = d_K; a.Ainv = d_Ainv; a.status = B->d_status; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states;
     const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
     const size_t budget = 200 * 1024;
-    static const bool force_blocked = []() { const char *e = getenv("WPCCC_FACTOR_BLOCKED"); return e && e[0] == '1'; }();   // tests
-    static const bool no_reg = []() { const char *e = getenv("WPCCC_FACTOR_NOREG"); return e && e[0] == '1'; }();            // tests, A/B timing
+    auto env_on = [](const char *name) { const char *e = getenv(name); return e && e[0] == '1'; };
+    const bool force_blocked = env_on("WPCCC_FACTOR_BLOCKED");               // tests: global-memory blocked route
+    const bool no_reg = env_on("WPCCC_FACTOR_NOREG");                        // tests, A/B timing: shared-memory route
     if (n <= (size_t)FR_NMAX && !force_blocked && !no_reg) {                    // A in registers
         const size_t tail = (2 * FR_NMAX * FR_NB + FR_NB * FR_NMAX) * 16 + 4 * FR_NMAX * 4;
         size_t cwr = (size_t)a.NT | 1;                                        // odd row stride: conflict-free column reads
@@ -859,6 +860,7 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     int cw = (int)std::min<size_t>((kbudget - fixed) / (n * 16), (size_t)a.NT);
     if (cw > 1 && (cw & 1) == 0) --cw;                        // odd width: conflict-free column reads
     if (cw < 1) WP_FAIL(WPCCC_EINVAL, "factorisation: N_P = %d too large", a.NP);
+    if (a.use_smem && cw < 2 * FJ_NB + 1) cw = 2 * FJ_NB + 1;    // the K chunk area doubles as the panel buffers (N_T < 17)
     a.cw = cw;
     const size_t smem = a.use_smem ? fixed + n * cw * 16 : std::max(fixed + n * cw * 16, blocked_need);
     static size_t attr = 0;

@@ -215,6 +215,25 @@ def test_two_centre_mirror_pairs(lib, two_centre, monkeypatch):
     assert np.abs(Ca[0] - co).max() < PTOL
 
 
+def test_two_centre_factor_routes(lib, two_centre, monkeypatch):
+    """The three routes of the a7 factorisation (matrix in registers for N_P <= 90, in shared memory, blocked in global
+    memory) choose the same pivots and differ by rounding only; each against the oracle.  N_P = 32 (whole panels) and
+    N_P = 9 (one lane group, ragged last panel)."""
+    small = tiny_problem(True, l_max=1, n_max=2, bins=1, k_max=1.5, Nr=300, h=0.1, quad=dict(QUAD), seed=5)
+    for prob, basis, b, v, zr, n_steps in ((two_centre[0], two_centre[1], np.array([0.3, 1.1]), np.array([0.9, 1.4]), 7.0, 30),
+                                           (small, lib.setup_basis(small), np.array([0.5]), np.array([1.2]), 6.0, 24)):
+        out = {}
+        for route, env in (("registers", None), ("shared", "WPCCC_FACTOR_NOREG"), ("blocked", "WPCCC_FACTOR_BLOCKED")):
+            if env: monkeypatch.setenv(env, "1")
+            out[route] = lib.propagate(basis, b, v, -zr, zr, n_steps).cpu().numpy()
+            if env: monkeypatch.delenv(env)
+        for t in range(len(b)):
+            co = oprop.propagate(prob, b[t], v[t], -zr, zr, n_steps)
+            for route, C in out.items():
+                assert np.abs(C[t] - co).max() < PTOL, (route, t, np.abs(C[t] - co).max())
+        assert np.abs(out["registers"] - out["shared"]).max() < 1e-11 and np.abs(out["blocked"] - out["shared"]).max() < 1e-11
+
+
 def test_argument_errors(lib, one_centre):
     prob, basis = one_centre
     with pytest.raises(lib.WpcccError):
