@@ -438,17 +438,23 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
             for (int i = 0; i < 2; ++i)
                 #pragma unroll
                 for (int j = 0; j < NJ; ++j) {
-                    double mir[8];       // DUAL, per e: (M'.re, M'.im, P'.re, P'.im) of the mirror position
+                    double mir[8];       // DUAL, per e: B of family (-) and of family (+), see below
                     if (DUAL) tmem_ld8(tacc + 16 * (i * NJ + j), mir);
                     #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const double cr = Cre[i][j][e], ci = Cim[i][j][e];
                         const double2 wm = rw[dm[i][j][e] >> 1], wp = rw[dp[i][j][e] >> 1];
-                        Mre[i][j][e] += wm.x * cr - wm.y * ci; Mim[i][j][e] += wm.x * ci + wm.y * cr;
-                        Pre[i][j][e] += wp.x * cr - wp.y * ci; Pim[i][j][e] += wp.x * ci + wp.y * cr;
-                        if (DUAL) {      // mirror position: same ring weight, conjugate z'-sum  w (cr - i ci)
-                            mir[4 * e + 0] += wm.x * cr + wm.y * ci; mir[4 * e + 1] += wm.y * cr - wm.x * ci;
-                            mir[4 * e + 2] += wp.x * cr + wp.y * ci; mir[4 * e + 3] += wp.y * cr - wp.x * ci;
+                        if (DUAL) {
+                            // The mirror position has the same ring weight and the conjugate z'-sum, w (cr - i ci).  With
+                            // A = sum_ring w cr (registers) and B = sum_ring w ci (tensor memory), both complex, the pair is
+                            // M = A + i B and M' = A - i B: eight plain fma per element and ring for both positions.
+                            Mre[i][j][e] = fma(wm.x, cr, Mre[i][j][e]); Mim[i][j][e] = fma(wm.y, cr, Mim[i][j][e]);
+                            Pre[i][j][e] = fma(wp.x, cr, Pre[i][j][e]); Pim[i][j][e] = fma(wp.y, cr, Pim[i][j][e]);
+                            mir[4 * e + 0] = fma(wm.x, ci, mir[4 * e + 0]); mir[4 * e + 1] = fma(wm.y, ci, mir[4 * e + 1]);
+                            mir[4 * e + 2] = fma(wp.x, ci, mir[4 * e + 2]); mir[4 * e + 3] = fma(wp.y, ci, mir[4 * e + 3]);
+                        } else {
+                            Mre[i][j][e] += wm.x * cr - wm.y * ci; Mim[i][j][e] += wm.x * ci + wm.y * cr;
+                            Pre[i][j][e] += wp.x * cr - wp.y * ci; Pim[i][j][e] += wp.x * ci + wp.y * cr;
                         }
                         Cre[i][j][e] = 0.0; Cim[i][j][e] = 0.0;
                     }
@@ -479,12 +485,17 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
                 const int hr = gr / a.nq8P, ir = gr % a.nq8P, hc = gc / a.nq8T, ic = gc % a.nq8T;
                 const int prod = hr ? 2 : (hc ? 1 : 0);
                 const size_t idx = ((size_t)prod * blk + (size_t)ir * a.nq8T + ic) * 2;
-                o[idx] = Mre[i][j][e]; o[idx + 1] = Mim[i][j][e];
                 double *op = o + 3 * blk * 2;
-                op[idx] = Pre[i][j][e]; op[idx + 1] = Pim[i][j][e];
-                if (DUAL && om) {
-                    om[idx] = mir[4 * e]; om[idx + 1] = mir[4 * e + 1];
-                    om[3 * blk * 2 + idx] = mir[4 * e + 2]; om[3 * blk * 2 + idx + 1] = mir[4 * e + 3];
+                if (DUAL) {          // M = A + i B here, M' = A - i B for the mirror position
+                    o[idx] = Mre[i][j][e] - mir[4 * e + 1]; o[idx + 1] = Mim[i][j][e] + mir[4 * e];
+                    op[idx] = Pre[i][j][e] - mir[4 * e + 3]; op[idx + 1] = Pim[i][j][e] + mir[4 * e + 2];
+                    if (om) {
+                        om[idx] = Mre[i][j][e] + mir[4 * e + 1]; om[idx + 1] = Mim[i][j][e] - mir[4 * e];
+                        om[3 * blk * 2 + idx] = Pre[i][j][e] + mir[4 * e + 3]; om[3 * blk * 2 + idx + 1] = Pim[i][j][e] - mir[4 * e + 2];
+                    }
+                } else {
+                    o[idx] = Mre[i][j][e]; o[idx + 1] = Mim[i][j][e];
+                    op[idx] = Pre[i][j][e]; op[idx + 1] = Pim[i][j][e];
                 }
             }
         }
