@@ -743,7 +743,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     int2 *d_tiles = (int2 *)take(P.tiles.size() * sizeof(int2));
     int *d_colidx[2], *d_qcol[2];
     for (int c = 0; c < 2; ++c) { d_colidx[c] = (int *)take((size_t)B->c[c].n_rad * (WP_MAX_L + 1) * 4); d_qcol[c] = (int *)take((size_t)B->c[c].nqc_pad * 4); }
-    // rotation chunks: consecutive projectile radial functions whose body rows (both families) fit ~100 KB of shared memory
+    // rotation chunks: consecutive projectile radial functions whose body rows (both families) fit ~48 KB of shared memory
     const int lmx = std::max(B->c[0].l_max, B->c[1].l_max);
     const size_t rot_nd = (((size_t)(lmx + 1) * (2 * lmx + 1) * (2 * lmx + 1) + 1) & ~(size_t)1) * 8;
     std::vector<TrotChunk> rchunks; std::vector<int> rowbase(B->c[1].n_rad, 0);
@@ -751,7 +751,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     {
         const CentreTab &C = B->c[1];
         const size_t rot_fixed = rot_nd + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
-        const int cap = std::min(256, std::max(C.l_max + 1, (int)((100 * 1024 - rot_fixed) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
+        const size_t rot_target = 48 * 1024;       // four CTAs per SM hide the staging latency (cfg 1: 36.8 ms at 100 KB, 26.6 ms at 48 KB)
+        const int cap = std::min(256, std::max(C.l_max + 1, (int)((rot_target - rot_fixed) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
         TrotChunk cur{0, 0, 0, 0, 0};
         for (int b = 0; b < C.n_rad; ++b) {
             if (cur.nrows + C.l[b] + 1 > cap) { rchunks.push_back(cur); cur = TrotChunk{b, b, C.rad_first[b], 0, 0}; }
