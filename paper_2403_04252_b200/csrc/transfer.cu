@@ -124,10 +124,14 @@ struct TtabArgs {
     SelDev sel; int q0;
 };
 
+__device__ __forceinline__ void st_global_256(double *p, const double (&v)[4]) {       // p 32-byte aligned (sm_100: STG.256)
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};\n" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+}
+
 // grid = (ring * n_kchunks, side, position), block = 256, dynamic smem (per-node quantities only).
-// Phase 1: one thread per node: geometry, Lagrange weights, Theta~_{lq}.  Phase 2: a warp covers 4 nodes x 8
-// radial functions (lane = 4 * (a % 8) + node % 4, the fragment order), interpolates (u_a, g_a) with one 16-byte
-// load per stencil point and stores X, Xh for q = 0..l_a straight into the fragment-major table.
+// Phase 1: one thread per node: geometry, Lagrange weights, Theta~_{lq}.  Phase 2: a warp takes a k4-group of 4 nodes,
+// lane = radial function: it interpolates (u_a, g_a) at the four nodes with one 16-byte load per stencil point and
+// stores X, Xh for q = 0..l_a straight into the fragment-major table, 32 bytes (4 nodes of one column) per store.
 __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     extern __shared__ __align__(16) double sm[];
     const int side = blockIdx.y, p = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -180,34 +184,45 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
     __syncthreads();
     const double2 *Ut = reinterpret_cast<const double2 *>(a.Ut[side]);
     const int nr = a.n_rad[side], nf2 = a.nf_pad[side] / 2;        // row stride in (u, g) pairs
-    const int ai = lane >> 2, kn = lane & 3;
     double *out = a.out[side] + (size_t)p * a.pos_stride[side];
+    // lane = radial function: a stencil row of all functions is ONE contiguous run per request (16 n_rad bytes), and a
+    // lane owns the four z' nodes of its columns in a k4-group, i.e. one whole 32-byte sector per (column, k4-group),
+    // written with a single 256-bit store
     for (int kcl = warp; kcl < KC / 4; kcl += 8) {
-        const int n = kcl * 4 + kn, j = sJ[n];
-        const double L0 = sLag[n], L1 = sLag[KC + n], L2 = sLag[2 * KC + n], L3 = sLag[3 * KC + n], L4 = sLag[4 * KC + n];
-        const double rinv = sRinv[n], pot = sPot[n];
-        double *dst = out + ((size_t)ring * nkc + (k0 / 4 + kcl)) * 256 + kn;
-        for (int aa = ai; aa < nr; aa += 8) {
-            double fu = 0.0, fg = 0.0;
-            if (j >= 0) {
-                const double2 *row = Ut + (size_t)(j - 2) * nf2 + aa;
-                const double2 v0 = row[0], v1 = row[nf2], v2 = row[2 * nf2], v3 = row[3 * nf2], v4 = row[4 * nf2];
-                fu = L0 * v0.x; fg = L0 * v0.y;
-                fu += L1 * v1.x; fg += L1 * v1.y;
-                fu += L2 * v2.x; fg += L2 * v2.y;
-                fu += L3 * v3.x; fg += L3 * v3.y;
-                fu += L4 * v4.x; fg += L4 * v4.y;
-                fu *= rinv; fg *= rinv;
+        double *dst = out + ((size_t)ring * nkc + (k0 / 4 + kcl)) * 256;
+        for (int aa = lane; aa < nr; aa += 32) {
+            double fu[4], fg[4], pt4[4];
+            #pragma unroll
+            for (int kn = 0; kn < 4; ++kn) {
+                const int n = kcl * 4 + kn, j = sJ[n];
+                fu[kn] = 0.0; fg[kn] = 0.0; pt4[kn] = sPot[n];
+                if (j >= 0) {
+                    const double L0 = sLag[n], L1 = sLag[KC + n], L2 = sLag[2 * KC + n], L3 = sLag[3 * KC + n], L4 = sLag[4 * KC + n];
+                    const double rinv = sRinv[n];
+                    const double2 *row = Ut + (size_t)(j - 2) * nf2 + aa;
+                    const double2 v0 = row[0], v1 = row[nf2], v2 = row[2 * nf2], v3 = row[3 * nf2], v4 = row[4 * nf2];
+                    double u = L0 * v0.x, g = L0 * v0.y;
+                    u += L1 * v1.x; g += L1 * v1.y;
+                    u += L2 * v2.x; g += L2 * v2.y;
+                    u += L3 * v3.x; g += L3 * v3.y;
+                    u += L4 * v4.x; g += L4 * v4.y;
+                    fu[kn] = u * rinv; fg[kn] = g * rinv;
+                }
             }
             const int l = a.lrad[side][aa];
             const int *cix = a.colidx[side] + aa * (WP_MAX_L + 1);
-            const double *th_l = sTh + (size_t)lq_index(l, 0) * KC + n;
+            const double *th_l = sTh + (size_t)lq_index(l, 0) * KC + kcl * 4;
             for (int q = 0; q <= l; ++q) {
                 const int col = cix[q], colh = nq8 + col;
-                const double th = th_l[q * KC];
-                const double X = fu * th, Xg = fg * th;
-                dst[(col >> 6) * tile_stride + (col & 63) * 4] = X;
-                dst[(colh >> 6) * tile_stride + (colh & 63) * 4] = pot * X + Xg;
+                double X[4], Xh[4];
+                #pragma unroll
+                for (int kn = 0; kn < 4; ++kn) {
+                    const double th = th_l[q * KC + kn];
+                    const double Xg = fg[kn] * th;
+                    X[kn] = fu[kn] * th; Xh[kn] = pt4[kn] * X[kn] + Xg;
+                }
+                st_global_256(dst + (size_t)(col >> 6) * tile_stride + (col & 63) * 4, X);
+                st_global_256(dst + (size_t)(colh >> 6) * tile_stride + (colh & 63) * 4, Xh);
             }
         }
     }
