@@ -355,7 +355,8 @@ extern "C" int wpccc_propagate(const wpccc_basis *Bc, int n_traj, const double *
         k_geometry_grid<<<(n_pos + 127) / 128, 128, 0, e>>>(n_groups, n_idx, d_b, two ? d_v : nullptr, i0, z_min, h, g);
         wp_span_end(B, e, 1);
         if (two) {
-            WP_CUDA(cudaMemsetAsync(d_H[buf], 0, (size_t)n_pos * N * N * 16, e));
+            // no clearing of d_H[buf]: the assembly kernels write every element of D^T, D^P and the rotation kernel every
+            // element of H_PT, H_TP at every position of the window (evaluated or fetched from the mirror stash)
             if (mirror) {
                 sel.n_idx = n_idx; sel.i0 = i0;
                 sel.n_pre = (int)std::max<long long>(0, std::min<long long>(n_idx, sel.i_mid + 1 - i0));
