@@ -98,7 +98,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) k_direct_gemm(const GemmArgs 
         #pragma unroll
         for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
 
-    const int wm = (warp >> 2) * 64, wn = (warp & 3) * 32;
+    // warps w and w + 4 share an SM sub-partition: give them N offsets 64 apart, so that a ragged tile (cnt <= 64) leaves
+    // one active warp on every sub-partition instead of two sub-partitions idle
+    const int wm = (warp & 1) * 64, wn = (warp >> 1) * 32;
     const bool warp_active = (wn < t.cnt);
     const int fr = lane >> 2, fk = lane & 3;
 
