@@ -170,8 +170,8 @@ extern "C" size_t wpccc_workspace_bytes(const wpccc_basis *B, int n_traj, int n_
     if (!B || n_traj < 1) return 0;
     if (what == 0) {
         const size_t N = B->n_tot;
-        size_t per = 6 * 8 + (size_t)B->E_tot * 8 + 64;
-        if (B->n_centres == 2) per += (size_t)B->c[0].n_states * B->c[1].n_states * 16 + N * N * 16;
+        size_t per = 9 * 8 + (size_t)B->E_tot * 8 + 64 + N * N * 16;           // the terms wpccc_matrix_elements checks (H scratch when no H output)
+        if (B->n_centres == 2) per += (size_t)B->c[0].n_states * B->c[1].n_states * 16;
         size_t tot = per * (size_t)n_traj + 65536;
         if (B->n_centres == 2) tot += align256(wp_transfer_ws_bytes(B, std::min(n_traj, wp_transfer_default_chunk(B))));
         return tot;

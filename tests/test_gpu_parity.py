@@ -241,3 +241,15 @@ def test_argument_errors(lib, one_centre):
     with pytest.raises(lib.WpcccError):
         lib.propagate(basis, [1.0], [1.0], -1.0, 1.0, 10, ws_bytes=1024)   # workspace too small
     assert lib.propagate(basis, np.zeros(0), np.zeros(0), -1.0, 1.0, 10).shape == (0, basis.n_tot)   # empty batch
+
+
+def test_workspace_query_is_sufficient_for_a_first_call(lib):
+    """wpccc_workspace_bytes(what = 0) must cover wpccc_matrix_elements on a fresh basis (no larger workspace cached by
+    an earlier call): one centre and two centres, with and without the H output."""
+    for two in (False, True):
+        prob = tiny_problem(two, l_max=1, n_max=2, bins=2, k_max=2.0, Nr=300, h=0.1, quad=dict(QUAD) if two else None, seed=5 if two else None)
+        for kw in ({}, {"want_H": False}, {"want_S": False}):
+            basis = lib.setup_basis(prob)
+            out = lib.matrix_elements(basis, [0.8, 1.1, 0.3], [-0.6, 0.2, 1.4], [1.2, 1.2, 0.9], **kw)
+            assert all(t is None or bool(t.isfinite().all()) for t in out)
+            basis.close()
