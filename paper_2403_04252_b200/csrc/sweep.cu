@@ -841,6 +841,7 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
         size_t cwr = (size_t)a.NT | 1;                                        // odd row stride: conflict-free column reads
         const size_t cw_max = ((160 * 1024 - tail) / (n * 16) - 1) | 1;
         if (cwr > cw_max) cwr = cw_max;
+        if (const char *e = getenv("WPCCC_FACTOR_CW")) { const size_t t = (size_t)std::max(1, atoi(e)) | 1; if (t < cwr) cwr = t; }   // tests: K staged in several chunks
         a.cw = (int)cwr;
         const size_t smem = n * cwr * 16 + tail;
         static size_t attr_r = 0;

@@ -223,15 +223,17 @@ def test_two_centre_factor_routes(lib, two_centre, monkeypatch):
     for prob, basis, b, v, zr, n_steps in ((two_centre[0], two_centre[1], np.array([0.3, 1.1]), np.array([0.9, 1.4]), 7.0, 30),
                                            (small, lib.setup_basis(small), np.array([0.5]), np.array([1.2]), 6.0, 24)):
         out = {}
-        for route, env in (("registers", None), ("shared", "WPCCC_FACTOR_NOREG"), ("blocked", "WPCCC_FACTOR_BLOCKED")):
-            if env: monkeypatch.setenv(env, "1")
+        for route, env, val in (("registers", None, None), ("registers, K staged in chunks of 5 columns", "WPCCC_FACTOR_CW", "5"),
+                                ("shared", "WPCCC_FACTOR_NOREG", "1"), ("blocked", "WPCCC_FACTOR_BLOCKED", "1")):
+            if env: monkeypatch.setenv(env, val)
             out[route] = lib.propagate(basis, b, v, -zr, zr, n_steps).cpu().numpy()
             if env: monkeypatch.delenv(env)
         for t in range(len(b)):
             co = oprop.propagate(prob, b[t], v[t], -zr, zr, n_steps)
             for route, C in out.items():
                 assert np.abs(C[t] - co).max() < PTOL, (route, t, np.abs(C[t] - co).max())
-        assert np.abs(out["registers"] - out["shared"]).max() < 1e-11 and np.abs(out["blocked"] - out["shared"]).max() < 1e-11
+        for route, C in out.items():
+            assert np.abs(C - out["shared"]).max() < 1e-11, route
 
 
 def test_argument_errors(lib, one_centre):
