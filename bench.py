@@ -1,19 +1,23 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the WP-CCC hot path on B200 (contract: see DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--no-per-config]
 
 One "step" = one pass of the whole hot path over one batch: wpccc_propagate of every
 trajectory of the workload (geometry, direct GEMM + assembly, transfer tables + contraction + rotation, factorisation,
-RK4 sweep) followed by wpccc_probabilities.  The workload is BASELINE.json configs[1] (two-centre p + H with electron
-transfer: 172 states, quadrature 64 x 16 x 128, 16 impact parameters, 1600 RK4 steps), the smallest configuration that
-exercises every row; inputs are seeded and synthetic (wpccc_inputs).  metric = trajectory * RK4-steps / s.
+RK4 sweep) followed by wpccc_probabilities.  The headline workload is BASELINE.json configs[3], the largest
+single-GPU configuration (BASELINE.json quotes its metric on no particular one): He2+ + H two-centre, 572 states,
+quadrature 96 x 24 x 192, 128 impact parameters.  Its whole job (3000 RK4 steps) takes minutes, so a step is one window
+of 64 RK4 steps of the configured size of all 128 trajectories, successive steps walking through the configured z-range
+from z_min with the amplitudes carried over (wpccc_propagate, WPCCC_INIT_FROM_DC); metric = trajectory * RK4-steps / s
+is intensive.  The same run then measures the other four configurations for a few steps each (key `per_config`; whole
+jobs).  Inputs are seeded and synthetic (wpccc_inputs).
 
 `value`: basis tables already resident in HBM (a0 staged once, outside the timed region).
-`e2e`:   the same job from HOST buffers: wpccc_setup_basis (H2D of the radial tables) + propagate + probabilities
-         + D2H of the probabilities and cross sections, all inside the timed region.
-N > 1 (torchrun): the 16 N impact parameters are sharded round-robin, 16 per rank (weak scaling); the only exchange
-is the all-gather of the final amplitudes before the cross-section integral (paper_2403_04252_b200/shard.py).
+`e2e`:   the same step from HOST buffers: wpccc_setup_basis (H2D of the radial tables) + H2D of the amplitudes a window
+         continues from + propagate + probabilities + D2H of the probabilities and cross sections, all timed.
+N > 1 (torchrun): the impact parameters are refined N-fold over the same range and sharded round-robin (weak scaling);
+the only exchange is the all-gather of the final amplitudes before the cross-section integral (shard.py).
 --impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -139,6 +143,130 @@ def family_work(prob, b_local, n_steps, units=None):
     return out
 
 
+# What one bench "step" is for each configuration: the whole job where that takes seconds, else one window of RK4 steps of
+# the configured size, successive steps walking through the configured z-range from z_min (amplitudes carried over,
+# WPCCC_INIT_FROM_DC); the metric trajectory*RK4-steps/s is intensive, so a window measures the rate of the whole job.
+STEP_WINDOW = {0: None, 1: None, 2: None, 3: 64, 4: None}
+
+
+class Job:
+    """One configuration staged on the GPU and its bench step."""
+
+    def __init__(self, wp, cfg, world, rank, window=None, direct_tables=False):
+        self.wp, self.cfg = wp, cfg
+        self.prob, run, self.mine = workload(cfg, world, rank)
+        self.b_all, self.v_all, self.vg_all = run["b"], run["v"], run["vgroup"]
+        self.b, self.v = self.b_all[self.mine], self.v_all[self.mine]
+        self.n_steps_job, self.z0, self.z1 = run["n_steps"], run["z_min"], run["z_max"]
+        self.hz = (self.z1 - self.z0) / self.n_steps_job
+        self.window = min(window, self.n_steps_job) if window else None
+        self.n_steps = self.window or self.n_steps_job            # RK4 steps per bench step
+        self.n_vg = int(self.vg_all.max()) + 1
+        self.basis = wp.setup_basis(self.prob)
+        if direct_tables:
+            self.basis.enable_direct_tables(True)
+        self.k, self.C, self.n_singular = 0, None, 0
+        self.world, self.rank = world, rank
+
+    def span(self):
+        """z-range of the next step."""
+        if not self.window:
+            return self.z0, self.z1, None
+        per_job = self.n_steps_job // self.window
+        k = self.k % per_job
+        if k == 0:
+            self.C = None                                           # (re)start at z_min with c = 1s
+        za = self.z0 + k * self.window * self.hz
+        return za, za + self.window * self.hz, self.C
+
+    def step(self, basis=None, C0="walk"):
+        from paper_2403_04252_b200.shard import gather_amplitudes
+        wp, basis = self.wp, basis or self.basis
+        za, zb, Cw = self.span()
+        C = wp.propagate(basis, self.b, self.v, za, zb, self.n_steps, C0=Cw if C0 == "walk" else C0, allow_singular=True)
+        if C0 == "walk":
+            self.C, self.k = C, self.k + 1
+        Call = gather_amplitudes(C, len(self.b_all), self.rank, self.world)
+        return wp.probabilities(basis, Call, b=self.b_all, vgroup=self.vg_all, n_vgroups=self.n_vg)
+
+    def describe(self):
+        prob = self.prob
+        kind = ("two-centre, Z_P=%g, quadrature %dx%dx%d" % (prob.Z_proj, prob.quad["n_rho"], prob.quad["n_phi"], prob.quad["n_z"])) if prob.quad else "one-centre"
+        what = ("one window of %d RK4 steps of the configured size (h=%.4g) of all trajectories per step, successive steps walking through z from z_min=%g "
+                "(amplitudes carried over); the full job is %d such steps" % (self.window, self.hz, self.z0, self.n_steps_job)) if self.window else \
+               ("the whole job per step: z in [%g, %g], %d RK4 steps" % (self.z0, self.z1, self.n_steps_job))
+        return "BASELINE.json configs[%d]: %s, N_tot=%d states, %d trajectories; %s" % (self.cfg, kind, self.basis.n_tot, len(self.b_all), what)
+
+    def close(self):
+        self.basis.close()
+        self.basis = None
+        self.C = None
+
+
+def measure(job, torch, dist, world, n_warm, n_timed, flush, sampler=None):
+    """Times n_timed steps of the job (CUDA events on the current stream, L2 flushed between steps, max over ranks);
+    returns (ms_per_step, family times, launches, units per family, clock marks)."""
+    wp = job.wp
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(n_warm):
+        job.step()
+    barrier()
+    m0 = sampler.mark() if sampler else 0
+    evs, launches, fam_ms, units_step = [], 0, {}, {}
+    for _ in range(n_timed):
+        flush.fill_(1)                                                     # L2 flush between timed iterations
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        job.step()
+        e1.record()
+        evs.append((e0, e1))
+        tm = wp.last_timing(job.basis)                                     # synchronises; per-family event times of this step
+        launches += sum(n for _, n in tm.values()) + 4                     # + init amplitudes, probabilities, 2 x cross sections
+        units_step = wp.last_units(job.basis)                              # positions per family of this step
+        st = wp.last_status(job.basis, len(job.b))
+        job.n_singular = max(job.n_singular, sum(1 for x in st if x is not None))
+        for k, (ms, n) in tm.items():
+            a = fam_ms.setdefault(k, [0.0, 0])
+            a[0] += ms; a[1] += n
+    barrier()
+    m1 = sampler.mark() if sampler else 0
+    ms_step = sum(e0.elapsed_time(e1) for e0, e1 in evs) / n_timed
+    t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item()), fam_ms, launches, units_step, (m0, m1)
+
+
+def families(job, fam_ms, n_timed, units_step, pk, dmma, dfma, direct_tables=False):
+    work = family_work(job.prob, job.b, job.n_steps, units_step)
+    if direct_tables:                                                      # NEXT-1: 16 B read + 8 B written per entry and position
+        work["direct_gemm"] = ("hbm", work["direct_gemm"][1] / (2.0 * job.prob.Nr) * 24.0, "byte")
+    fams = {}
+    for k, (ms, n) in fam_ms.items():
+        if n == 0 or k not in work:
+            continue
+        bound, w, unit = work[k]
+        per_step_ms = ms / n_timed
+        if bound == "hbm":
+            ach, peak, u = w / (per_step_ms * 1e-3) / 1e9, pk["hbm_gbs"], "GB/s"
+        else:
+            ach, peak, u = w / (per_step_ms * 1e-3) / 1e12, (dmma if bound == "tensor" else dfma), "TFLOP/s"
+        fams[k] = {"bound": bound, "achieved": round(ach, 3), "peak": round(peak, 3), "unit": u, "frac": round(ach / peak, 4),
+                   "ms_per_step": round(per_step_ms, 3), "launches_per_step": n // n_timed}
+    return fams
+
+
+def elements_per_position(prob):
+    Nc = [c.n_states for c in prob.centres]
+    return (Nc[0] ** 2 + Nc[1] ** 2 + 3 * Nc[0] * Nc[1]) if len(Nc) == 2 else Nc[0] ** 2
+
+
 def run_ours(args):
     import torch
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -151,76 +279,36 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     import paper_2403_04252_b200 as wp
-    from paper_2403_04252_b200.shard import gather_amplitudes
 
-    prob, run, mine = workload(args.config, world, rank)
-    b_all, v_all, vg_all = run["b"], run["v"], run["vgroup"]
-    b, v = b_all[mine], v_all[mine]
-    n_steps, z0, z1 = run["n_steps"], run["z_min"], run["z_max"]
-    if args.window_steps:                                                  # not the headline: a window of the configured step size around z = 0
-        hz = (z1 - z0) / n_steps
-        n_steps = int(args.window_steps)
-        z0, z1 = -0.5 * n_steps * hz, 0.5 * n_steps * hz
-    n_vg = int(vg_all.max()) + 1
-    basis = wp.setup_basis(prob)
-    if args.direct_tables:
-        basis.enable_direct_tables(True)
-    N = basis.n_tot
+    window = args.window_steps or STEP_WINDOW[args.config]
+    job = Job(wp, args.config, world, rank, window=window, direct_tables=args.direct_tables)
+    prob, b, v, b_all = job.prob, job.b, job.v, job.b_all
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ms_step, fam_ms, launches, units_step, (m0, m1) = measure(job, torch, dist, world, args.warmup, args.steps, flush, sampler)
+    units = len(b_all) * job.n_steps                                       # trajectory * RK4-steps per step, all ranks
+    value = units / (ms_step * 1e-3)
 
-    def step():
-        C = wp.propagate(basis, b, v, z0, z1, n_steps)
-        Call = gather_amplitudes(C, len(b_all), rank, world)
-        return wp.probabilities(basis, Call, b=b_all, vgroup=vg_all, n_vgroups=n_vg)
-
-    def barrier():
+    # ---- e2e: the same step from host buffers through the public API, H2D and D2H inside the timed region
+    h2d = sum(np.asarray(getattr(c, k)).nbytes for c in prob.centres for k in ("u", "g", "eps", "l", "kind", "nq")) + np.asarray(prob.w).nbytes + b.nbytes + v.nbytes
+    keys = ("P_state", "P_nl", "P_class", "sigma_nl", "sigma_class")
+    C_host = None
+    if job.window:                                                         # a window continues from amplitudes: they come from the host too
+        _, _, Cw = job.span()
+        C_host = (Cw if Cw is not None else torch.zeros((len(b), job.basis.n_tot), dtype=torch.complex128, device="cuda")).cpu().pin_memory()
+        h2d += C_host.numel() * 16
+    d2h, e2e_ms = 0, []
+    for it in range(1 + min(args.steps, 3)):
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
-            torch.cuda.synchronize()
-
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    m0 = sampler.mark() if sampler else 0
-    evs, launches, fam_ms, units_step = [], 0, {}, {}
-    for _ in range(args.steps):
-        flush.fill_(1)                                                     # L2 flush between timed iterations
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        out = step()
-        e1.record()
-        evs.append((e0, e1))
-        tm = wp.last_timing(basis)                                         # synchronises; per-family event times of this step
-        launches += sum(n for _, n in tm.values()) + 4                     # + init amplitudes, probabilities, 2 x cross sections
-        units_step = wp.last_units(basis)                                  # positions per family of this step (same every step)
-        for k, (ms, n) in tm.items():
-            a = fam_ms.setdefault(k, [0.0, 0])
-            a[0] += ms; a[1] += n
-    barrier()
-    m1 = sampler.mark() if sampler else 0
-    ms_step = sum(e0.elapsed_time(e1) for e0, e1 in evs) / args.steps
-    t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item())
-    units = len(b_all) * n_steps                                           # trajectory * RK4-steps per step, all ranks
-    value = units / (ms_step * 1e-3)
-
-    # ---- e2e: the same job from host buffers through the public API, H2D and D2H inside the timed region
-    h2d = sum(np.asarray(getattr(c, k)).nbytes for c in prob.centres for k in ("u", "g", "eps", "l", "kind", "nq")) + np.asarray(prob.w).nbytes + b.nbytes + v.nbytes
-    keys = ("P_state", "P_nl", "P_class", "sigma_nl", "sigma_class")
-    d2h, e2e_ms = 0, []
-    for it in range(1 + min(args.steps, 3)):
-        barrier()
         flush.fill_(1)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         bs2 = wp.setup_basis(prob)                                         # H2D of every table
-        C = wp.propagate(bs2, b, v, z0, z1, n_steps)
-        Call = gather_amplitudes(C, len(b_all), rank, world)
-        o = wp.probabilities(bs2, Call, b=b_all, vgroup=vg_all, n_vgroups=n_vg)
+        if args.direct_tables:
+            bs2.enable_direct_tables(True)
+        o = job.step(basis=bs2, C0=C_host.cuda(non_blocking=True) if C_host is not None else None)
         host = {k: o[k].cpu() for k in keys}                               # D2H (synchronises)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) * 1e3
@@ -238,63 +326,87 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     clocks = sampler.summary(m0, m1)
-    sampler.stop()
 
     # ---- roofline of the dominant kernel family (device time measured with CUDA events inside the library, on the
     # stream each kernel was launched on, during the timed steps above)
     pk = measured_peaks()
     dmma, dfma = wp.fp64_peak(1), wp.fp64_peak(0)
-    work = family_work(prob, b, n_steps, units_step)
-    if args.direct_tables:                                                 # NEXT-1: 16 B read + 8 B written per entry and position
-        work["direct_gemm"] = ("hbm", work["direct_gemm"][1] / (2.0 * prob.Nr) * 24.0, "byte")
-    fams = {}
-    for k, (ms, n) in fam_ms.items():
-        if n == 0 or k not in work:
-            continue
-        bound, w, unit = work[k]
-        per_step_ms = ms / args.steps
-        if bound == "hbm":
-            ach, peak, u = w / (per_step_ms * 1e-3) / 1e9, pk["hbm_gbs"], "GB/s"
-        else:
-            ach, peak, u = w / (per_step_ms * 1e-3) / 1e12, (dmma if bound == "tensor" else dfma), "TFLOP/s"
-        fams[k] = {"bound": bound, "achieved": round(ach, 3), "peak": round(peak, 3), "unit": u, "frac": round(ach / peak, 4),
-                   "ms_per_step": round(per_step_ms, 3), "launches_per_step": n // args.steps}
+    fams = families(job, fam_ms, args.steps, units_step, pk, dmma, dfma, args.direct_tables)
     dom = max(fams, key=lambda k: fams[k]["ms_per_step"])
     roof = dict(fams[dom])
     roof.update({"kernel": dom, "traffic": None,
+                 "timing": "CUDA events on the stream the kernels run on; families launched once per chunk of positions (node tables, contraction) "
+                           "are sampled on every 8th launch group and scaled by the number of groups",
                  "peak_source": ("in-run FP64 micro-benchmark through wpccc_fp64_peak (DMMA m8n8k4 %.2f, DFMA %.2f TFLOP/s); "
                                  "MEASURED_PEAKS.json (%s) has no fp64 figure: bf16 burst %.1f x nominal fp64-tensor/bf16 ratio %.3f = %.2f TFLOP/s; hbm %.1f GB/s"
                                  % (dmma, dfma, pk["src"], pk["bf16"], NOMINAL_FP64_TENSOR_OVER_BF16, pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16, pk["hbm_gbs"]))})
-    tr = os.path.join(ROOT, "profiles", "traffic.json")                    # dram bytes per launch from the committed ncu --set full capture
+    tr = os.path.join(ROOT, "profiles", "traffic.json")                    # dram bytes per launch from the committed ncu --set full captures
     if os.path.exists(tr):
-        roof["traffic"] = json.load(open(tr)).get(dom)
+        tj = json.load(open(tr))
+        roof["traffic"] = tj.get("configs[%d]" % args.config, {}).get(dom)
+        roof["traffic_source"] = "not measured in this run: ncu --set full capture recorded in profiles/traffic.json (%s)" % tj.get("_source", "")
 
-    Nc = [c.n_states for c in prob.centres]
-    elems_per_pos = (Nc[0] ** 2 + Nc[1] ** 2 + 3 * Nc[0] * Nc[1]) if len(Nc) == 2 else Nc[0] ** 2
+    per_config = {str(args.config): {"value": round(value, 3), "ms_per_step": round(ms_step, 3), "steps": args.steps, "warmup": args.warmup,
+                                     "workload": job.describe(), "dominant": dom, "frac": fams[dom]["frac"], "kernel_families": fams}}
     line = {
         "metric": METRIC, "value": round(value, 3), "unit": "trajectory*steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms_step, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": "BASELINE.json configs[%d]: %s, N_tot=%d states, %d trajectories x %d RK4 steps per step%s" % (
-                       args.config, "two-centre p+H with electron transfer, quadrature %dx%dx%d" % (prob.quad["n_rho"], prob.quad["n_phi"], prob.quad["n_z"]) if prob.quad else "one-centre",
-                       N, len(b_all), n_steps, (" (%d per rank)" % len(b) if world > 1 else "") + (" [window of the configured step size around z = 0, not the full z-range]" if args.window_steps else "")),
+        "config": {"workload": job.describe() + ((" (%d trajectories per rank)" % len(b)) if world > 1 else ""),
                    "l2": "512 MiB buffer written between timed iterations (L2 flush); window buffers of one step are several GB >> L2",
                    "parallelism": "dp%d over impact parameters" % world,
                    "direct": "prefix/suffix tables (NEXT-1)" if args.direct_tables else "DMMA GEMM",
-                   "mirror_pairs": "body-frame integrals of (b,-z),(b,+z) evaluated together: %d of %d positions per step run the node tables and the contraction; roofline work counts those only" % (
-                       units_step.get("transfer_contraction", 0), units_step.get("rotation", 0)) if prob.quad else "n/a"},
-        "matrix_elements_per_s": round(elems_per_pos * len(b_all) * (2 * n_steps + 1) / (ms_step * 1e-3), 1),
+                   "overlap_solve": "solve_route 0: blocked Cholesky factor of I - K K^H + triangular solves per RK4 stage" if prob.quad else "n/a (S = I)",
+                   "not_positive_definite": ("%d of %d trajectories met a position where the overlap matrix of the configured basis and quadrature is not positive "
+                                             "definite (DESIGN.md A23); they are flagged (WPCCC_ESINGULAR, amplitudes NaN), every kernel still ran for them" % (job.n_singular, len(b))) if prob.quad else "n/a",
+                   "mirror_pairs": ("body-frame integrals of (b,-z),(b,+z) evaluated together where the z-range of a step is symmetric about 0: %d of %d positions per step ran the node tables and the contraction; roofline work counts those only" % (
+                       units_step.get("transfer_contraction", 0), units_step.get("rotation", 0))) if prob.quad else "n/a"},
+        "matrix_elements_per_s": round(elements_per_position(prob) * len(b_all) * (2 * job.n_steps + 1) / (ms_step * 1e-3), 1),
         "clocks": clocks,
         "e2e": {"value": round(e2e_val, 3), "unit": "trajectory*steps/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": int(launches),
         "roofline": roof,
         "kernel_families": fams,
     }
+    job.close()
+    del job
+    wp.release_workspace()
+    torch.cuda.empty_cache()
+
+    # ---- the other configurations, a few steps each in the same run (BASELINE.json north_star: steps/s "reported for each")
+    if world == 1 and args.per_config:
+        for cfg in (0, 1, 2, 4, 3):
+            if str(cfg) in per_config:
+                continue
+            n_warm, n_timed = (3, 5) if cfg in (0, 1) else (1, 2)
+            j2 = Job(wp, cfg, 1, 0, window=STEP_WINDOW[cfg])
+            if STEP_WINDOW[cfg] is None and cfg in (2, 4):                  # whole jobs of several seconds: warm up on short windows first
+                jw = Job(wp, cfg, 1, 0, window=16)
+                jw.basis.close(); jw.basis = j2.basis
+                for _ in range(3):
+                    jw.step()
+                jw.basis = None
+            ms2, fam2, ln2, un2, _ = measure(j2, torch, dist, 1, n_warm, n_timed, flush)
+            f2 = families(j2, fam2, n_timed, un2, pk, dmma, dfma)
+            d2 = max(f2, key=lambda k: f2[k]["ms_per_step"])
+            per_config[str(cfg)] = {"value": round(len(j2.b_all) * j2.n_steps / (ms2 * 1e-3), 3), "ms_per_step": round(ms2, 3), "steps": n_timed, "warmup": n_warm,
+                                    "workload": j2.describe(), "dominant": d2, "frac": f2[d2]["frac"], "kernel_families": f2,
+                                    "matrix_elements_per_s": round(elements_per_position(j2.prob) * len(j2.b_all) * (2 * j2.n_steps + 1) / (ms2 * 1e-3), 1)}
+            line["gpu_launches"] += int(ln2)
+            j2.close()
+            del j2
+            wp.release_workspace()
+            torch.cuda.empty_cache()
+    line["per_config"] = {k: per_config[k] for k in sorted(per_config)}
+    sampler.stop()
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(args.config, budget_steps=args.cpu_steps)
+        line["cpu_baseline"] = cpu_baseline(args.config, budget_steps=args.cpu_steps or CPU_STEPS[args.config])
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+CPU_STEPS = {0: 400, 1: 16, 2: 40, 3: 1, 4: 40}     # RK4 steps of one trajectory the oracle does in roughly 10-30 s
 
 
 def cpu_sample(cfg_idx, n_rk4_steps):
@@ -328,7 +440,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n = 2                                               # RK4 steps of one trajectory per bench "step" (bounded sample)
+    n = {0: 50, 1: 2, 2: 5, 3: 1, 4: 5}[args.config]    # RK4 steps of one trajectory per bench "step" (bounded sample)
     for _ in range(min(args.warmup, 1)):
         cpu_sample(args.config, 1)
     tot, sample, thr = 0.0, "", 1
@@ -352,11 +464,13 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--cpu-steps", type=int, default=16, help="RK4 steps of the cpu_baseline sample")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[i] of the headline line (default: the largest single-GPU configuration)")
+    ap.add_argument("--per-config", dest="per_config", action="store_true", default=True, help="also measure the other four configurations (a few steps each) into per_config")
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false")
+    ap.add_argument("--cpu-steps", type=int, default=0, help="RK4 steps of the cpu_baseline sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--direct-tables", action="store_true", help="SURVEY.md 8(f) NEXT-1: radial sums from prefix/suffix tables instead of the DMMA GEMM (family direct_gemm then counts HBM bytes)")
-    ap.add_argument("--window-steps", type=int, default=0, help="propagate only this many RK4 steps (configured step size) around z = 0; for configs whose full run takes many minutes")
+    ap.add_argument("--window-steps", type=int, default=0, help="RK4 steps per bench step (windows walking through z from z_min) instead of the per-config default")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

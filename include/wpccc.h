@@ -8,21 +8,27 @@
  *
  * Conventions common to every entry point
  *   - Plain pointers and sizes only.  Each pointer argument is marked [host] or [device].
- *   - The library NEVER allocates device memory for data: the caller owns the basis arena, the
- *     workspace and every output buffer.  A pointer is borrowed for the duration of the call,
- *     except the arena, which the basis handle keeps using until wpccc_free_basis().
+ *   - The library NEVER allocates device memory (no cudaMalloc / cudaMallocAsync anywhere): the
+ *     caller owns the basis arena, the workspace and every output buffer.  A pointer is borrowed
+ *     for the duration of the call, except the arena, which the basis handle keeps using until
+ *     wpccc_free_basis() (it also holds 1 MiB of index scratch for wpccc_probabilities).
  *   - All device work is enqueued on the caller's CUDA stream (`stream` is a cudaStream_t passed
- *     as void*; NULL = legacy default stream).  wpccc_propagate additionally forks onto one
- *     internal stream and joins back before it returns control to `stream` order.
+ *     as void*; NULL = legacy default stream).  wpccc_propagate additionally forks onto two
+ *     internal streams and joins them back, also on every error path, before it returns.
  *     Calls are asynchronous with respect to the host unless stated otherwise.
+ *   - A basis handle is NOT re-entrant: it carries per-call state (timing events, the status of
+ *     the last propagation, its two internal streams, the options).  One call at a time per
+ *     handle, from one host thread; use one handle per concurrent caller.  The entry points take
+ *     `const wpccc_basis *` because they never change the staged basis itself.
  *   - Complex numbers are interleaved double[2] = (re, im).  All arithmetic is IEEE fp64.
  *   - Return value: 0 on success, a negative WPCCC_E* code otherwise; wpccc_last_error() gives a
  *     thread-local message.  There is no CPU fallback: without a CUDA device every compute call
  *     returns WPCCC_ECUDA.
  *   - State ordering (binding): centre T then centre P; inside a centre the radial functions in
  *     caller order; each radial function expands to m = -l .. +l ascending.
- *   - Geometry (A.1): target nucleus at the origin, projectile at (b, 0, z), velocity v along +z,
- *     b >= 0.  Atomic units.
+ *   - Geometry (A.1): target nucleus at the origin, projectile at (b, 0, z), velocity v along +z.
+ *     wpccc_matrix_elements accepts b >= 0 (with R > 0); wpccc_propagate and the cross sections of
+ *     wpccc_probabilities need b > 0.  Atomic units.
  */
 #ifndef WPCCC_H
 #define WPCCC_H
@@ -37,7 +43,9 @@ extern "C" {
 #define WPCCC_EINVAL     (-1)  /* bad argument (message says which)                               */
 #define WPCCC_ENOMEM     (-2)  /* arena or workspace too small                                     */
 #define WPCCC_ECUDA      (-3)  /* CUDA runtime error / no device                                   */
-#define WPCCC_ESINGULAR  (-4)  /* zero pivot in the overlap solve, or |S_PT| >= 1 (see propagate)  */
+#define WPCCC_ESINGULAR  (-4)  /* overlap system of some trajectory not factorisable (see propagate) */
+
+#define WPCCC_INIT_FROM_DC (-1) /* init_state of wpccc_propagate: start from the amplitudes already in dC */
 
 typedef struct wpccc_basis wpccc_basis; /* opaque */
 
@@ -54,18 +62,25 @@ typedef struct {
     const double *g;      /* [n_rad][Nr+1] residual (H_c - eps_a) u_a (A5); NULL = all zero        */
 } wpccc_centre;
 
-/* Fixed Gauss-Legendre product rule for the two-centre integrals in body-frame cylindrical
- * coordinates (rho', phi', z') (BASELINE.json configs[1], [3]; A10):
+/* Fixed product rule for the two-centre integrals of eq. (9) in the body frame.
+ * kind 0 (BASELINE.json configs[1], [3]; A10): Gauss-Legendre in cylindrical coordinates (rho', phi', z'):
  *   rho' one panel on [0, rho_max] (n_rho nodes); phi' one panel on [0, 2 pi] (n_phi nodes);
  *   z' three panels [-z_pad, 0], [0, R], [R, R + z_pad] with n_z/4, n_z/2, n_z/4 nodes.
- * n_z must be a multiple of 16, n_rho >= 1, n_phi >= 1.
- * phi_rule 0: the discrete n_phi-node sum.  phi_rule 1: the continuum azimuthal integral
- * (-+i)^Delta J_Delta(x) of eq. (9), evaluated by a 512-node periodic trapezoid rule
- * (exact to rounding for x + |Delta| < 400). */
+ *   n_z must be a multiple of 16, n_rho >= 1, n_phi >= 1.
+ *   phi_rule 0: the discrete n_phi-node sum.  phi_rule 1: the continuum azimuthal integral
+ *   (-+i)^Delta J_Delta(x) of eq. (9), evaluated by a 512-node periodic trapezoid rule
+ *   (exact to rounding for x + |Delta| < 400).
+ * kind 1 (the paper's own rule): prolate spheroidal coordinates
+ *   r_T = R (eta + tau)/2, r_P = R (eta - tau)/2: n_rho-point Gauss-Laguerre rule in eta, with
+ *   x = eta_scale (R/2)(eta - 1), n_z-point Gauss-Legendre rule in tau on [-1, 1] (n_z a multiple of 16), analytic
+ *   azimuthal integral (-+i)^Delta J_Delta (Bessel functions by backward recurrence); n_phi, phi_rule, rho_max, z_pad
+ *   are ignored.  No mirror pairing. */
 typedef struct {
     int    n_rho, n_phi, n_z;
     double rho_max, z_pad;
     int    phi_rule;
+    int    kind;        /* 0 cylindrical Gauss-Legendre, 1 spheroidal Gauss-Laguerre x Gauss-Legendre */
+    double eta_scale;   /* kind 1: decay constant of the Laguerre weight e^{-eta_scale (r_T + r_P - R)/2}, > 0 */
 } wpccc_quad;
 
 /* ---- a0: staging ("stored in the GPU global memory") ------------ */
@@ -104,6 +119,28 @@ int wpccc_radial_entry(const wpccc_basis *basis, int c, int e, int *a_prime, int
  * windows); what = 2: the minimum wpccc_propagate accepts. */
 size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, int what);
 
+/* ---- options -------------------------------------------------------------------------------------
+ * Selects between CUDA routes that compute the same thing (never a CPU path); takes effect from the
+ * next call on this handle.  Keys:
+ *   "mirror_pairs"       1 (default) / 0: on a z-grid symmetric about 0, evaluate the body-frame integrals of
+ *                        eq. (9) at (b, -z) and (b, +z) together (see wpccc_last_units).
+ *   "solve_route"        how S(R) x = y is solved in every RK4 stage (role of ZGESV), with
+ *                        S = [[I, K^H], [K, I]] reduced to its Schur complement A = I - K K^H (Hermitian,
+ *                        positive definite whenever S is):
+ *                        0 (default): blocked Cholesky factor A = L L^H, two triangular solves per stage
+ *                           (a linear solve, as the paper insists, not an inverse); a position where A is not
+ *                           positive definite is reported (WPCCC_ESINGULAR, wpccc_last_status);
+ *                        1: explicit inverse A^{-1} by Gauss-Jordan elimination with partial pivoting
+ *                           (the pivots plain partial pivoting of S would take, A22), applied as a
+ *                           matrix-vector product per stage; works for any non-singular S, rounding error
+ *                           cond(A) 2^-53.
+ *   "inverse_kernel"     solve_route 1 only: 0 automatic, 1 shared-memory kernel, 2 global-memory blocked kernel.
+ *   "inverse_chunk_cols" solve_route 1, register kernel: stage K in chunks of this many columns (0 automatic).
+ *   "sweep_cluster"      CTAs per thread-block cluster of the RK4 sweep (0 automatic; 1, 2, 4, 8).
+ *   "timing"             1 (default) / 0: record the CUDA events behind wpccc_last_timing.
+ * Returns 0 or WPCCC_EINVAL (unknown key, value out of range). */
+int wpccc_set_option(wpccc_basis *basis, const char *key, long long value);
+
 /* ---- a2 alternative: tabulated direct couplings (the paper's own route, in exact form)
  * V_lambda(r, R) = min^lambda / max^(lambda+1) separates at r = R, so the grid sum of eq. (7) is
  *   F^c_lambda(a', a; R) = R^-(lambda+1) P_e[g] + R^lambda Q_e[g],   g = #{k : r_k < R},
@@ -140,19 +177,38 @@ int wpccc_matrix_elements(const wpccc_basis *basis, int n_pos, const double *b /
  * straight-line trajectories (b[t], v[t]) [host arrays] concurrently, with classical RK4
  * (Algorithm 1) on the uniform grid z_i = z_min + i (z_max - z_min)/n_steps (A13).
  * The 2 n_steps + 1 evaluations of (S, H) per path are computed in windows for all
- * trajectories at once; the overlap system is factorised by Gaussian elimination with partial
- * pivoting (the role of ZGESV) and solved once per RK4 stage (A14).
- * Initial condition c = delta_{j, init_state}.
+ * trajectories at once; the overlap system is factorised once per position and solved once per
+ * RK4 stage (A14) by the route "solve_route" of wpccc_set_option selects (the role of ZGESV).
+ * Initial condition c = delta_{j, init_state}; init_state = WPCCC_INIT_FROM_DC continues
+ * from the amplitudes in dC (and the running maxima in d_norm_drift), e.g. to walk through a long
+ * z-range in several calls.
  * Outputs [device]: dC [n_traj][N_tot] complex amplitudes at z_max;
  *   d_norm_drift [n_traj] max over steps of |c^H S c - 1| (A17), or NULL.
- * Errors: WPCCC_ENOMEM if ws_bytes < wpccc_workspace_bytes(.., 2).  A zero pivot, or an overlap
- * element with |S_PT| >= 1 (which would invalidate the pivot order the factorisation relies on,
- * DESIGN.md "a7"), is detected on the device; the call then synchronises and returns
- * WPCCC_ESINGULAR.  The call synchronises `stream` before returning (it reads that status). */
+ * Errors: WPCCC_ENOMEM if ws_bytes < wpccc_workspace_bytes(.., 2).
+ * WPCCC_ESINGULAR: at some position of some trajectory the overlap system could not be factorised:
+ *   I - K K^H not positive definite (solve_route 0: with an over-complete two-centre basis the
+ *   configured quadrature can leave S(R) indefinite at small R, A23), or a zero pivot /
+ *   |S_PT| >= 1 (solve_route 1).  The amplitudes and the drift of those trajectories are NaN, every
+ *   other trajectory is complete and valid; wpccc_last_status tells which and where.
+ * The call synchronises `stream` before returning (it reads that status). */
 int wpccc_propagate(const wpccc_basis *basis, int n_traj, const double *b /*[host]*/,
                     const double *v /*[host]*/, double z_min, double z_max, int n_steps, int init_state,
                     double *dC /*[device]*/, double *d_norm_drift /*[device] or NULL*/,
                     void *ws /*[device]*/, size_t ws_bytes, void *stream);
+
+/* The same on an explicit step grid zgrid[0] < ... < zgrid[n_points - 1] [host], e.g. the paper's
+ * z-grid zgrid[+-i] = +-z_min (z_max / z_min)^(i / n_z), zgrid[0] = 0: step i goes from z = zgrid[i] to
+ * z_new = zgrid[i + 1] with h = z_new - z and z_mid = z + h / 2 (Algorithm 1 lines 13-15), n_points - 1 steps,
+ * 2 n_points - 1 evaluations of (S, H) (4 n_z + 1 for the paper's 2 n_z + 1 points).  Everything else as above. */
+int wpccc_propagate_grid(const wpccc_basis *basis, int n_traj, const double *b /*[host]*/, const double *v /*[host]*/,
+                         int n_points, const double *zgrid /*[host]*/, int init_state,
+                         double *dC /*[device]*/, double *d_norm_drift /*[device] or NULL*/,
+                         void *ws /*[device]*/, size_t ws_bytes, void *stream);
+
+/* Outcome of the last wpccc_propagate / wpccc_propagate_grid per trajectory: traj_status[t] [host, n_traj] = 0 (complete),
+ * or (code << 28) | (1 + half-step index of the first position whose overlap system could not be factorised), code
+ * 1 zero pivot, 2 |S_PT| >= 1, 3 not positive definite.  Half-step index i: z = z_min + i h / 2 on the uniform grid. */
+int wpccc_last_status(const wpccc_basis *basis, int n_traj, int *traj_status /*[host]*/);
 
 /* ---- a9: observables ------------------------------------------------------------------
  * From amplitudes dC [device, n_traj][N_tot] complex:
@@ -163,8 +219,9 @@ int wpccc_propagate(const wpccc_basis *basis, int n_traj, const double *b /*[hos
  *   sigma_nl [n_vgroups][n_rad_tot], sigma_class [n_vgroups][5]
  *                                 2 pi Int b P(b) db by the trapezoid rule in ln b over the
  *                                 trajectories of each velocity group, sorted by b (units a0^2).
- * b [host][n_traj], vgroup [host][n_traj] in 0..n_vgroups-1.  All outputs [device]; any may be NULL
- * (sigma_* need b and vgroup). */
+ * b [host][n_traj] (> 0: the rule lives on ln b), vgroup [host][n_traj] in 0..n_vgroups-1.  All outputs
+ * [device]; any may be NULL (sigma_* need b and vgroup, P_nl / P_class respectively, and at most ~80 000
+ * trajectories per call: their index scratch lives in the basis arena).  With sigma_* the call synchronises. */
 int wpccc_probabilities(const wpccc_basis *basis, int n_traj, const double *dC /*[device]*/,
                         const double *b /*[host]*/, const int *vgroup /*[host]*/, int n_vgroups,
                         int init_state, double *P_state, double *P_nl, double *P_class,
@@ -185,7 +242,7 @@ int wpccc_last_timing(const wpccc_basis *basis, double *ms /*[host][8]*/, long l
  * eq. (9) once per mirror pair (b, -z), (b, +z) -- they differ only by the complex conjugation of the
  * axial phase -- as far as the workspace beyond wpccc_workspace_bytes(.., 2) can hold the second
  * member's integrals until the sweep reaches it; units[3] is then smaller
- * than the number of positions.  The environment variable WPCCC_NO_MIRROR disables this.
+ * than the number of positions.  wpccc_set_option(basis, "mirror_pairs", 0) disables this.
  * Returns the number of families (8) or WPCCC_EINVAL. */
 int wpccc_last_units(const wpccc_basis *basis, long long *units /*[host][8]*/);
 

@@ -42,7 +42,7 @@ class _Centre(C.Structure):
 
 class _Quad(C.Structure):
     _fields_ = [("n_rho", C.c_int), ("n_phi", C.c_int), ("n_z", C.c_int), ("rho_max", C.c_double), ("z_pad", C.c_double),
-                ("phi_rule", C.c_int)]
+                ("phi_rule", C.c_int), ("kind", C.c_int), ("eta_scale", C.c_double)]
 
 
 _dp, _ip, _vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p
@@ -67,6 +67,12 @@ _lib.wpccc_matrix_elements.restype = C.c_int
 _lib.wpccc_matrix_elements.argtypes = [_vp, C.c_int, _dp, _dp, _dp, C.c_int, _vp, _vp, _vp, _vp, C.c_size_t, _vp]
 _lib.wpccc_propagate.restype = C.c_int
 _lib.wpccc_propagate.argtypes = [_vp, C.c_int, _dp, _dp, C.c_double, C.c_double, C.c_int, C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]
+_lib.wpccc_propagate_grid.restype = C.c_int
+_lib.wpccc_propagate_grid.argtypes = [_vp, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]
+_lib.wpccc_last_status.restype = C.c_int
+_lib.wpccc_last_status.argtypes = [_vp, C.c_int, _ip]
+_lib.wpccc_set_option.restype = C.c_int
+_lib.wpccc_set_option.argtypes = [_vp, C.c_char_p, C.c_longlong]
 _lib.wpccc_probabilities.restype = C.c_int
 _lib.wpccc_probabilities.argtypes = [_vp, C.c_int, _vp, _dp, _ip, C.c_int, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.wpccc_last_timing.restype = C.c_int
@@ -84,7 +90,7 @@ _lib.wpccc_version.restype = C.c_char_p
 
 EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
-           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
+           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
            "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
 
 
@@ -135,7 +141,8 @@ def _marshal(prob):
     quad = None
     if prob.quad is not None:
         q = prob.quad
-        quad = _Quad(int(q["n_rho"]), int(q["n_phi"]), int(q["n_z"]), float(q["rho_max"]), float(q["z_pad"]), int(q.get("phi_rule", 0)))
+        quad = _Quad(int(q["n_rho"]), int(q["n_phi"]), int(q["n_z"]), float(q["rho_max"]), float(q["z_pad"]), int(q.get("phi_rule", 0)),
+                     int(q.get("kind", 0)), float(q.get("eta_scale", 1.0)))
     return cs, quad, keep
 
 
@@ -161,7 +168,6 @@ class Basis:
         self.n_states = [_lib.wpccc_n_states_centre(h, c) for c in range(self.n_centres)]
         self.n_rad = [_lib.wpccc_n_rad_centre(h, c) for c in range(self.n_centres)]
         self.n_entries = [_lib.wpccc_n_radial_entries(h, c) for c in range(self.n_centres)]
-        self._ws = None
 
     def close(self):
         if getattr(self, "_h", None):
@@ -173,6 +179,10 @@ class Basis:
             self.close()
         except Exception:
             pass
+
+    def set_option(self, key: str, value: int):
+        """wpccc_set_option: choose between CUDA routes ("mirror_pairs", "solve_route", "inverse_kernel", ...; see wpccc.h)."""
+        _check(_lib.wpccc_set_option(self._h, key.encode(), int(value)))
 
     def enable_direct_tables(self, on: bool = True):
         """wpccc_enable_direct_tables: evaluate the radial sums of eq. (7) from prefix/suffix tables
@@ -196,11 +206,23 @@ class Basis:
         return out
 
     def workspace(self, nbytes):
+        """The call workspace: ONE torch tensor per process, shared by every handle and grown on demand (a handle is
+        single-caller and every compute call has finished with the workspace when it returns)."""
+        global _WS
         torch = _torch()
-        if self._ws is None or self._ws.numel() < nbytes + 256:
-            self._ws = None
-            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
-        return C.c_void_p((self._ws.data_ptr() + 255) & ~255), self._ws.numel() - 256
+        if _WS is None or _WS.numel() < nbytes + 256:
+            _WS = None
+            _WS = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        return C.c_void_p((_WS.data_ptr() + 255) & ~255), _WS.numel() - 256
+
+
+_WS = None
+
+
+def release_workspace():
+    """Drops the shared call workspace (tens of GB for the large configurations)."""
+    global _WS
+    _WS = None
 
 
 def setup_basis(prob) -> Basis:
@@ -225,20 +247,53 @@ def matrix_elements(basis: Basis, b, z, v, phases: bool = True, want_S: bool = T
     return (S, H, F) if want_F else (S, H)
 
 
-def propagate(basis: Basis, b, v, z_min: float, z_max: float, n_steps: int, init_state: int = 0, track_norm: bool = False,
-              ws_bytes: int | None = None):
-    """wpccc_propagate: amplitudes c(z_max) [n_traj, N] complex128 on the device (and the norm drift if asked)."""
+def _propagate_common(basis, b, v, n_steps, init_state, track_norm, ws_bytes, C0, drift0, allow_singular, call):
     torch = _torch()
     b, v = _f64(np.atleast_1d(b)), _f64(np.atleast_1d(v))
     n, N = len(b), basis.n_tot
-    Cc = torch.empty((n, N), dtype=torch.complex128, device="cuda")
-    drift = torch.zeros(n, dtype=torch.float64, device="cuda") if track_norm else None
-    need = _lib.wpccc_workspace_bytes(basis._h, n, int(n_steps), 1) if ws_bytes is None else ws_bytes
+    if C0 is not None:                         # continue from given amplitudes (WPCCC_INIT_FROM_DC): updated in place
+        if tuple(C0.shape) != (n, N) or C0.dtype != torch.complex128 or not C0.is_cuda or not C0.is_contiguous():
+            raise ValueError("C0 must be a contiguous complex128 CUDA tensor [n_traj, N]")
+        Cc, init_state = C0, -1
+    else:
+        Cc = torch.empty((n, N), dtype=torch.complex128, device="cuda")
+    drift = None
+    if track_norm:
+        drift = drift0 if drift0 is not None else torch.zeros(n, dtype=torch.float64, device="cuda")
+    need = _lib.wpccc_workspace_bytes(basis._h, max(n, 1), int(n_steps), 1) if ws_bytes is None else ws_bytes
     ws, cap = basis.workspace(need)
-    _check(_lib.wpccc_propagate(basis._h, n, _ptr(b), _ptr(v), float(z_min), float(z_max), int(n_steps), int(init_state),
-                                C.c_void_p(Cc.data_ptr()), C.c_void_p(drift.data_ptr()) if track_norm else None, ws, min(cap, need),
-                                _stream(torch)))
+    rc = call(n, _ptr(b), _ptr(v), int(init_state), C.c_void_p(Cc.data_ptr()), C.c_void_p(drift.data_ptr()) if track_norm else None, ws,
+              min(cap, need), _stream(torch))
+    if not (allow_singular and rc == -4):
+        _check(rc)
     return (Cc, drift) if track_norm else Cc
+
+
+def propagate(basis: Basis, b, v, z_min: float, z_max: float, n_steps: int, init_state: int = 0, track_norm: bool = False,
+              ws_bytes: int | None = None, C0=None, drift0=None, allow_singular: bool = False):
+    """wpccc_propagate: amplitudes c(z_max) [n_traj, N] complex128 on the device (and the norm drift if asked).
+    C0: continue from these amplitudes (updated in place).  allow_singular: do not raise on WPCCC_ESINGULAR (the flagged
+    trajectories are NaN; see last_status)."""
+    return _propagate_common(basis, b, v, n_steps, init_state, track_norm, ws_bytes, C0, drift0, allow_singular,
+                             lambda n, bp, vp, ini, cp, dp, ws, nb, st: _lib.wpccc_propagate(
+                                 basis._h, n, bp, vp, float(z_min), float(z_max), int(n_steps), ini, cp, dp, ws, nb, st))
+
+
+def propagate_grid(basis: Basis, b, v, zgrid, init_state: int = 0, track_norm: bool = False, ws_bytes: int | None = None, C0=None,
+                   drift0=None, allow_singular: bool = False):
+    """wpccc_propagate_grid: the same on an explicit step grid zgrid[0] < ... < zgrid[n] (e.g. the paper's geometric grid)."""
+    zg = _f64(zgrid)
+    return _propagate_common(basis, b, v, len(zg) - 1, init_state, track_norm, ws_bytes, C0, drift0, allow_singular,
+                             lambda n, bp, vp, ini, cp, dp, ws, nb, st: _lib.wpccc_propagate_grid(
+                                 basis._h, n, bp, vp, len(zg), _ptr(zg), ini, cp, dp, ws, nb, st))
+
+
+def last_status(basis: Basis, n_traj: int):
+    """wpccc_last_status: per trajectory (code, half_step_index) of the first position whose overlap system could not be
+    factorised in the last propagate call (code 1 zero pivot, 2 |S_PT| >= 1, 3 not positive definite), or None."""
+    st = (C.c_int * max(n_traj, 1))()
+    _check(_lib.wpccc_last_status(basis._h, n_traj, st))
+    return [None if st[t] == 0 else (st[t] >> 28, (st[t] & 0x0fffffff) - 1) for t in range(n_traj)]
 
 
 def probabilities(basis: Basis, Cc, b=None, vgroup=None, n_vgroups: int = 0, init_state: int = 0):

@@ -14,6 +14,7 @@
 #define WP_MAX_L 6        // largest orbital momentum supported per centre
 #define WP_MAX_LAMBDA 12  // largest multipole (2 * WP_MAX_L)
 #define WP_NFAM 8         // timing families (wpccc_last_timing)
+#define WP_SCRATCH_BYTES (1u << 20)   // index scratch of wpccc_probabilities inside the basis arena
 
 enum { FAM_GEMM = 0, FAM_DASM = 1, FAM_TTAB = 2, FAM_TCON = 3, FAM_ROT = 4, FAM_FACT = 5, FAM_SWEEP = 6, FAM_OTHER = 7 };
 
@@ -97,7 +98,10 @@ struct wpccc_basis {
     int *d_ent_lam = nullptr;   // [E_tot] multipole of every radial entry (both centres)
     double2 *d_dtab = nullptr;  // [Nr+1][E_tot] (P_e[g], Q_e[g]) prefix/suffix sums of eq. (7), caller-owned; nullptr: GEMM
     double *d_gl_rho = nullptr, *d_gl_phi = nullptr, *d_gl_zq = nullptr, *d_gl_zh = nullptr;  // GL x,w on [-1,1]: [2][n]
-    int    *d_status = nullptr; // [4] device status word (0 ok; 1 zero pivot; 2 |S_PT| >= 1), position index
+    int    *d_st_rad_glob = nullptr;  // [n_tot] global radial-function index of every state (centre T functions first)
+    int    *d_rad_info = nullptr;     // [n_rad_tot] 2 * centre + kind (0 bound, 1 wave packet) of every radial function
+    char   *d_scratch = nullptr;      // WP_SCRATCH_BYTES of index scratch for wpccc_probabilities (sorted order, b)
+    int n_rad_tot = 0;
     char *arena = nullptr; size_t arena_bytes = 0;
     const void *tab_zeroed = nullptr; size_t tab_zeroed_bytes = 0;   // node-table buffer whose padding columns are zero (per API call)
     // timing
@@ -114,7 +118,25 @@ struct wpccc_basis {
     long long groups[WP_NFAM] = {0};
     long long units[WP_NFAM] = {0};       // positions processed per family in the last call (wpccc_last_units)
     int cur_fam = 0; bool cur_sampled = false;
+    // options (wpccc_set_option) and the per-trajectory outcome of the last wpccc_propagate (wpccc_last_status)
+    struct Options {
+        int mirror_pairs = 1;        // evaluate the body-frame integrals of (b, -z), (b, +z) together on symmetric z-grids
+        int solve_route = 0;         // 0: Cholesky factor of I - K K^H + triangular solves per RK4 stage; 1: explicit inverse (Gauss-Jordan)
+        int inverse_kernel = 0;      // solve_route 1: 0 automatic, 1 shared-memory kernel, 2 global-memory blocked kernel
+        int inverse_chunk_cols = 0;  // solve_route 1, register kernel: K staged in chunks of this many columns (0: automatic)
+        int sweep_cluster = 0;       // CTAs per cluster of the RK4 sweep (0: automatic)
+        bool timing = true;          // record CUDA events per kernel family (wpccc_last_timing)
+    } opt;
+    std::vector<int> last_status;
 };
+
+// cudaFuncSetAttribute / constant uploads are per device: remember the largest value set on each device ordinal
+struct PerDevice { size_t v[64] = {0}; };
+inline bool wp_raise(PerDevice &a, size_t want) {
+    int d = 0; cudaGetDevice(&d); d &= 63;
+    if (want > a.v[d]) { a.v[d] = want; return true; }
+    return false;
+}
 
 // timing helpers (api.cu)
 void wp_span_begin(wpccc_basis *B, int fam, cudaStream_t s);
@@ -146,7 +168,8 @@ bool wp_transfer_mirror_ok(const wpccc_basis *B);         // the mirror-pair con
 int wp_transfer_default_chunk(const wpccc_basis *B);
 
 // ---- sweep.cu ----
-int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cudaStream_t s);
+// Factorises the overlap system of every position: flags[p] = 0, or 1 zero pivot / 2 |S_PT| >= 1 / 3 not positive definite.
+int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_factor, int *d_flags, void *d_scratch, cudaStream_t s);   // d_factor: wp_factor_elems(N_P) complex per position (sweep.cuh)
 
 // ---- device helpers ----
 __host__ __device__ inline int lm_index(int l, int m) { return l * l + l + m; }

@@ -10,22 +10,13 @@
 #include <algorithm>
 
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace {
 
 constexpr int BM = 128, BN = 128, BK = 32, LDS_ = BK + 4;   // row stride 36 doubles: conflict-free fragment reads
 constexpr int GEMM_THREADS = 256, NSTG = 3;    // three k-chunks in flight, one block-wide barrier per chunk
 
-__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 struct GemmArgs {
     const GemmTile *tiles;
@@ -366,11 +357,8 @@ int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, in
     a.rp = B->d_rp; a.rm = B->d_rm; a.rk = B->d_rk; a.R = d_R; a.F = d_F; a.ldF = ldF; a.n_pos = n_pos; a.Kpad = B->Kpad;
     a.rmap = rmap ? *rmap : ident; a.fmap = fmap ? *fmap : ident;
     const size_t smem = (size_t)NSTG * (BM + BN) * LDS_ * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        WP_CUDA(cudaFuncSetAttribute(k_direct_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static PerDevice attr_g;
+    if (wp_raise(attr_g, smem)) WP_CUDA(cudaFuncSetAttribute(k_direct_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((n_pos + BM - 1) / BM, (unsigned)B->tiles.size());
     wp_span_begin(B, FAM_GEMM, s);
     k_direct_gemm<<<grid, GEMM_THREADS, smem, s>>>(a);
@@ -403,8 +391,8 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
         b.n_rad = C.n_rad; b.n_pairs = C.n_pairs; b.E = C.E; b.N = C.n_states; b.Lc = C.l_max; b.lambda_max = B->lambda_max; b.ldF = ldF;
         b.f_off = a.f_off; b.ld_out = ld_out; b.complex_out = complex_out; b.n_pos = n_pos; b.pos_stride = pos_stride;
         b.charge = a.charge; b.alt_sign = a.alt_sign; b.fmap = a.fmap;
-        static size_t attr2 = 0;
-        if (smem2 > attr2) { WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2)); attr2 = smem2; }
+        static PerDevice attr2;
+        if (wp_raise(attr2, smem2)) WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
         const int per_sm = smem2 <= 100 * 1024 ? 2 : 1;
         const int threads = (C.n_states * C.n_states >= 64 * 1024) ? 1024 : 512;
         wp_span_begin(B, FAM_DASM, s);

@@ -66,6 +66,38 @@ void gauss_legendre(int n, double *x, double *w) {
     if (n & 1) x[n / 2] = 0.0;
 }
 
+// n-point Gauss-Laguerre rule: nodes x_i ascending and SCALED weights w_i e^{x_i} (the plain weights underflow).
+// Nodes = eigenvalues of the Jacobi matrix (diagonal 2k + 1, off-diagonal k), isolated by Sturm-sequence bisection and
+// polished by Newton's method on L_n; w_i e^{x_i} = x_i / ((n + 1) s_{n+1}(x_i))^2 with s_k = L_k(x) e^{-x/2}
+// ((k + 1) s_{k+1} = (2k + 1 - x) s_k - k s_{k-1}).  Long double throughout.
+void gauss_laguerre_scaled(int n, double *x, double *wx) {
+    auto count_below = [&](long double t) {           // eigenvalues of the Jacobi matrix smaller than t
+        int cnt = 0; long double q = 1.0L;
+        for (int k = 0; k < n; ++k) {
+            q = (2 * k + 1) - t - (k > 0 ? (long double)k * k / q : 0.0L);
+            if (q == 0.0L) q = 1e-300L;
+            if (q < 0.0L) ++cnt;
+        }
+        return cnt;
+    };
+    for (int i = 0; i < n; ++i) {
+        long double lo = 0.0L, hi = 4.0L * n + 3.0L;
+        for (int it = 0; it < 200 && hi - lo > 1e-12L * hi; ++it) { const long double mid = 0.5L * (lo + hi); if (count_below(mid) > i) hi = mid; else lo = mid; }
+        long double z = 0.5L * (lo + hi);
+        for (int it = 0; it < 8; ++it) {                // Newton on L_n: x L_n' = n (L_n - L_{n-1})
+            long double s0 = expl(-0.5L * z), s1 = (1.0L - z) * s0;          // s_0, s_1
+            for (int k = 1; k < n; ++k) { const long double s2 = ((2 * k + 1 - z) * s1 - k * s0) / (k + 1); s0 = s1; s1 = s2; }
+            const long double ln = (n == 1) ? s1 : s1, lnm1 = s0;
+            const long double dz = z * ln / (n * (ln - lnm1));
+            z -= dz;
+            if (fabsl(dz) < 1e-18L * fabsl(z)) break;
+        }
+        long double s0 = expl(-0.5L * z), s1 = (1.0L - z) * s0;
+        for (int k = 1; k <= n; ++k) { const long double s2 = ((2 * k + 1 - z) * s1 - k * s0) / (k + 1); s0 = s1; s1 = s2; }
+        x[i] = (double)z; wx[i] = (double)(z / (((long double)(n + 1) * s1) * ((long double)(n + 1) * s1)));
+    }
+}
+
 struct Bump {
     char *base; size_t off = 0;
     explicit Bump(char *b) : base(b) {}
@@ -143,12 +175,12 @@ size_t layout(wpccc_basis &B, char *base) {
     B.d_rk = bump.take<double>(B.Kpad);
     B.d_tiles = bump.take<GemmTile>(B.tiles.size());
     B.d_ent_lam = bump.take<int>(B.E_tot);
-    B.d_status = bump.take<int>(64);
+    B.d_st_rad_glob = bump.take<int>(B.n_tot); B.d_rad_info = bump.take<int>(B.n_rad_tot); B.d_scratch = bump.take<char>(WP_SCRATCH_BYTES);
     if (B.has_quad) {
         B.d_gl_rho = bump.take<double>(2 * (size_t)B.quad.n_rho);
         B.d_gl_phi = bump.take<double>(2 * (size_t)std::max(B.quad.n_phi, 512));
         B.d_gl_zq = bump.take<double>(2 * (size_t)(B.quad.n_z / 4));
-        B.d_gl_zh = bump.take<double>(2 * (size_t)(B.quad.n_z / 2));
+        B.d_gl_zh = bump.take<double>(2 * (size_t)B.quad.n_z);        // kind 0: n_z/2 nodes of the middle panel; kind 1: n_z nodes in tau
     }
     for (int ci = 0; ci < B.n_centres; ++ci) {
         CentreTab &C = B.c[ci];
@@ -176,14 +208,17 @@ int describe(wpccc_basis &B, int n_centres, const wpccc_centre *centres, int Nr,
     B.has_quad = quad != nullptr;
     if (quad) {
         B.quad = *quad;
-        if (quad->n_rho < 1 || quad->n_phi < 1 || quad->n_z < 16 || quad->n_z % 16 || quad->rho_max <= 0 || quad->z_pad <= 0 ||
-            quad->phi_rule < 0 || quad->phi_rule > 1) { wp_set_error("bad wpccc_quad (n_z must be a multiple of 16)"); return WPCCC_EINVAL; }
+        if (quad->kind == 0 && (quad->n_rho < 1 || quad->n_phi < 1 || quad->n_z < 16 || quad->n_z % 16 || quad->rho_max <= 0 || quad->z_pad <= 0 ||
+            quad->phi_rule < 0 || quad->phi_rule > 1)) { wp_set_error("bad wpccc_quad (n_z must be a multiple of 16)"); return WPCCC_EINVAL; }
+        if (quad->kind == 1 && (quad->n_rho < 1 || quad->n_rho > 128 || quad->n_z < 16 || quad->n_z % 16 || !(quad->eta_scale > 0))) {
+            wp_set_error("bad spheroidal wpccc_quad (1 <= n_rho <= 128 Laguerre nodes, n_z a multiple of 16, eta_scale > 0)"); return WPCCC_EINVAL; }
+        if (quad->kind < 0 || quad->kind > 1) { wp_set_error("wpccc_quad.kind must be 0 or 1"); return WPCCC_EINVAL; }
     }
-    B.n_tot = 0; B.E_tot = 0; B.tiles.clear();
+    B.n_tot = 0; B.E_tot = 0; B.n_rad_tot = 0; B.tiles.clear();
     for (int ci = 0; ci < n_centres; ++ci) {
         if (centres[ci].n_rad < 1 || centres[ci].n_rad > 60000 || !centres[ci].l || !centres[ci].eps || !centres[ci].u) { wp_set_error("centre %d: missing arrays", ci); return WPCCC_EINVAL; }
         if (fill_centre_host(B.c[ci], centres[ci], lambda_max)) { wp_set_error("centre %d: l out of range 0..%d", ci, WP_MAX_L); return WPCCC_EINVAL; }
-        B.n_tot += B.c[ci].n_states; B.E_tot += B.c[ci].E;
+        B.n_tot += B.c[ci].n_states; B.E_tot += B.c[ci].E; B.n_rad_tot += B.c[ci].n_rad;
         for (int lam = 0; lam <= lambda_max; ++lam) {
             int cnt = B.c[ci].lam_off[lam + 1] - B.c[ci].lam_off[lam];
             for (int n0 = 0; n0 < cnt; n0 += 128) B.tiles.push_back(GemmTile{ci, lam, n0, std::min(128, cnt - n0)});
@@ -256,7 +291,12 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     std::vector<int> all_lam;
     for (int ci = 0; ci < n_centres; ++ci) all_lam.insert(all_lam.end(), B->c[ci].ent_lam.begin(), B->c[ci].ent_lam.end());
     chk(upload(B->d_ent_lam, all_lam, s));
-    if (!rc && cudaMemsetAsync(B->d_status, 0, 64 * sizeof(int), s) != cudaSuccess) rc = WPCCC_ECUDA;
+    std::vector<int> st_rad_glob, rad_info;
+    for (int ci = 0, off = 0; ci < n_centres; off += B->c[ci].n_rad, ++ci) {
+        for (int j = 0; j < B->c[ci].n_states; ++j) st_rad_glob.push_back(off + B->c[ci].st_rad[j]);
+        for (int a = 0; a < B->c[ci].n_rad; ++a) rad_info.push_back(2 * ci + (B->c[ci].kind[a] != 0));
+    }
+    chk(upload(B->d_st_rad_glob, st_rad_glob, s)); chk(upload(B->d_rad_info, rad_info, s));
     if (!rc && cudaMemcpyAsync(d_w, w, (size_t)(Nr + 1) * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = WPCCC_ECUDA;
     std::vector<std::vector<double>> keep_d; std::vector<std::vector<int>> keep_i;   // host staging must outlive the async copies
     if (!rc && B->has_quad) {
@@ -265,10 +305,17 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
             gauss_legendre(n, keep_d.back().data(), keep_d.back().data() + n);
             chk(upload(dst, keep_d.back(), s));
         };
-        rule(B->quad.n_rho, B->d_gl_rho);
-        if (B->quad.phi_rule == 0) rule(B->quad.n_phi, B->d_gl_phi);
-        rule(B->quad.n_z / 4, B->d_gl_zq);
-        rule(B->quad.n_z / 2, B->d_gl_zh);
+        if (B->quad.kind == 1) {
+            keep_d.emplace_back(2 * (size_t)B->quad.n_rho);
+            gauss_laguerre_scaled(B->quad.n_rho, keep_d.back().data(), keep_d.back().data() + B->quad.n_rho);
+            chk(upload(B->d_gl_rho, keep_d.back(), s));
+            rule(B->quad.n_z, B->d_gl_zh);
+        } else {
+            rule(B->quad.n_rho, B->d_gl_rho);
+            if (B->quad.phi_rule == 0) rule(B->quad.n_phi, B->d_gl_phi);
+            rule(B->quad.n_z / 4, B->d_gl_zq);
+            rule(B->quad.n_z / 2, B->d_gl_zh);
+        }
     }
     for (int ci = 0; ci < n_centres && !rc; ++ci) {
         CentreTab &C = B->c[ci];

@@ -16,41 +16,10 @@
 #include <cstdlib>
 
 #include "sweep.cuh"
+#include "ptx.cuh"
 
 namespace {
 
-struct __align__(16) cplx { double x, y; };
-__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
-__device__ __forceinline__ cplx cmulc(cplx a, cplx b) { return {a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y}; }  // a * conj(b)
-__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return {a.x + b.x, a.y + b.y}; }
-__device__ __forceinline__ cplx csub(cplx a, cplx b) { return {a.x - b.x, a.y - b.y}; }
-__device__ __forceinline__ double warp_sum(double v) {
-    #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-__device__ __forceinline__ double zpos(double z_min, double h, long long i) { return __dadd_rn(z_min, __dmul_rn(0.5 * (double)i, h)); }
-
-// ------------------------------------------------------------------ TMA / mbarrier helpers (both sweeps)
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
-    asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
-        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
 
 constexpr int SW_STAGES = 4;
@@ -106,15 +75,15 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep1(const Sweep1Args a
     #pragma unroll
     for (int q = 0; q < SWEEP_NV; ++q) drift[q] = (a.drift && q < nv) ? a.drift[u.traj[q]] : 0.0;
     consumer_sync();
-    const double h = a.h;
     long long g = 0;
     for (int s = 0; s < a.steps; ++s) {
+        const double h = a.hs[s];
         #pragma unroll 1
         for (int st = 0; st < 4; ++st) {
             const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));       // local half-step index of this stage
             const double alpha = (st == 0) ? 0.0 : (st == 3 ? h : 0.5 * h);
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
-            const double z = zpos(a.z_min, h, a.i0 + li);
+            const double z = a.zh[li];
             for (int j = tid; j < nv * a.n_rad; j += SW_CONSUMERS) {
                 const int q = j / a.n_rad, r = j - q * a.n_rad;
                 double sn, cs; sincos(a.eps[r] * z / vel[q], &sn, &cs);
@@ -273,14 +242,14 @@ __device__ void gauss_jordan_blocked(cplx *G, int n, cplx *Pn /*[n][FJ_NB]*/, cp
 // the output buffer (global).  K is staged through shared memory in column chunks of odd width cw (conflict-free).
 // A^{-1} by in-place Gauss-Jordan elimination with partial (row) pivoting, first maximal |pivot| wins; the row
 // interchanges are undone as column interchanges in reverse order at the end.
-struct FactorArgs { const double *K; double *Ainv; int *status; int NT, NP, use_smem, cw; };
+struct FactorArgs { const double *K; double *Ainv; int *flags; int NT, NP, use_smem, cw; size_t out_stride; };
 
 __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
     extern __shared__ __align__(16) double sm[];
     const int n = a.NP, NT = a.NT, cw = a.cw, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const size_t p = blockIdx.x;
     const cplx *K = reinterpret_cast<const cplx *>(a.K) + p * (size_t)n * NT;
-    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + p * (size_t)n * n;
+    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + p * a.out_stride;
     cplx *smc = reinterpret_cast<cplx *>(sm);
     cplx *A = a.use_smem ? smc : G;
     cplx *Kc = smc + (a.use_smem ? (size_t)n * n : 0);     // [n][cw]
@@ -322,7 +291,7 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
                 __syncthreads();
             }
         }
-        if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
+        if (tid == 0 && s_flag) a.flags[p] = s_flag;
         return;
     }
     {   // shared-memory A: the same blocked elimination, panel buffers in the area that staged K (piv, idx lie behind it)
@@ -345,7 +314,7 @@ __global__ void __launch_bounds__(512) k_factor(const FactorArgs a) {
             }
         }
     }
-    if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)p + 1); }
+    if (tid == 0 && s_flag) a.flags[p] = s_flag;
 }
 
 // ------------------------------------------------------------------ a7, N_P <= 90: A and the elimination in registers
@@ -362,8 +331,6 @@ constexpr int FR_WW = 15, FR_RN = 6, FR_CN = 3, FR_NMAX = FR_WW * FR_RN, FR_WORK
 constexpr int FR_NB = 4;                                              // panel width (the panel warp holds 3 rows of it per lane)
 constexpr int FR_BAR_DONE = 1, FR_BAR_WORK = 2, FR_BAR_PANEL = 3;      // named barriers (0 is unused here)
 
-__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
-__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
 
 // Gauss-Jordan steps j0 .. j0 + w - 1 on the panel Pn [n][FR_NB] (shared), by one warp, in registers.  The warp is
 // alone on the critical path of the whole kernel, so a step is kept short: branch-free pivot search on integer
@@ -471,7 +438,7 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
     // ---- workers
     const int ty = warp, tx = lane;
     const cplx *K = reinterpret_cast<const cplx *>(a.K) + pos * (size_t)n * NT;
-    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + pos * (size_t)n * n;
+    cplx *G = reinterpret_cast<cplx *>(a.Ainv) + pos * a.out_stride;
     int rc[FR_RN], cc[FR_CN];                                         // clamped: out-of-range copies are computed, never stored
     #pragma unroll
     for (int r = 0; r < FR_RN; ++r) rc[r] = min(ty + FR_WW * r, n - 1);
@@ -581,24 +548,28 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
         #pragma unroll
         for (int s = 0; s < FR_CN; ++s)
             if (ty + FR_WW * r < n && tx + 32 * s < n) G[(size_t)pinv[ty + FR_WW * r] * n + piv[tx + 32 * s]] = acc[r][s];
-    if (tid == 0 && s_flag) { atomicMax(a.status, s_flag); atomicCAS(a.status + 1, 0, (int)pos + 1); }
+    if (tid == 0 && s_flag) a.flags[pos] = s_flag;
 }
 
 // ------------------------------------------------------------------ two-centre sweep
-// grid = trajectories; block = 8 consumer warps + 1 producer warp.  Per RK4 stage, with phase-free H0, K and
-// Ainv = (I - K K^H)^{-1} of the stage's position:
-//     y = H0 x;   y_P -= K y_T;   w_P = Ainv y_P;   w_T = y_T - K^H w_P;   k = -(i/v) P w.
-// The matrices do not depend on the amplitudes, so the producer warp streams them (rows of H0, K, Ainv, K again)
-// through a shared-memory ring with TMA bulk copies, running ahead of the consumers across stage boundaries.
-// Chunk schedule of one RK4 step: stages 0..3 each [H rows | K rows | Ainv rows | K rows], then (drift only) K rows.
+// grid = trajectories; block = 8 consumer warps + 1 producer warp.  Per RK4 stage, with the phase-free H0, K of the
+// stage's position and the factorised Schur complement A = I - K K^H (a7):
+//     y = H0 x;   y_P -= K y_T;   w_P = A^{-1} y_P;   w_T = y_T - K^H w_P;   k = -(i/v) P w.
+// A^{-1} y_P: SOLVE = false: explicit inverse, one matrix-vector product;  SOLVE = true: blocked Cholesky factor
+// (CholLayout, sweep.cuh), forward solve over the block rows of Lr, backward solve over the block columns of Lc.
+// The matrices do not depend on the amplitudes, so the producer warp streams them through a shared-memory ring with TMA
+// bulk copies (one per chunk), running ahead of the consumers across stage boundaries.  Chunk order of one RK4 step:
+// stages 0..3 each [H rows | K rows | factor | K rows], then (drift only) K rows; producer and consumers walk the same
+// loops (SweepSched gives the chunk shapes).
 struct SweepSched {
-    int N, NT, NP, rH, rK, rA, nH, nK, nA, per_stage, per_step;
-    __device__ SweepSched(int NT_, int NP_, int chunk_bytes, bool drift) {
-        NT = NT_; NP = NP_; N = NT + NP;
+    int N, NT, NP, rH, rK, rA, nH, nK, nA, cb;
+    __device__ SweepSched(int NT_, int NP_, int chunk_bytes) {
+        NT = NT_; NP = NP_; N = NT + NP; cb = chunk_bytes;
         rH = max(1, chunk_bytes / (16 * N)); rK = max(1, chunk_bytes / (16 * NT)); rA = max(1, chunk_bytes / (16 * NP));
         nH = (N + rH - 1) / rH; nK = (NP + rK - 1) / rK; nA = (NP + rA - 1) / rA;
-        per_stage = nH + 2 * nK + nA; per_step = 4 * per_stage + (drift ? nK : 0);
     }
+    __device__ int rows_fwd(const CholLayout &L, int j) const { return max(1, min(L.nb(j), cb / (16 * L.len(j)))); }   // rows of block row j per chunk
+    __device__ int rows_bwd(const CholLayout &L, int j) const { return max(1, cb / (16 * L.nb(j))); }                  // rows below block j per chunk
 };
 
 // sum over c of row[c] * x[c], c = 0..n-1, by one warp (every lane returns the sum)
@@ -608,57 +579,81 @@ __device__ __forceinline__ cplx warp_dot(const cplx *row, const cplx *x, int n, 
     return {warp_sum(sr), warp_sum(si)};
 }
 
+constexpr int SW_DLD = CHOL_NB + 1;      // row stride of the staged diagonal block
+
+template <bool SOLVE>
 __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a, const int chunk_bytes) {
     extern __shared__ __align__(128) unsigned char smraw[];
     const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int t = blockIdx.x;
     const bool track = a.drift != nullptr;
-    const SweepSched S(NT, NP, chunk_bytes, track);
+    const SweepSched S(NT, NP, chunk_bytes);
+    const CholLayout CL(NP);
     unsigned char *ring = smraw;
     cplx *C = reinterpret_cast<cplx *>(smraw + (size_t)SW_STAGES * chunk_bytes);
     cplx *Acc = C + N, *X = Acc + N, *Kn = X + N, *Y = Kn + N, *ph = Y + N, *Wp = ph + N, *part = Wp + NP;   // part [8][NT]
+    cplx *Tj = part + 8 * NT, *Dblk = Tj + CHOL_NB, *part2 = Dblk + CHOL_NB * SW_DLD;                          // SOLVE: [32], [32][33], [8][32]
     __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
     __shared__ double red[8];
+    __shared__ int redi[8];
     if (tid == 0) {
         for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+        mbar_fence_init();
     }
     __syncthreads();
     const cplx *Hg = reinterpret_cast<const cplx *>(a.H), *Kg = reinterpret_cast<const cplx *>(a.K), *Ag = reinterpret_cast<const cplx *>(a.Ainv);
+    const size_t a_stride = wp_factor_elems(NP);
 
     if (warp == SW_CONSUMERS / 32) {
         // ---------------- producer: one lane streams the chunk sequence of the whole window
         if (lane != 0) return;
-        const long long total = (long long)a.steps * S.per_step;
-        for (long long g = 0; g < total; ++g) {
+        long long g = 0;
+        auto push = [&](const cplx *src, unsigned bytes) {
             const int slot = (int)(g % SW_STAGES); const long long use = g / SW_STAGES;
             if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
-            const int s = (int)(g / S.per_step); int rem = (int)(g - (long long)s * S.per_step);
-            int st = rem / S.per_stage, phase, q;
-            if (st >= 4) { st = 4; phase = 1; q = rem - 4 * S.per_stage; }
-            else {
-                q = rem - st * S.per_stage;
-                if (q < S.nH) phase = 0;
-                else if (q < S.nH + S.nK) { phase = 1; q -= S.nH; }
-                else if (q < S.nH + S.nK + S.nA) { phase = 2; q -= S.nH + S.nK; }
-                else { phase = 3; q -= S.nH + S.nK + S.nA; }
-            }
-            const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
-            const size_t pos = (size_t)t * a.n_idx + li;
-            const cplx *src; unsigned bytes;
-            if (phase == 0) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); src = Hg + pos * (size_t)N * N + (size_t)r0 * N; bytes = (unsigned)rows * N * 16u; }
-            else if (phase == 2) { const int r0 = q * S.rA, rows = min(S.rA, NP - r0); src = Ag + pos * (size_t)NP * NP + (size_t)r0 * NP; bytes = (unsigned)rows * NP * 16u; }
-            else { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); src = Kg + pos * (size_t)NP * NT + (size_t)r0 * NT; bytes = (unsigned)rows * NT * 16u; }
             mbar_expect_tx(&full[slot], bytes);
             tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
-        }
+            ++g;
+        };
+        auto push_K = [&](const cplx *Kp) { for (int q = 0; q < S.nK; ++q) { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); push(Kp + (size_t)r0 * NT, (unsigned)rows * NT * 16u); } };
+        for (int s = 0; s < a.steps; ++s)
+            for (int st = 0; st < (track ? 5 : 4); ++st) {
+                const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
+                const size_t pos = (size_t)t * a.n_idx + li;
+                const cplx *Kp = Kg + pos * (size_t)NP * NT;
+                if (st == 4) { push_K(Kp); break; }
+                const cplx *Hp = Hg + pos * (size_t)N * N, *Ap = Ag + pos * a_stride;
+                for (int q = 0; q < S.nH; ++q) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); push(Hp + (size_t)r0 * N, (unsigned)rows * N * 16u); }
+                push_K(Kp);
+                if (!SOLVE) {
+                    for (int q = 0; q < S.nA; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NP - r0); push(Ap + (size_t)r0 * NP, (unsigned)rows * NP * 16u); }
+                } else {
+                    for (int j = 0; j < CL.nblk; ++j) {                                   // forward: block rows of Lr
+                        const int nbj = CL.nb(j), len = CL.len(j), rf = S.rows_fwd(CL, j);
+                        for (int r0 = 0; r0 < nbj; r0 += rf) push(Ap + CL.off_r(j) + (size_t)r0 * len, (unsigned)min(rf, nbj - r0) * len * 16u);
+                    }
+                    for (int j = CL.nblk - 1; j >= 0; --j) {                              // backward: block columns of Lc, the part below first
+                        const int nbj = CL.nb(j), below = NP - CHOL_NB * j - nbj, rb = S.rows_bwd(CL, j);
+                        for (int r0 = 0; r0 < below; r0 += rb) push(Ap + CL.off_c(j) + (size_t)(nbj + r0) * nbj, (unsigned)min(rb, below - r0) * nbj * 16u);
+                        push(Ap + CL.off_c(j), (unsigned)nbj * nbj * 16u);
+                    }
+                }
+                push_K(Kp);
+            }
         return;
     }
     // ---------------- consumers (256 threads)
-    const double vel = a.v[t], h = a.h;
+    const double vel = a.v[t];
     for (int j = tid; j < N; j += SW_CONSUMERS) {
         const double *src = a.C + ((size_t)t * N + j) * 2;
         C[j] = {src[0], src[1]}; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0};
+    }
+    // first position of this window whose overlap factorisation failed (n_idx: none)
+    int first_bad = a.n_idx;
+    if (a.flags) {
+        for (int li = tid; li < a.n_idx; li += SW_CONSUMERS) if (a.flags[(size_t)t * a.n_idx + li]) first_bad = min(first_bad, li);
+        first_bad = __reduce_min_sync(0xffffffffu, first_bad);
+        if (lane == 0) redi[warp] = first_bad;
     }
     double drift = track ? a.drift[t] : 0.0;
     long long g = 0;                                         // chunk counter, in step with the producer
@@ -673,8 +668,10 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
         ++g;
     };
     consumer_sync();
+    if (a.flags) { for (int w = 0; w < 8; ++w) first_bad = min(first_bad, redi[w]); }
 
     for (int s = 0; s < a.steps; ++s) {
+        const double h = a.hs[s];
         #pragma unroll 1
         for (int st = 0; st < 5; ++st) {
             // st = 0..3: RK4 stages; st = 4: norm c^H S c at z_new (only when drift is tracked)
@@ -682,7 +679,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
             const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
             const double alpha = (st == 0 || st == 4) ? 0.0 : (st == 3 ? h : 0.5 * h);
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
-            const double z = zpos(a.z_min, h, a.i0 + li);
+            const double z = a.zh[li];
             for (int j = tid; j < N; j += SW_CONSUMERS) {
                 const double e = (j < NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - NT]];
                 double sn, cs; sincos(e * z / vel, &sn, &cs);
@@ -737,17 +734,78 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
                 release();
             }
             consumer_sync();
-            // w_P = Ainv y_P
-            for (int q = 0; q < S.nA; ++q) {
-                const cplx *buf = acquire();
-                const int r0 = q * S.rA, rows = min(S.rA, NP - r0);
-                for (int r = warp; r < rows; r += 8) {
-                    const cplx d = warp_dot(buf + (size_t)r * NP, Y + NT, NP, lane);
-                    if (lane == 0) Wp[r0 + r] = d;
+            if (!SOLVE) {
+                // w_P = Ainv y_P
+                for (int q = 0; q < S.nA; ++q) {
+                    const cplx *buf = acquire();
+                    const int r0 = q * S.rA, rows = min(S.rA, NP - r0);
+                    for (int r = warp; r < rows; r += 8) {
+                        const cplx d = warp_dot(buf + (size_t)r * NP, Y + NT, NP, lane);
+                        if (lane == 0) Wp[r0 + r] = d;
+                    }
+                    release();
                 }
-                release();
+                consumer_sync();
+            } else {
+                // forward solve L w = y_P:  w_j = Linv_jj (y_j - sum_{i<j} L_ji w_i)
+                for (int j = 0; j < CL.nblk; ++j) {
+                    const int nbj = CL.nb(j), len = CL.len(j), j0 = CHOL_NB * j, rf = S.rows_fwd(CL, j);
+                    for (int q0 = 0; q0 < nbj; q0 += rf) {
+                        const cplx *buf = acquire();
+                        const int rows = min(rf, nbj - q0);
+                        for (int r = warp; r < rows; r += 8) {
+                            const cplx *row = buf + (size_t)r * len;
+                            const cplx d = warp_dot(row, Wp, j0, lane);
+                            if (lane == 0) { const cplx y = Y[NT + j0 + q0 + r]; Tj[q0 + r] = {y.x - d.x, y.y - d.y}; }
+                            if (lane < nbj) Dblk[(q0 + r) * SW_DLD + lane] = row[j0 + lane];
+                        }
+                        release();
+                    }
+                    consumer_sync();
+                    for (int r = warp; r < nbj; r += 8) {
+                        double sr = 0.0, si = 0.0;
+                        if (lane <= r) { const cplx l = Dblk[r * SW_DLD + lane], x = Tj[lane]; sr = l.x * x.x - l.y * x.y; si = l.x * x.y + l.y * x.x; }
+                        sr = warp_sum(sr); si = warp_sum(si);
+                        if (lane == 0) Wp[j0 + r] = {sr, si};
+                    }
+                    consumer_sync();
+                }
+                // backward solve L^H x = w:  x_j = Linv_jj^H (w_j - sum_{i>j} L_ij^H x_i), in place in Wp
+                for (int j = CL.nblk - 1; j >= 0; --j) {
+                    const int nbj = CL.nb(j), j0 = CHOL_NB * j, below = NP - j0 - nbj, rb = S.rows_bwd(CL, j);
+                    double pr = 0.0, pi = 0.0;                                   // lane = column c of block j
+                    for (int q0 = 0; q0 < below; q0 += rb) {
+                        const cplx *buf = acquire();
+                        const int rows = min(rb, below - q0);
+                        if (lane < nbj)
+                            for (int r = warp; r < rows; r += 8) {
+                                const cplx l = buf[(size_t)r * nbj + lane], x = Wp[j0 + nbj + q0 + r];
+                                pr += l.x * x.x + l.y * x.y; pi += l.x * x.y - l.y * x.x;      // conj(l) x
+                            }
+                        release();
+                    }
+                    part2[warp * CHOL_NB + lane] = {pr, pi};
+                    consumer_sync();
+                    {
+                        const cplx *buf = acquire();                            // Linv_jj [nbj][nbj]
+                        if (warp == 0) {
+                            if (lane < nbj) {
+                                cplx u = Wp[j0 + lane];
+                                for (int w = 0; w < 8; ++w) { u.x -= part2[w * CHOL_NB + lane].x; u.y -= part2[w * CHOL_NB + lane].y; }
+                                Tj[lane] = u;
+                            }
+                            __syncwarp();
+                            if (lane < nbj) {
+                                double sr = 0.0, si = 0.0;
+                                for (int k = lane; k < nbj; ++k) { const cplx l = buf[(size_t)k * nbj + lane], u = Tj[k]; sr += l.x * u.x + l.y * u.y; si += l.x * u.y - l.y * u.x; }
+                                Wp[j0 + lane] = {sr, si};
+                            }
+                        }
+                        release();
+                    }
+                    consumer_sync();
+                }
             }
-            consumer_sync();
             // w_T = y_T - K^H w_P: per-warp partial sums over its rows of K
             for (int q = 0; q < S.nK; ++q) {
                 const cplx *buf = acquire();
@@ -774,8 +832,17 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
             consumer_sync();
         }
     }
-    for (int j = tid; j < N; j += SW_CONSUMERS) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = C[j].x; dst[1] = C[j].y; }
-    if (track && tid == 0) a.drift[t] = drift;
+    // a trajectory that met a failed factorisation (or had met one in an earlier window) has no amplitudes: NaN, and the
+    // first failed half-step index is kept in traj_status (wpccc_last_status)
+    const bool dead = first_bad < a.n_idx || (a.traj_status && a.traj_status[t] != 0);
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    for (int j = tid; j < N; j += SW_CONSUMERS) {
+        double *dst = a.C + ((size_t)t * N + j) * 2;
+        dst[0] = dead ? qnan : C[j].x; dst[1] = dead ? qnan : C[j].y;
+    }
+    if (tid == 0 && a.traj_status && a.traj_status[t] == 0 && first_bad < a.n_idx)
+        a.traj_status[t] = (a.flags[(size_t)t * a.n_idx + first_bad] << 28) | ((int)(a.i0 + first_bad) + 1);
+    if (track && tid == 0) a.drift[t] = dead ? qnan : drift;
 }
 }  // namespace
 
@@ -798,8 +865,8 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
     if (n_units <= 0 || a.steps <= 0) return 0;
     const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + ((size_t)4 * a.nv * a.N + (size_t)a.nv * a.n_rad) * 16;
     if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
-    static size_t attr = 0;
-    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_sweep1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    static PerDevice attr_1;
+    if (wp_raise(attr_1, smem)) WP_CUDA(cudaFuncSetAttribute(k_sweep1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     wp_span_begin(B, FAM_SWEEP, s);
     k_sweep1<<<n_units, SW_CONSUMERS + 32, smem, s>>>(a);
     wp_span_end(B, s, 1);
@@ -810,42 +877,48 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
 int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStream_t s) {
     if (n_traj <= 0 || a.steps <= 0) return 0;
     const int N = a.NT + a.NP;
-    const size_t vec = ((size_t)6 * N + a.NP + (size_t)8 * a.NT) * 16;
+    const size_t vec = ((size_t)6 * N + a.NP + (size_t)8 * a.NT + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB) * 16;
     // ring chunk: at least one row of H0 (16 N bytes), about 40 KB, so that four of them and the vectors fit 220 KB
     size_t chunk = 40 * 1024;
     while (chunk > (size_t)16 * N && SW_STAGES * chunk + vec > 220 * 1024) chunk -= 1024;
-    chunk = std::max(chunk, (size_t)16 * N);
+    chunk = std::max(chunk, std::max((size_t)16 * N, (size_t)16 * CHOL_NB * CHOL_NB));     // a row of H0, a diagonal block of the factor
     chunk = (chunk + 127) & ~(size_t)127;
     const size_t smem = SW_STAGES * chunk + vec;
     if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
-    static size_t attr = 0;
-    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_sweep2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    static PerDevice attr_2;
+    if (wp_raise(attr_2, smem)) {
+        WP_CUDA(cudaFuncSetAttribute(k_sweep2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        WP_CUDA(cudaFuncSetAttribute(k_sweep2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
     wp_span_begin(B, FAM_SWEEP, s);
-    k_sweep2<<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
+    if (a.solve) k_sweep2<true><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
+    else k_sweep2<false><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;
 }
 
-int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cudaStream_t s) {
+int wp_factor_cholesky(wpccc_basis *B, int n_pos, const double *d_K, double *d_out, int *d_flags, void *d_scratch, cudaStream_t s);
+
+int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, int *d_flags, void *d_scratch, cudaStream_t s) {
     if (n_pos <= 0) return 0;
+    if (B->opt.solve_route == 0) return wp_factor_cholesky(B, n_pos, d_K, d_Ainv, d_flags, d_scratch, s);
     FactorArgs a{};
-    a.K = d_K; a.Ainv = d_Ainv; a.status = B->d_status; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states;
+    a.K = d_K; a.Ainv = d_Ainv; a.flags = d_flags; a.NT = B->c[0].n_states; a.NP = B->c[1].n_states; a.out_stride = wp_factor_elems(a.NP);
     const size_t n = a.NP, small = 2 * n * 16 + 2 * n * 4 + 64;
     const size_t budget = 200 * 1024;
-    auto env_on = [](const char *name) { const char *e = getenv(name); return e && e[0] == '1'; };
-    const bool force_blocked = env_on("WPCCC_FACTOR_BLOCKED");               // tests: global-memory blocked route
-    const bool no_reg = env_on("WPCCC_FACTOR_NOREG");                        // tests, A/B timing: shared-memory route
+    const bool force_blocked = B->opt.inverse_kernel == 2;                   // wpccc_set_option "inverse_kernel": global-memory blocked route
+    const bool no_reg = B->opt.inverse_kernel == 1;                          // shared-memory route
     if (n <= (size_t)FR_NMAX && !force_blocked && !no_reg) {                    // A in registers
         const size_t tail = (2 * FR_NMAX * FR_NB + FR_NB * FR_NMAX) * 16 + 4 * FR_NMAX * 4;
         size_t cwr = (size_t)a.NT | 1;                                        // odd row stride: conflict-free column reads
         const size_t cw_max = ((160 * 1024 - tail) / (n * 16) - 1) | 1;
         if (cwr > cw_max) cwr = cw_max;
-        if (const char *e = getenv("WPCCC_FACTOR_CW")) { const size_t t = (size_t)std::max(1, atoi(e)) | 1; if (t < cwr) cwr = t; }   // tests: K staged in several chunks
+        if (B->opt.inverse_chunk_cols > 0) { const size_t t = (size_t)B->opt.inverse_chunk_cols | 1; if (t < cwr) cwr = t; }   // K staged in several chunks
         a.cw = (int)cwr;
         const size_t smem = n * cwr * 16 + tail;
-        static size_t attr_r = 0;
-        if (smem > attr_r) { WP_CUDA(cudaFuncSetAttribute(k_factor_reg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_r = smem; }
+        static PerDevice attr_r;
+        if (wp_raise(attr_r, smem)) WP_CUDA(cudaFuncSetAttribute(k_factor_reg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         wp_span_begin(B, FAM_FACT, s);
         k_factor_reg<<<n_pos, FR_THREADS, smem, s>>>(a);
         wp_span_end(B, s, 1);
@@ -864,8 +937,8 @@ int wp_factor(wpccc_basis *B, int n_pos, const double *d_K, double *d_Ainv, cuda
     if (a.use_smem && cw < 2 * FJ_NB + 1) cw = 2 * FJ_NB + 1;    // the K chunk area doubles as the panel buffers (N_T < 17)
     a.cw = cw;
     const size_t smem = a.use_smem ? fixed + n * cw * 16 : std::max(fixed + n * cw * 16, blocked_need);
-    static size_t attr = 0;
-    if (smem > attr) { WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    static PerDevice attr_f;
+    if (wp_raise(attr_f, smem)) WP_CUDA(cudaFuncSetAttribute(k_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     wp_span_begin(B, FAM_FACT, s);
     k_factor<<<n_pos, 512, smem, s>>>(a);
     wp_span_end(B, s, 1);

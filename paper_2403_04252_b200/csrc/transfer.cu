@@ -17,19 +17,10 @@
 //     only q, q' >= 0 columns are tabulated and contracted; the two families Phi_{|q-q'|} and Phi_{q+q'} of ring
 //     weights rebuild all sign combinations;
 //   * Phi^+_{-Delta} = conj(Phi^-_Delta) and the axial phases are conjugate, so H_TP shares the weights of S_PT.
-#include <cstdlib>
-
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace {
-
-struct cplx { double x, y; };
-__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
-
-__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
 
 constexpr int MAXD = 2 * WP_MAX_L;          // largest Delta
 constexpr int NLQ = (WP_MAX_L + 1) * (WP_MAX_L + 2) / 2;
@@ -119,6 +110,7 @@ struct TtabArgs {
     const int *colidx[2];                    // [n_rad][WP_MAX_L+1] column of (a, q) or -1
     double Zother[2];                        // side 0 (T functions): Z_P;  side 1: Z_T
     double h; int Nr, KC;                    // KC: z' nodes per CTA (multiple of 4)
+    int sph;                                 // 1: spheroidal nodes: ring = eta_i (pos[off_rho]), axial node = tau_k (pos[off_zq])
     double *out[2]; size_t pos_stride[2];    // doubles per position for each side
     int lmax[2];
     SelDev sel; int q0;
@@ -149,11 +141,21 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
 
     if (tid < KC) {
         const double rho = pt[a.L.off_rho() + ring], zk = pt[a.L.off_zq() + k0 + tid];
-        const double zP = __dsub_rn(zk, R);
-        const double rT = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zk, zk)));
-        const double rP = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zP, zP)));
-        const double rs = side ? rP : rT, ro = side ? rT : rP;
-        const double c = (side ? zP : zk) / rs;
+        double rs, ro, c;
+        if (a.sph) {
+            // eq. (9): r_T = R (eta + tau)/2, r_P = R (eta - tau)/2, cos th'_T = (eta tau + 1)/(eta + tau), cos th'_P = (eta tau - 1)/(eta - tau)
+            const double eta = rho, tau = zk, hR = __dmul_rn(0.5, R), et = __dmul_rn(eta, tau);
+            const double sp = __dadd_rn(eta, tau), sm_ = __dsub_rn(eta, tau);
+            const double rT = __dmul_rn(hR, sp), rP = __dmul_rn(hR, sm_);
+            rs = side ? rP : rT; ro = side ? rT : rP;
+            c = side ? __dsub_rn(et, 1.0) / sm_ : __dadd_rn(et, 1.0) / sp;
+        } else {
+            const double zP = __dsub_rn(zk, R);
+            const double rT = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zk, zk)));
+            const double rP = sqrt(__dadd_rn(__dmul_rn(rho, rho), __dmul_rn(zP, zP)));
+            rs = side ? rP : rT; ro = side ? rT : rP;
+            c = (side ? zP : zk) / rs;
+        }
         int j = (int)floor(rs / a.h + 0.5);
         j = max(2, min(a.Nr - 2, j));
         const double t = rs / a.h - (double)j;
@@ -229,23 +231,6 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------ contraction (a5)
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
-    asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
-        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
 // TMA ring of the contraction: 3 stages of 16 k4-groups of z' nodes per operand (256 doubles each), 192 KB.
 // Mirror-pair kernel (DUAL): the 64 accumulators per thread of the mirror position (128 KB per CTA; the register file
 // holds the 96 of the position itself) live in tensor memory, 256 of the SM's 512 TMEM columns, moved with
@@ -327,10 +312,6 @@ __device__ __forceinline__ void tcon_stage(const double *Ab, const double *Bb, c
         #pragma unroll 2
         for (int kc = 0; kc < nk; ++kc) { load(0, kc); mma(0); }
     }
-}
-
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
 
 // grid = (tile, ring split, position); block = 4 (rows) x 8/NJ (cols) warps; warp tile 16 x 8 NJ complex
@@ -519,6 +500,199 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
         __syncthreads();
         if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(s_tmem), "n"(TcRing<DUAL>::TMEM_COLS));
     }
+}
+
+// ------------------------------------------------------------------------------------------------ spheroidal rule (NEXT-2)
+// eq. (9) in the paper's own coordinates: eta_i Gauss-Laguerre, tau_k Gauss-Legendre, analytic azimuth.
+// The weight  W_d(i,k) = w^eta_i w^tau_k (R/2)^3 (eta_i^2 - tau_k^2) e^{-i v cosTh (R/2) eta_i tau_k} (+i)^d J_d(x_ik),
+// x_ik = v sinTh (R/2) sqrt((eta_i^2 - 1)(1 - tau_k^2)), does not separate into a ring and an axial factor, so the
+// contraction applies it per 8 x 8 sub-tile: the columns (a, q >= 0) are grouped by q and every group is padded to a
+// multiple of 8, hence a sub-tile has one q and one q' and needs W_{|q-q'|} (family -) and W_{q+q'} (family +).
+// Table layout per position: Wd [ring i][k4-group kc][d = 0..dmax][4 nodes] complex (one TMA bulk copy per stage).
+
+// J_0 .. J_dmax (x), x >= 0: three-term series for x < 1e-3, else Miller's backward recurrence normalised by
+// J_0 + 2 sum_{k>=1} J_2k = 1.
+__device__ void bessel_j_all(double x, int dmax, double *J) {
+    if (x < 1e-3) {
+        const double hx = 0.5 * x, h2 = hx * hx;
+        double pw = 1.0, fact = 1.0;
+        for (int d = 0; d <= dmax; ++d) {
+            if (d > 0) { pw *= hx; fact *= d; }
+            J[d] = pw / fact * (1.0 - h2 / (d + 1) + h2 * h2 / (2.0 * (d + 1) * (d + 2)));
+        }
+        return;
+    }
+    int M = (int)(x + 14.0 * cbrt(x) + 32.0) + dmax;
+    M += M & 1;                                              // even start order
+    double jp = 0.0, jc = 1e-30, sum = 0.0;                  // J_{k+1}, J_k (unnormalised), k = M
+    const double tox = 2.0 / x;
+    for (int k = M; k >= 1; --k) {
+        const double jm = k * tox * jc - jp;                 // J_{k-1}
+        jp = jc; jc = jm;
+        if (k - 1 <= dmax) J[k - 1] = jc;
+        if (((k - 1) & 1) == 0 && k - 1 > 0) sum += jc;
+        if (fabs(jc) > 1e200) { jc *= 1e-200; jp *= 1e-200; sum *= 1e-200; for (int d = k - 1; d <= dmax && d < M; ++d) if (d >= k - 1) J[d] *= 1e-200; }
+    }
+    const double norm = 1.0 / (2.0 * sum + jc);              // jc = J_0
+    for (int d = 0; d <= dmax; ++d) J[d] *= norm;
+}
+
+struct TsphArgs {
+    PosTabs L; const double *R, *cosT, *sinT, *v; const double *gl_eta, *gl_tau; double eta_scale;
+    double *out; double *wd; size_t wd_stride;      // per-position tables (eta_i, tau_k) and weights
+    int q0;
+};
+
+// grid = (ring, position), block = n_z threads (one per tau node), rounded up to a warp multiple
+__global__ void __launch_bounds__(256) k_tpos_sph(const TsphArgs a) {
+    const int ring = blockIdx.x, p = blockIdx.y, gp = a.q0 + p;
+    const PosTabs &L = a.L;
+    double *o = a.out + (size_t)p * L.size();
+    const double R = a.R[gp], cT = a.cosT[gp], sT = a.sinT[gp], v = a.v[gp];
+    const double s = __dmul_rn(__dmul_rn(0.5, a.eta_scale), R);                      // x = s (eta - 1)
+    const double eta = __dadd_rn(1.0, a.gl_eta[ring] / s), weta = a.gl_eta[L.n_rho + ring] / s;
+    if (threadIdx.x == 0) o[L.off_rho() + ring] = eta;
+    const double hR = __dmul_rn(0.5, R), hR3 = hR * hR * hR;
+    cplx *wd = reinterpret_cast<cplx *>(a.wd + (size_t)p * a.wd_stride) + (size_t)ring * L.n_z * (L.dmax + 1);
+    for (int k = threadIdx.x; k < L.n_z; k += blockDim.x) {
+        const double tau = a.gl_tau[k], wtau = a.gl_tau[L.n_z + k];
+        if (ring == 0) o[L.off_zq() + k] = tau;
+        const double W = weta * wtau * hR3 * (eta * eta - tau * tau);
+        const double x = fabs(v * sT * hR) * sqrt(fmax(0.0, (eta * eta - 1.0) * (1.0 - tau * tau)));
+        double sn, cs; sincos(-(v * cT * hR) * (eta * tau), &sn, &cs);
+        double J[MAXD + 1];
+        bessel_j_all(x, L.dmax, J);
+        const bool neg = v * sT < 0.0;                       // J_d(-x) = (-1)^d J_d(x)
+        for (int d = 0; d <= L.dmax; ++d) {
+            const double j = (neg && (d & 1)) ? -J[d] : J[d];
+            // (+i)^d J_d times W e^{-i ...}
+            double pr, pi;
+            switch (d & 3) { case 0: pr = j; pi = 0.0; break; case 1: pr = 0.0; pi = j; break; case 2: pr = -j; pi = 0.0; break; default: pr = 0.0; pi = -j; }
+            const double wr = W * (pr * cs - pi * sn), wi = W * (pr * sn + pi * cs);
+            wd[((size_t)(k >> 2) * (L.dmax + 1) + d) * 4 + (k & 3)] = cplx{wr, wi};
+        }
+    }
+}
+
+struct TconSphArgs {
+    PosTabs L;
+    const double *tabT, *tabP; size_t strideT, strideP;
+    const double *wd; size_t wd_stride;
+    int nq8T, nq8P;
+    const int *qT, *qP;
+    const int2 *tiles;
+    double *part;                                                // [p][fam 2][prod 3][nq8P][nq8T] complex
+    int stages;                                                  // TMA ring depth (2 or 3)
+};
+
+constexpr int TS_KCS = 16, TS_STAGE_DOUBLES = TS_KCS * 256;
+
+// grid = (tile, 1, position); 8 warps as 4 (rows) x 2 (cols), warp tile 16 x 32 of a 64 x 64 tile; both families are
+// accumulated directly (no ring epilogue): M += (B W_{|q-q'|})^T A, P += (B W_{q+q'})^T A for q, q' > 0.
+__global__ void __launch_bounds__(256, 1) k_tcon_sph(const TconSphArgs a) {
+    constexpr int NJ = 4;
+    extern __shared__ __align__(128) double sm[];
+    const int NS = a.stages, nd = a.L.dmax + 1;
+    const int w_stage = TS_KCS * nd * 8;                         // doubles of weights per stage
+    double *sA = sm, *sB = sA + NS * TS_STAGE_DOUBLES, *sW = sB + NS * TS_STAGE_DOUBLES;
+    __shared__ __align__(8) unsigned long long bar[3], empty[3];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, p = blockIdx.z;
+    const int2 tl = a.tiles[blockIdx.x];
+    const int rt = tl.x, ct = tl.y;
+    const int n_rho = a.L.n_rho, nkc = a.L.n_z / 4, spr = (nkc + TS_KCS - 1) / TS_KCS, n_st = n_rho * spr;
+    if (tid == 0) { for (int s = 0; s < NS; ++s) { mbar_init(&bar[s], 1); mbar_init(&empty[s], 8); } mbar_fence_init(); }
+    __syncthreads();
+    const double *gA = a.tabT + (size_t)p * a.strideT + (size_t)ct * n_rho * nkc * 256;
+    const double *gB = a.tabP + (size_t)p * a.strideP + (size_t)rt * n_rho * nkc * 256;
+    const double *gW = a.wd + (size_t)p * a.wd_stride;
+    auto issue = [&](int st) {
+        const int ring = st / spr, kc0 = (st % spr) * TS_KCS, nk = min(TS_KCS, nkc - kc0), buf = st % NS;
+        const unsigned bytes = (unsigned)nk * 256 * 8, wbytes = (unsigned)nk * nd * 64;
+        mbar_expect_tx(&bar[buf], 2 * bytes + wbytes);
+        tma_bulk_g2s(sA + buf * TS_STAGE_DOUBLES, gA + ((size_t)ring * nkc + kc0) * 256, bytes, &bar[buf]);
+        tma_bulk_g2s(sB + buf * TS_STAGE_DOUBLES, gB + ((size_t)ring * nkc + kc0) * 256, bytes, &bar[buf]);
+        tma_bulk_g2s(sW + buf * w_stage, gW + ((size_t)ring * nkc + kc0) * nd * 8, wbytes, &bar[buf]);
+    };
+    if (tid == 0) for (int st = 0; st < min(NS, n_st); ++st) issue(st);
+
+    const int wr = warp / 2, wc = warp % 2, fr = lane >> 2, fk = lane & 3;
+    bool need[2][NJ]; int dm[2][NJ], dp[2][NJ];                  // weight offsets (doubles) into a k4-group of sW; dp < 0: family + empty
+    bool any_need = false;
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int r8 = rt * 64 + 16 * wr + 8 * i, c8 = ct * 64 + 32 * wc + 8 * j;
+            need[i][j] = (r8 < 2 * a.nq8P) && (c8 < 2 * a.nq8T) && !(r8 >= a.nq8P && c8 >= a.nq8T);
+            int qp = 0, qq = 0;
+            if (need[i][j]) { qp = max(0, a.qP[r8 % a.nq8P]); qq = max(0, a.qT[c8 % a.nq8T]); }
+            dm[i][j] = abs(qq - qp) * 8 + 2 * fk;
+            dp[i][j] = (qp > 0 && qq > 0) ? (qq + qp) * 8 + 2 * fk : -1;
+            any_need |= need[i][j];
+        }
+    double Mre[2][NJ][2], Mim[2][NJ][2], Pre[2][NJ][2], Pim[2][NJ][2];
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < NJ; ++j)
+            #pragma unroll
+            for (int e = 0; e < 2; ++e) Mre[i][j][e] = Mim[i][j][e] = Pre[i][j][e] = Pim[i][j][e] = 0.0;
+
+    for (int st = 0; st < n_st; ++st) {
+        const int buf = st % NS, kc0 = (st % spr) * TS_KCS, nk = min(TS_KCS, nkc - kc0);
+        mbar_wait(&bar[buf], (st / NS) & 1);
+        if (any_need) {
+            const double *Ab = sA + buf * TS_STAGE_DOUBLES + (NJ * wc) * 32 + lane;
+            const double *Bb = sB + buf * TS_STAGE_DOUBLES + (2 * wr) * 32 + lane;
+            const double *Wb = sW + buf * w_stage;
+            #pragma unroll 2
+            for (int kc = 0; kc < nk; ++kc) {
+                double af[NJ], bb[2];
+                #pragma unroll
+                for (int j = 0; j < NJ; ++j) af[j] = Ab[kc * 256 + j * 32];
+                #pragma unroll
+                for (int i = 0; i < 2; ++i) bb[i] = Bb[kc * 256 + i * 32];
+                const double *wk = Wb + kc * nd * 8;
+                #pragma unroll
+                for (int i = 0; i < 2; ++i)
+                    #pragma unroll
+                    for (int j = 0; j < NJ; ++j)
+                        if (need[i][j]) {
+                            const double2 wm = *reinterpret_cast<const double2 *>(wk + dm[i][j]);
+                            dmma884(Mre[i][j][0], Mre[i][j][1], bb[i] * wm.x, af[j]);
+                            dmma884(Mim[i][j][0], Mim[i][j][1], bb[i] * wm.y, af[j]);
+                            if (dp[i][j] >= 0) {
+                                const double2 wp = *reinterpret_cast<const double2 *>(wk + dp[i][j]);
+                                dmma884(Pre[i][j][0], Pre[i][j][1], bb[i] * wp.x, af[j]);
+                                dmma884(Pim[i][j][0], Pim[i][j][1], bb[i] * wp.y, af[j]);
+                            }
+                        }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[buf]);
+        if (tid == 0 && st >= 1 && st - 1 + NS < n_st) {
+            mbar_wait(&empty[(st - 1) % NS], ((st - 1) / NS) & 1);
+            issue(st - 1 + NS);
+        }
+    }
+    const size_t blk = (size_t)a.nq8P * a.nq8T;
+    double *o = a.part + (size_t)p * 6 * blk * 2;
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < NJ; ++j)
+            #pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int gr = rt * 64 + 16 * wr + 8 * i + fr, gc = ct * 64 + 32 * wc + 8 * j + 2 * fk + e;
+                if (!need[i][j] || gr >= 2 * a.nq8P || gc >= 2 * a.nq8T) continue;
+                if (a.qP[gr % a.nq8P] < 0 || a.qT[gc % a.nq8T] < 0) continue;            // padding column
+                const int hr = gr / a.nq8P, ir = gr % a.nq8P, hc = gc / a.nq8T, ic = gc % a.nq8T;
+                const int prod = hr ? 2 : (hc ? 1 : 0);
+                const size_t idx = ((size_t)prod * blk + (size_t)ir * a.nq8T + ic) * 2;
+                o[idx] = Mre[i][j][e]; o[idx + 1] = Mim[i][j][e];
+                o[3 * blk * 2 + idx] = Pre[i][j][e]; o[3 * blk * 2 + idx + 1] = Pim[i][j][e];
+            }
 }
 
 // ------------------------------------------------------------------------------------------------ rotation (a6)
@@ -733,15 +907,14 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         sd = SelDev{sel->n_idx - n_fetch, sel->n_idx, sel->n_pre, sel->suf0};
         n_eval = sel->n_groups * sd.n_c;
     }
-    static bool consts = false;
-    if (!consts) {
+    static PerDevice consts;
+    if (wp_raise(consts, 1)) {
         double f[2 * WP_MAX_L + 2]; f[0] = 1.0;
         for (int i = 1; i < 2 * WP_MAX_L + 2; ++i) f[i] = f[i - 1] * i;
         WP_CUDA(cudaMemcpyToSymbol(c_fact, f, sizeof f));
         double tn[NLQ];
         for (int l = 0; l <= WP_MAX_L; ++l) for (int q = 0; q <= l; ++q) tn[lq_index(l, q)] = std::sqrt((2 * l + 1) / 2.0 * f[l - q] / f[l + q]);
         WP_CUDA(cudaMemcpyToSymbol(c_thnorm, tn, sizeof tn));
-        consts = true;
     }
     const int max_chunk = wp_transfer_chunk_positions(B, ws_bytes);
     if (max_chunk < 1) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small (%zu bytes)", ws_bytes);
@@ -783,8 +956,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     WP_CUDA(cudaMemcpyAsync(d_rowbase, rowbase.data(), rowbase.size() * sizeof(int), cudaMemcpyHostToDevice, s));
     const size_t rot_smem = rot_nd + 2 * (size_t)rot_max_rows * ((size_t)P.nq8[0] + B->c[0].n_states) * 16 + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
     if (rot_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the rotation kernel's shared memory");
-    static size_t rot_attr = 0;
-    if (rot_smem > rot_attr) { WP_CUDA(cudaFuncSetAttribute(k_trot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem)); rot_attr = rot_smem; }
+    static PerDevice rot_attr;
+    if (wp_raise(rot_attr, rot_smem)) WP_CUDA(cudaFuncSetAttribute(k_trot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
     {   // padding columns of the node tables are never written by k_ttab: zero the buffer once per API call
         const size_t tab_bytes = (size_t)((char *)d_part - (char *)d_tab[0]);
         if (B->tab_zeroed != d_tab[0] || B->tab_zeroed_bytes != tab_bytes) {      // (the layout depends on the chunk size)
@@ -807,7 +980,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     const int nlq = (lmx + 1) * (lmx + 2) / 2;
     const int KC = (P.L.n_z % 64 == 0) ? 64 : ((P.L.n_z % 32 == 0) ? 32 : 16);
     const size_t tab_smem = (size_t)(7 + nlq) * KC * 8 + (size_t)KC * 4 + 64;
-    static size_t con_attr = 0;
+    static PerDevice con_attr, dual_attr;
     const size_t con_tabs = 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho;
     const size_t con_smem = ((size_t)2 * TcRing<false>::STAGES * TcRing<false>::STAGE_DOUBLES + con_tabs) * 8;
     const size_t dual_smem = dual_smem_bytes(P);
@@ -815,17 +988,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     // mirror-pair kernel: whenever some evaluated position of this window has a stash slot
     const bool dual = sel && sel->stash && sel->n_st > 0 && sel->i0 < sel->i_mid && sel->i0 + sel->n_pre > sel->i_mid - sel->n_st;
     if (dual && dual_smem > 226 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: mirror stash requested but the pair kernel does not fit shared memory");
-    static const int tcon_nj = []() { const char *e = getenv("WPCCC_TCON_NJ"); return (e && atoi(e) == 2) ? 2 : 4; }();
-    if (con_smem > con_attr) {
-        WP_CUDA(cudaFuncSetAttribute(k_tcon<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
-        WP_CUDA(cudaFuncSetAttribute(k_tcon<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
-        con_attr = con_smem;
-    }
-    static size_t dual_attr = 0;
-    if (dual && dual_smem > dual_attr) {
-        WP_CUDA(cudaFuncSetAttribute(k_tcon<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dual_smem));
-        dual_attr = dual_smem;
-    }
+    if (wp_raise(con_attr, con_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+    if (dual && wp_raise(dual_attr, dual_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dual_smem));
 
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
     TrotArgs tr{}; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta;
@@ -863,8 +1027,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         dim3 gc((unsigned)P.tiles.size(), n_split, np);
         wp_span_begin(B, FAM_TCON, s);
         if (dual) k_tcon<4, true><<<gc, 256, dual_smem, s>>>(tc);
-        else if (tcon_nj == 4) k_tcon<4, false><<<gc, 256, con_smem, s>>>(tc);
-        else k_tcon<2, false><<<gc, 512, con_smem, s>>>(tc);
+        else k_tcon<4, false><<<gc, 256, con_smem, s>>>(tc);
         wp_span_end(B, s, 1);
         B->units[FAM_TCON] += np;
         WP_CUDA(cudaGetLastError());

@@ -188,7 +188,7 @@ def test_two_centre_propagation(lib, two_centre):
     assert np.abs(Cs - Cg).max() < 1e-13
 
 
-def test_two_centre_mirror_pairs(lib, two_centre, monkeypatch):
+def test_two_centre_mirror_pairs(lib, two_centre):
     """On a z-grid symmetric about 0 the body-frame integrals of (b, -z) and (b, +z) are evaluated together (wpccc.h,
     wpccc_last_units).  Several windows (150 steps > 64), full and partial stash, against the run with the pairing
     switched off; and an asymmetric grid, where pairing must switch itself off, against the oracle."""
@@ -204,10 +204,12 @@ def test_two_centre_mirror_pairs(lib, two_centre, monkeypatch):
     Cp = lib.propagate(basis, b, v, -9.0, 9.0, n_steps, ws_bytes=part).cpu().numpy()
     up = lib.last_units(basis)
     assert 3 * (n_steps + 2) < up["transfer_contraction"] < n_pos and part < base, (up, part, base)
-    monkeypatch.setenv("WPCCC_NO_MIRROR", "1")
-    C0 = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
-    assert lib.last_units(basis)["transfer_contraction"] == n_pos
-    monkeypatch.delenv("WPCCC_NO_MIRROR")
+    basis.set_option("mirror_pairs", 0)
+    try:
+        C0 = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
+        assert lib.last_units(basis)["transfer_contraction"] == n_pos
+    finally:
+        basis.set_option("mirror_pairs", 1)
     assert np.abs(Cm - C0).max() < 1e-12 and np.abs(Cp - C0).max() < 1e-12, (np.abs(Cm - C0).max(), np.abs(Cp - C0).max())
     Ca = lib.propagate(basis, b[:1], v[:1], -6.0, 4.0, 25).cpu().numpy()
     assert lib.last_units(basis)["transfer_contraction"] == 51
@@ -215,25 +217,68 @@ def test_two_centre_mirror_pairs(lib, two_centre, monkeypatch):
     assert np.abs(Ca[0] - co).max() < PTOL
 
 
-def test_two_centre_factor_routes(lib, two_centre, monkeypatch):
-    """The three routes of the a7 factorisation (matrix in registers for N_P <= 90, in shared memory, blocked in global
-    memory) choose the same pivots and differ by rounding only; each against the oracle.  N_P = 32 (whole panels) and
-    N_P = 9 (one lane group, ragged last panel)."""
+ROUTES = (("cholesky + triangular solves", {"solve_route": 0}),
+          ("inverse, registers", {"solve_route": 1}),
+          ("inverse, registers, K staged in chunks of 5 columns", {"solve_route": 1, "inverse_chunk_cols": 5}),
+          ("inverse, shared memory", {"solve_route": 1, "inverse_kernel": 1}),
+          ("inverse, global-memory blocked", {"solve_route": 1, "inverse_kernel": 2}))
+ROUTE_DEFAULTS = {"solve_route": 0, "inverse_kernel": 0, "inverse_chunk_cols": 0}
+
+
+def with_route(basis, opts, fn):
+    for k, val in {**ROUTE_DEFAULTS, **opts}.items():
+        basis.set_option(k, val)
+    try:
+        return fn()
+    finally:
+        for k, val in ROUTE_DEFAULTS.items():
+            basis.set_option(k, val)
+
+
+def test_two_centre_factor_routes(lib, two_centre):
+    """The routes of the a7 overlap solve (wpccc_set_option "solve_route": blocked Cholesky factor + triangular solves per
+    stage; explicit Gauss-Jordan inverse with the matrix in registers for N_P <= 90, in shared memory, blocked in global
+    memory) solve the same systems and differ by rounding only; each against the oracle's plain partial-pivoting solve
+    on the full S.  N_P = 32 (whole panels) and N_P = 9 (one lane group, ragged last panel / block)."""
     small = tiny_problem(True, l_max=1, n_max=2, bins=1, k_max=1.5, Nr=300, h=0.1, quad=dict(QUAD), seed=5)
-    for prob, basis, b, v, zr, n_steps in ((two_centre[0], two_centre[1], np.array([0.3, 1.1]), np.array([0.9, 1.4]), 7.0, 30),
+    for prob, basis, b, v, zr, n_steps in ((two_centre[0], two_centre[1], np.array([1.6, 1.1]), np.array([0.9, 1.4]), 7.0, 30),
                                            (small, lib.setup_basis(small), np.array([0.5]), np.array([1.2]), 6.0, 24)):
-        out = {}
-        for route, env, val in (("registers", None, None), ("registers, K staged in chunks of 5 columns", "WPCCC_FACTOR_CW", "5"),
-                                ("shared", "WPCCC_FACTOR_NOREG", "1"), ("blocked", "WPCCC_FACTOR_BLOCKED", "1")):
-            if env: monkeypatch.setenv(env, val)
-            out[route] = lib.propagate(basis, b, v, -zr, zr, n_steps).cpu().numpy()
-            if env: monkeypatch.delenv(env)
+        out = {name: with_route(basis, opts, lambda: lib.propagate(basis, b, v, -zr, zr, n_steps).cpu().numpy()) for name, opts in ROUTES}
         for t in range(len(b)):
             co = oprop.propagate(prob, b[t], v[t], -zr, zr, n_steps)
             for route, C in out.items():
                 assert np.abs(C[t] - co).max() < PTOL, (route, t, np.abs(C[t] - co).max())
         for route, C in out.items():
-            assert np.abs(C - out["shared"]).max() < 1e-11, route
+            assert np.abs(C - out["inverse, shared memory"]).max() < 1e-11, route
+
+
+def test_overlap_not_positive_definite_is_reported(lib, two_centre):
+    """With the coarse 24 x 8 x 48 rule the discretised overlap matrix of this basis is indefinite at small R: the default
+    route (Cholesky) reports the first such position of the trajectory (WPCCC_ESINGULAR, wpccc_last_status) and returns
+    NaN for it, the other trajectory is complete; the oracle confirms the sign change of the smallest eigenvalue of
+    I - K K^H exactly there; the explicit-inverse route propagates straight through (S is indefinite, not singular)."""
+    prob, basis = two_centre
+    b, v, zr, n_steps = np.array([0.3, 1.1]), np.array([0.9, 1.4]), 7.0, 30
+    with pytest.raises(lib.WpcccError) as ei:
+        lib.propagate(basis, b, v, -zr, zr, n_steps)
+    assert ei.value.code == -4 and "not positive definite" in str(ei.value)
+    C = lib.propagate(basis, b, v, -zr, zr, n_steps, allow_singular=True).cpu().numpy()
+    st = lib.last_status(basis, 2)
+    assert st[1] is None and st[0] is not None and st[0][0] == 3
+    assert np.isnan(C[0]).all() and np.isfinite(C[1]).all()
+    assert np.abs(C[1] - oprop.propagate(prob, b[1], v[1], -zr, zr, n_steps)).max() < PTOL
+    i_bad = st[0][1]
+    h = 2 * zr / n_steps
+    NT = prob.centres[0].n_states
+
+    def min_eig(i):
+        S, _ = assemble.S_and_H(prob, b[0], -zr + 0.5 * i * h, v[0], time_phase=False)
+        K = S[NT:, :NT]
+        return np.linalg.eigvalsh(np.eye(K.shape[0]) - K @ K.conj().T).min()
+
+    assert min_eig(i_bad) < 0.0 < min(min_eig(i) for i in range(max(0, i_bad - 3), i_bad))
+    Ci = with_route(basis, {"solve_route": 1}, lambda: lib.propagate(basis, b, v, -zr, zr, n_steps).cpu().numpy())
+    assert np.abs(Ci[0] - oprop.propagate(prob, b[0], v[0], -zr, zr, n_steps)).max() < PTOL
 
 
 def test_argument_errors(lib, one_centre):
