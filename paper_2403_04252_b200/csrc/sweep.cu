@@ -25,29 +25,35 @@ __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;
 constexpr int SW_STAGES = 4;
 constexpr int SW_CONSUMERS = 256;
 
+constexpr int SW1_CONSUMERS = 224;
+
 // ------------------------------------------------------------------ one-centre sweep
-// grid = units (up to nv trajectories that share b, hence D); block = 8 consumer warps + 1 producer warp.
+// grid = units (up to NV trajectories that share b, hence D); block = 7 consumer warps + 1 producer warp (256 threads: the full 255 registers per thread).
 // The real matrices D(z) do not depend on the amplitudes: the producer warp streams their rows through a
-// shared-memory ring with TMA bulk copies (running ahead across stages), the consumer warps do the GEMV for the nv
-// stage vectors at once.  Dynamic smem: ring, then C, Acc, X, Kn [nv][N] complex, ph [nv][n_rad] complex.
-__global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep1(const Sweep1Args a) {
+// shared-memory ring with TMA bulk copies (running ahead across stages).  D is symmetric (eq. (6) without the time
+// phase), so y_r = sum_c D[c][r] x_c: consumer thread r owns the rows r, r + 224, .. (NTILE of them) of every
+// trajectory of the unit, reads element r of each streamed row c (consecutive lanes, conflict-free) and the stage
+// vector x_c as a broadcast, and accumulates in registers -- no reductions, no re-reading of x per matrix row.  The
+// state (C, RK4 accumulator, phases) of a thread's rows lives in registers; only the stage vector X is shared
+// (double-buffered: one block barrier per RK4 stage).  Dynamic smem: ring, then X [2][NV][N] complex.
+template <int NTILE, int NV>
+__global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args a) {
     extern __shared__ __align__(128) unsigned char smraw1[];
     const SweepUnit u = a.units[blockIdx.x];
-    const int N = a.N, ld = a.ldD, nvm = a.nv, nv = u.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = a.N, ld = a.ldD, nv = u.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int rpc = a.rows_per_chunk, n_chunks = (N + rpc - 1) / rpc;
     const size_t chunk_bytes = (size_t)rpc * ld * 8;
     const int NS = a.ring_stages;
     unsigned char *ring = smraw1;
-    cplx *C = reinterpret_cast<cplx *>(smraw1 + (size_t)NS * chunk_bytes);
-    cplx *Acc = C + nvm * N, *X = Acc + nvm * N, *Kn = X + nvm * N, *ph = Kn + nvm * N;   // ph [nv][n_rad]
+    cplx *X = reinterpret_cast<cplx *>(smraw1 + (size_t)NS * chunk_bytes);           // [2][NV][N]
     __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
     __shared__ double red[SWEEP_NV][8];
     if (tid == 0) {
-        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW1_CONSUMERS / 32); }
+        mbar_fence_init();
     }
     __syncthreads();
-    if (warp == SW_CONSUMERS / 32) {
+    if (warp == SW1_CONSUMERS / 32) {
         if (lane != 0) return;
         const long long total = (long long)a.steps * 4 * n_chunks;
         for (long long g = 0; g < total; ++g) {
@@ -63,101 +69,139 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep1(const Sweep1Args a
         }
         return;
     }
-    double vel[SWEEP_NV];
+    // ---------------- consumers: thread tid owns rows tid + 224 t
+    int row[NTILE]; double eov[NTILE][NV];                  // eps of the row's radial function / v of the trajectory
+    cplx C[NTILE][NV], Acc[NTILE][NV], ph[NTILE][NV];
+    double vinv[NV];
     #pragma unroll
-    for (int q = 0; q < SWEEP_NV; ++q) vel[q] = (q < nv) ? a.v[u.traj[q]] : 1.0;
-    for (int q = 0; q < nv; ++q)
-        for (int j = tid; j < N; j += SW_CONSUMERS) {
-            const double *src = a.C + ((size_t)u.traj[q] * N + j) * 2;
-            C[q * N + j] = {src[0], src[1]}; Acc[q * N + j] = {0.0, 0.0}; Kn[q * N + j] = {0.0, 0.0};
+    for (int q = 0; q < NV; ++q) vinv[q] = (q < nv) ? 1.0 / a.v[u.traj[q]] : 1.0;
+    #pragma unroll
+    for (int t = 0; t < NTILE; ++t) {
+        row[t] = tid + SW1_CONSUMERS * t;
+        const int rc = min(row[t], N - 1);
+        const double e = a.eps[a.st_rad[rc]];
+        #pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            eov[t][q] = (q < nv) ? e / a.v[u.traj[q]] : 0.0;
+            C[t][q] = cplx{0.0, 0.0}; Acc[t][q] = cplx{0.0, 0.0};
+            if (q < nv && row[t] < N) { const double *src = a.C + ((size_t)u.traj[q] * N + row[t]) * 2; C[t][q] = cplx{src[0], src[1]}; }
         }
-    double drift[SWEEP_NV];
+    }
+    double drift[NV];
     #pragma unroll
-    for (int q = 0; q < SWEEP_NV; ++q) drift[q] = (a.drift && q < nv) ? a.drift[u.traj[q]] : 0.0;
-    consumer_sync();
+    for (int q = 0; q < NV; ++q) drift[q] = (a.drift && q < nv) ? a.drift[u.traj[q]] : 0.0;
+    const bool active = warp * 32 < N;                       // some lane of this warp owns a row
+    auto phases = [&](double z) {
+        #pragma unroll
+        for (int t = 0; t < NTILE; ++t)
+            #pragma unroll
+            for (int q = 0; q < NV; ++q) { double sn, cs; sincos(eov[t][q] * z, &sn, &cs); ph[t][q] = cplx{cs, sn}; }
+    };
+    // x = P^H (C + alpha k) of this thread's rows into the stage-vector buffer `xb`
+    auto put_x = [&](cplx *xb, double alpha, const cplx (&k)[NTILE][NV]) {
+        #pragma unroll
+        for (int t = 0; t < NTILE; ++t)
+            if (row[t] < N) {
+                #pragma unroll
+                for (int q = 0; q < NV; ++q)
+                    if (q < nv) xb[q * N + row[t]] = cmulc(cplx{C[t][q].x + alpha * k[t][q].x, C[t][q].y + alpha * k[t][q].y}, ph[t][q]);
+            }
+    };
+    cplx kk[NTILE][NV];
+    #pragma unroll
+    for (int t = 0; t < NTILE; ++t)
+        #pragma unroll
+        for (int q = 0; q < NV; ++q) kk[t][q] = cplx{0.0, 0.0};
+    phases(a.zh[0]);
+    put_x(X, 0.0, kk);
+    int xb = 0;
     long long g = 0;
+    bar_sync(1, SW1_CONSUMERS);
     for (int s = 0; s < a.steps; ++s) {
         const double h = a.hs[s];
         #pragma unroll 1
         for (int st = 0; st < 4; ++st) {
-            const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));       // local half-step index of this stage
-            const double alpha = (st == 0) ? 0.0 : (st == 3 ? h : 0.5 * h);
-            const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
-            const double z = a.zh[li];
-            for (int j = tid; j < nv * a.n_rad; j += SW_CONSUMERS) {
-                const int q = j / a.n_rad, r = j - q * a.n_rad;
-                double sn, cs; sincos(a.eps[r] * z / vel[q], &sn, &cs);
-                ph[j] = {cs, sn};
-            }
-            consumer_sync();
-            // X = P^H (C + alpha * Kn)
-            for (int j = tid; j < nv * N; j += SW_CONSUMERS) {
-                const int q = j / N, col = j - q * N;
-                const cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
-                X[j] = cmulc(x, ph[q * a.n_rad + a.st_rad[col]]);
-            }
-            consumer_sync();
+            const cplx *Xc = X + (size_t)xb * NV * N;
+            cplx acc[NTILE][NV];
+            #pragma unroll
+            for (int t = 0; t < NTILE; ++t)
+                #pragma unroll
+                for (int q = 0; q < NV; ++q) acc[t][q] = cplx{0.0, 0.0};
             for (int c = 0; c < n_chunks; ++c) {
                 const int slot = (int)(g % NS);
                 mbar_wait(&full[slot], (unsigned)((g / NS) & 1));
-                const double *buf = reinterpret_cast<const double *>(ring + (size_t)slot * chunk_bytes);
-                const int r0 = c * rpc, rows = min(rpc, N - r0);
-                for (int r = warp; r < rows; r += 8) {
-                    const double *Dr = buf + (size_t)r * ld;
-                    const int row = r0 + r;
-                    double sr[SWEEP_NV], si[SWEEP_NV];
-                    #pragma unroll
-                    for (int q = 0; q < SWEEP_NV; ++q) { sr[q] = 0.0; si[q] = 0.0; }
-                    for (int col = lane; col < N; col += 32) {
-                        const double d = Dr[col];
+                if (active) {
+                    const double *buf = reinterpret_cast<const double *>(ring + (size_t)slot * chunk_bytes);
+                    const int c0 = c * rpc, rows = min(rpc, N - c0);
+                    #pragma unroll 2
+                    for (int rr = 0; rr < rows; ++rr) {
+                        const double *Dc = buf + (size_t)rr * ld;
+                        cplx xq[NV];
                         #pragma unroll
-                        for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) { const cplx x = X[q * N + col]; sr[q] += d * x.x; si[q] += d * x.y; }
-                    }
-                    #pragma unroll
-                    for (int q = 0; q < SWEEP_NV; ++q) if (q < nv) {
-                        const double yr = warp_sum(sr[q]), yi = warp_sum(si[q]);
-                        if (lane == 0) Kn[q * N + row] = {yr, yi};          // raw y = D x; finished below
+                        for (int q = 0; q < NV; ++q) xq[q] = Xc[(q < nv ? q : 0) * N + c0 + rr];
+                        #pragma unroll
+                        for (int t = 0; t < NTILE; ++t) {
+                            const double d = Dc[min(row[t], N - 1)];
+                            #pragma unroll
+                            for (int q = 0; q < NV; ++q) { acc[t][q].x = fma(d, xq[q].x, acc[t][q].x); acc[t][q].y = fma(d, xq[q].y, acc[t][q].y); }
+                        }
                     }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[slot]);
                 ++g;
             }
-            consumer_sync();
-            // k = -(i/v) P y, accumulate; after the fourth stage the RK4 combination
-            for (int j = tid; j < nv * N; j += SW_CONSUMERS) {
-                const int q = j / N, row = j - q * N;
-                const cplx y = cmul(Kn[j], ph[q * a.n_rad + a.st_rad[row]]);
-                const cplx k = {y.y / vel[q], -y.x / vel[q]};
-                Kn[j] = k;
-                Acc[j].x += wgt * k.x; Acc[j].y += wgt * k.y;
-                if (st == 3) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
+            // k = -(i/v) P y; RK4 accumulation; the next stage's vector goes into the other buffer
+            const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
+            #pragma unroll
+            for (int t = 0; t < NTILE; ++t)
+                #pragma unroll
+                for (int q = 0; q < NV; ++q) {
+                    const cplx y = cmul(acc[t][q], ph[t][q]);
+                    kk[t][q] = cplx{y.y * vinv[q], -y.x * vinv[q]};
+                    Acc[t][q].x += wgt * kk[t][q].x; Acc[t][q].y += wgt * kk[t][q].y;
+                    if (st == 3) { C[t][q].x += (h / 6.0) * Acc[t][q].x; C[t][q].y += (h / 6.0) * Acc[t][q].y; Acc[t][q] = cplx{0.0, 0.0}; }
+                }
+            // stage st + 1 (or stage 0 of the next step): position and alpha
+            const bool last = (st == 3 && s + 1 == a.steps);
+            if (!last) {
+                const int nst = (st + 1) & 3, ns = s + (st == 3);
+                const int li = 2 * ns + (nst == 0 ? 0 : (nst == 3 ? 2 : 1));
+                if (st == 0 || st == 2) phases(a.zh[li]);            // the position changes at z -> z_mid and z_mid -> z_new
+                const double hn = (st == 3) ? 0.0 : h;
+                const double alpha = (nst == 0) ? 0.0 : (nst == 3 ? hn : 0.5 * hn);
+                put_x(X + (size_t)(xb ^ 1) * NV * N, alpha, kk);
             }
-            consumer_sync();
+            xb ^= 1;
+            bar_sync(1, SW1_CONSUMERS);
         }
         if (a.drift) {
-            for (int q = 0; q < nv; ++q) {
+            #pragma unroll
+            for (int q = 0; q < NV; ++q) {
                 double part = 0.0;
-                for (int j = tid; j < N; j += SW_CONSUMERS) part += C[q * N + j].x * C[q * N + j].x + C[q * N + j].y * C[q * N + j].y;
+                #pragma unroll
+                for (int t = 0; t < NTILE; ++t) if (row[t] < N) part += C[t][q].x * C[t][q].x + C[t][q].y * C[t][q].y;
                 part = warp_sum(part);
                 if (lane == 0) red[q][warp] = part;
             }
-            consumer_sync();
-            for (int q = 0; q < nv; ++q) {
+            bar_sync(1, SW1_CONSUMERS);
+            #pragma unroll
+            for (int q = 0; q < NV; ++q) {
                 double tot = 0.0;
-                for (int w = 0; w < 8; ++w) tot += red[q][w];
+                for (int w = 0; w < SW1_CONSUMERS / 32; ++w) tot += red[q][w];
                 drift[q] = fmax(drift[q], fabs(tot - 1.0));
             }
-            consumer_sync();
+            bar_sync(1, SW1_CONSUMERS);
         }
     }
-    for (int q = 0; q < nv; ++q) {
-        for (int j = tid; j < N; j += SW_CONSUMERS) {
-            double *dst = a.C + ((size_t)u.traj[q] * N + j) * 2;
-            dst[0] = C[q * N + j].x; dst[1] = C[q * N + j].y;
+    #pragma unroll
+    for (int q = 0; q < NV; ++q)
+        if (q < nv) {
+            #pragma unroll
+            for (int t = 0; t < NTILE; ++t)
+                if (row[t] < N) { double *dst = a.C + ((size_t)u.traj[q] * N + row[t]) * 2; dst[0] = C[t][q].x; dst[1] = C[t][q].y; }
+            if (a.drift && tid == 0) a.drift[u.traj[q]] = drift[q];
         }
-        if (a.drift && tid == 0) a.drift[u.traj[q]] = drift[q];
-    }
 }
 
 // ------------------------------------------------------------------ a7, large N_P: blocked Gauss-Jordan in global memory
@@ -846,29 +890,47 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
 }
 }  // namespace
 
+// (rows per thread, trajectories per unit) of the one-centre sweep for N states: 224 NTILE >= N, state in registers
+static bool sweep1_shape(int N, int *ntile, int *nv) {
+    static const int shapes[][3] = {{224, 1, 4}, {448, 2, 4}, {672, 3, 3}, {896, 4, 2}, {1344, 6, 1}, {2016, 9, 1}, {3136, 14, 1}};
+    for (auto &sh : shapes) if (N <= sh[0]) { *ntile = sh[1]; *nv = sh[2]; return true; }
+    return false;
+}
+
 void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages) {
-    // ring of `stages` chunks of whole rows + 4 nv N + nv n_rad complex numbers within the 227 KB of a CTA;
-    // preferred: 8 rows per chunk (one per consumer warp), 3-4 stages, as many trajectories per unit as fit
+    (void)n_rad;
+    int ntile = 1;
+    if (!sweep1_shape(N, &ntile, nv)) { *nv = 1; *rows_per_chunk = 1; *stages = 2; return; }      // wp_sweep_one_centre reports the limit
+    // ring of whole rows (about 16 KB per chunk, 4 stages) + the double-buffered stage vectors within the 227 KB of a CTA
     const int ld = wp_sweep1_ld(N);
-    const size_t cap = 226 * 1024;
-    auto bytes = [&](int vv, int rr, int ss) { return (size_t)ss * rr * ld * 8 + ((size_t)4 * vv * N + (size_t)vv * n_rad) * 16; };
-    for (int v = SWEEP_NV; v >= 1; --v)
-        for (int rr : {16, 8})
-            for (int ss : {4, 3})
-                if (bytes(v, rr, ss) <= cap && (v >= 3 || rr == 8)) { *nv = v; *rows_per_chunk = rr; *stages = ss; return; }
-    int v = 1, rr = 8, ss = 2;
-    while (rr > 1 && bytes(v, rr, ss) > cap) --rr;
-    *nv = v; *rows_per_chunk = rr; *stages = ss;
+    const size_t cap = 220 * 1024, vec = (size_t)2 * *nv * N * 16;
+    int rr = std::max(1, std::min(16, (int)(16384 / ((size_t)ld * 8)))), ss = 4;
+    while (ss > 2 && (size_t)ss * rr * ld * 8 + vec > cap) --ss;
+    while (rr > 1 && (size_t)ss * rr * ld * 8 + vec > cap) --rr;
+    *rows_per_chunk = rr; *stages = ss;
 }
 
 int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s) {
     if (n_units <= 0 || a.steps <= 0) return 0;
-    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + ((size_t)4 * a.nv * a.N + (size_t)a.nv * a.n_rad) * 16;
+    int ntile = 0, nvs = 0;
+    if (!sweep1_shape(a.N, &ntile, &nvs)) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d exceeds the register-resident design (N <= 3136)", a.N);
+    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + (size_t)2 * nvs * a.N * 16;
     if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
     static PerDevice attr_1;
-    if (wp_raise(attr_1, smem)) WP_CUDA(cudaFuncSetAttribute(k_sweep1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool raise = wp_raise(attr_1, smem);
     wp_span_begin(B, FAM_SWEEP, s);
-    k_sweep1<<<n_units, SW_CONSUMERS + 32, smem, s>>>(a);
+#define WP_SWEEP1(NT_, NV_) do { if (raise) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
+        k_sweep1<NT_, NV_><<<n_units, SW1_CONSUMERS + 32, smem, s>>>(a); } while (0)
+    switch (ntile) {
+        case 1: WP_SWEEP1(1, 4); break;
+        case 2: WP_SWEEP1(2, 4); break;
+        case 3: WP_SWEEP1(3, 3); break;
+        case 4: WP_SWEEP1(4, 2); break;
+        case 6: WP_SWEEP1(6, 1); break;
+        case 9: WP_SWEEP1(9, 1); break;
+        default: WP_SWEEP1(14, 1); break;
+    }
+#undef WP_SWEEP1
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;

@@ -837,14 +837,32 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
 // ---------------------------------------------------------------------------------------------------- host side
 struct TransferPlan {
     PosTabs L; int nq8[2], ntile[2]; size_t stride[2]; size_t part_per_pos; int n_split; std::vector<int2> tiles;
-    size_t per_pos_bytes() const { return ((size_t)L.size() + stride[0] + stride[1]) * 8 + part_per_pos * 8 + 64; }
+    size_t wd_stride = 0;                    // spheroidal rule: doubles of weights W_d(i,k) per position
+    size_t per_pos_bytes() const { return ((size_t)L.size() + stride[0] + stride[1] + wd_stride) * 8 + part_per_pos * 8 + 64; }
 };
+
+// Columns (a, q >= 0) of a centre, grouped by q.  pad8 (spheroidal rule): every q-group starts at a multiple of 8, so that
+// an 8-column block of the contraction has a single q.  Returns the padded column count (a multiple of 8).
+static int column_map(const CentreTab &C, bool pad8, std::vector<int> *col_of /*[n_rad][WP_MAX_L+1] or null*/, std::vector<int> *q_of /*[cols] or null*/) {
+    int col = 0;
+    if (col_of) col_of->assign((size_t)C.n_rad * (WP_MAX_L + 1), -1);
+    std::vector<int> q;
+    for (int qq = 0; qq <= C.l_max; ++qq) {
+        if (pad8) while (col & 7) { q.push_back(-1); ++col; }
+        for (int a = 0; a < C.n_rad; ++a) if (C.l[a] >= qq) { if (col_of) (*col_of)[(size_t)a * (WP_MAX_L + 1) + qq] = col; q.push_back(qq); ++col; }
+    }
+    while (col & 7) { q.push_back(-1); ++col; }
+    if (q_of) *q_of = q;
+    return col;
+}
 
 static TransferPlan make_plan(const wpccc_basis *B, int n_split) {
     TransferPlan P;
+    const bool sph = B->quad.kind == 1;
     P.L.n_rho = B->quad.n_rho; P.L.n_z = B->quad.n_z; P.L.n_phi = B->quad.n_phi; P.L.dmax = B->c[0].l_max + B->c[1].l_max;
+    if (sph) P.wd_stride = (size_t)P.L.n_rho * P.L.n_z * (P.L.dmax + 1) * 2;
     for (int s = 0; s < 2; ++s) {
-        P.nq8[s] = B->c[s].nqc_pad;
+        P.nq8[s] = column_map(B->c[s], sph, nullptr, nullptr);
         P.ntile[s] = (2 * P.nq8[s] + 63) / 64;
         P.stride[s] = (size_t)P.ntile[s] * 64 * P.L.n_rho * P.L.n_z;
     }
@@ -859,6 +877,7 @@ static TransferPlan make_plan(const wpccc_basis *B, int n_split) {
 // Ring splits (split-K of the contraction) as a function of the positions per launch: none once a launch has two
 // waves of CTAs on the 148 SMs; for a handful of positions (wpccc_matrix_elements) enough to occupy the GPU.
 static int pick_split(const wpccc_basis *B, int chunk) {
+    if (B->quad.kind == 1) return 1;
     TransferPlan P = make_plan(B, 1);
     const long long ctas = (long long)P.tiles.size() * std::max(chunk, 1);
     int s = (int)std::min<long long>((296 + ctas - 1) / ctas, std::max(1, B->quad.n_rho / 4));
@@ -869,7 +888,7 @@ size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk) {
     TransferPlan P = make_plan(B, pick_split(B, n_pos_chunk));
     return P.per_pos_bytes() * (size_t)n_pos_chunk + P.tiles.size() * sizeof(int2) + 4096 +
            2 * (size_t)(B->c[0].n_rad + B->c[1].n_rad) * (WP_MAX_L + 1) * sizeof(int) +
-           2 * (size_t)(B->c[0].nqc_pad + B->c[1].nqc_pad) * sizeof(int) +
+           2 * (size_t)(P.nq8[0] + P.nq8[1]) * sizeof(int) +
            (size_t)B->c[1].n_rad * (sizeof(TrotChunk) + sizeof(int)) + 1024;
 }
 
@@ -893,7 +912,7 @@ size_t wp_transfer_stash_doubles(const wpccc_basis *B) { return make_plan(B, 1).
 static size_t dual_smem_bytes(const TransferPlan &P) {
     return ((size_t)2 * TcRing<true>::STAGES * TcRing<true>::STAGE_DOUBLES + TcRing<true>::ACC_DOUBLES + 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho) * 8;
 }
-bool wp_transfer_mirror_ok(const wpccc_basis *B) { return dual_smem_bytes(make_plan(B, 1)) <= 226 * 1024; }
+bool wp_transfer_mirror_ok(const wpccc_basis *B) { return B->quad.kind == 0 && dual_smem_bytes(make_plan(B, 1)) <= 226 * 1024; }
 
 int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
                 const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s,
@@ -928,9 +947,11 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     double *d_pos = (double *)take((size_t)chunk * P.L.size() * 8);
     double *d_tab[2] = {(double *)take((size_t)chunk * P.stride[0] * 8), (double *)take((size_t)chunk * P.stride[1] * 8)};
     double *d_part = (double *)take((size_t)chunk * P.part_per_pos * 8);
+    const bool sph = B->quad.kind == 1;
+    double *d_wd = sph ? (double *)take((size_t)chunk * P.wd_stride * 8) : nullptr;
     int2 *d_tiles = (int2 *)take(P.tiles.size() * sizeof(int2));
     int *d_colidx[2], *d_qcol[2];
-    for (int c = 0; c < 2; ++c) { d_colidx[c] = (int *)take((size_t)B->c[c].n_rad * (WP_MAX_L + 1) * 4); d_qcol[c] = (int *)take((size_t)B->c[c].nqc_pad * 4); }
+    for (int c = 0; c < 2; ++c) { d_colidx[c] = (int *)take((size_t)B->c[c].n_rad * (WP_MAX_L + 1) * 4); d_qcol[c] = (int *)take((size_t)P.nq8[c] * 4); }
     // rotation chunks: consecutive projectile radial functions whose body rows (both families) fit ~48 KB of shared memory
     const int lmx = std::max(B->c[0].l_max, B->c[1].l_max);
     const size_t rot_nd = (((size_t)(lmx + 1) * (2 * lmx + 1) * (2 * lmx + 1) + 1) & ~(size_t)1) * 8;
@@ -968,10 +989,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     WP_CUDA(cudaMemcpyAsync(d_tiles, P.tiles.data(), P.tiles.size() * sizeof(int2), cudaMemcpyHostToDevice, s));
     std::vector<int> hcol[2], hq[2];
     for (int c = 0; c < 2; ++c) {
-        const CentreTab &C = B->c[c];
-        hcol[c].assign((size_t)C.n_rad * (WP_MAX_L + 1), -1);
-        hq[c].assign(C.nqc_pad, -1);
-        for (int col = 0; col < C.nqc; ++col) { hcol[c][(size_t)C.col_rad[col] * (WP_MAX_L + 1) + C.col_q[col]] = col; hq[c][col] = C.col_q[col]; }
+        column_map(B->c[c], sph, &hcol[c], &hq[c]);
         WP_CUDA(cudaMemcpyAsync(d_colidx[c], hcol[c].data(), hcol[c].size() * 4, cudaMemcpyHostToDevice, s));
         WP_CUDA(cudaMemcpyAsync(d_qcol[c], hq[c].data(), hq[c].size() * 4, cudaMemcpyHostToDevice, s));
     }
@@ -984,11 +1002,17 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     const size_t con_tabs = 2 * P.L.n_z + 2 * (size_t)(P.L.dmax + 2) * P.L.n_rho;
     const size_t con_smem = ((size_t)2 * TcRing<false>::STAGES * TcRing<false>::STAGE_DOUBLES + con_tabs) * 8;
     const size_t dual_smem = dual_smem_bytes(P);
-    if (con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
+    if (!sph && con_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: quadrature too large for the contraction kernel's shared memory");
+    // spheroidal contraction: ring of operand stages + the weights of each stage
+    const int sph_nd = P.L.dmax + 1;
+    const int sph_stages = (3 * ((size_t)2 * TS_STAGE_DOUBLES * 8 + (size_t)TS_KCS * sph_nd * 64) <= 226 * 1024) ? 3 : 2;
+    const size_t sph_smem = (size_t)sph_stages * ((size_t)2 * TS_STAGE_DOUBLES * 8 + (size_t)TS_KCS * sph_nd * 64);
+    static PerDevice sph_attr;
+    if (sph && wp_raise(sph_attr, sph_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon_sph, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sph_smem));
     // mirror-pair kernel: whenever some evaluated position of this window has a stash slot
     const bool dual = sel && sel->stash && sel->n_st > 0 && sel->i0 < sel->i_mid && sel->i0 + sel->n_pre > sel->i_mid - sel->n_st;
     if (dual && dual_smem > 226 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: mirror stash requested but the pair kernel does not fit shared memory");
-    if (wp_raise(con_attr, con_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
+    if (!sph && wp_raise(con_attr, con_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)con_smem));
     if (dual && wp_raise(dual_attr, dual_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dual_smem));
 
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
@@ -1005,8 +1029,12 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         ta.gl_rho = B->d_gl_rho; ta.gl_phi = B->d_gl_phi; ta.gl_zq = B->d_gl_zq; ta.gl_zh = B->d_gl_zh;
         ta.rho_max = B->quad.rho_max; ta.z_pad = B->quad.z_pad; ta.phi_rule = B->quad.phi_rule; ta.out = d_pos;
         wp_span_begin(B, FAM_TTAB, s);
-        k_tpos<<<np, 128, 0, s>>>(ta);
-        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R; tb.sel = sd; tb.q0 = p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC;
+        if (sph) {
+            TsphArgs ts{}; ts.L = P.L; ts.R = d_R; ts.cosT = d_cos; ts.sinT = d_sin; ts.v = d_v; ts.gl_eta = B->d_gl_rho; ts.gl_tau = B->d_gl_zh;
+            ts.eta_scale = B->quad.eta_scale; ts.out = d_pos; ts.wd = d_wd; ts.wd_stride = P.wd_stride; ts.q0 = p0;
+            k_tpos_sph<<<dim3(P.L.n_rho, np), std::min(256, (P.L.n_z + 31) / 32 * 32), 0, s>>>(ts);
+        } else k_tpos<<<np, 128, 0, s>>>(ta);
+        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R; tb.sel = sd; tb.q0 = p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC; tb.sph = sph;
         for (int c = 0; c < 2; ++c) {
             tb.Ut[c] = B->c[c].d_Ut; tb.lrad[c] = B->c[c].d_l; tb.n_rad[c] = B->c[c].n_rad; tb.nf_pad[c] = B->c[c].nf_pad;
             tb.nq8[c] = P.nq8[c]; tb.ntile[c] = P.ntile[c]; tb.colidx[c] = d_colidx[c]; tb.out[c] = d_tab[c]; tb.pos_stride[c] = P.stride[c];
@@ -1026,7 +1054,12 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         if (dual) { tc.n_st = sel->n_st; tc.i0 = sel->i0; tc.i_mid = sel->i_mid; tc.stash = sel->stash; }
         dim3 gc((unsigned)P.tiles.size(), n_split, np);
         wp_span_begin(B, FAM_TCON, s);
-        if (dual) k_tcon<4, true><<<gc, 256, dual_smem, s>>>(tc);
+        if (sph) {
+            TconSphArgs th{}; th.L = P.L; th.tabT = d_tab[0]; th.tabP = d_tab[1]; th.strideT = P.stride[0]; th.strideP = P.stride[1];
+            th.wd = d_wd; th.wd_stride = P.wd_stride; th.nq8T = P.nq8[0]; th.nq8P = P.nq8[1]; th.qT = d_qcol[0]; th.qP = d_qcol[1];
+            th.tiles = d_tiles; th.part = d_part; th.stages = sph_stages;
+            k_tcon_sph<<<gc, 256, sph_smem, s>>>(th);
+        } else if (dual) k_tcon<4, true><<<gc, 256, dual_smem, s>>>(tc);
         else k_tcon<4, false><<<gc, 256, con_smem, s>>>(tc);
         wp_span_end(B, s, 1);
         B->units[FAM_TCON] += np;

@@ -300,3 +300,26 @@ def test_workspace_query_is_sufficient_for_a_first_call(lib):
             out = lib.matrix_elements(basis, [0.8, 1.1, 0.3], [-0.6, 0.2, 1.4], [1.2, 1.2, 0.9], **kw)
             assert all(t is None or bool(t.isfinite().all()) for t in out)
             basis.close()
+
+
+def test_paper_zgrid_propagation(lib, one_centre, two_centre):
+    """wpccc_propagate_grid on the z-grid of PAPER.md L67 (geometric, symmetric about 0, step sizes
+    from 1e-3 to ~1) against Algorithm 1 on the same grid (oracle/zgrid.py), one and two centres; windows of 64 steps,
+    mirror pairs on the symmetric grid."""
+    from oracle import zgrid
+    g = zgrid.paper_zgrid(1e-3, 9.0, 70)                                   # 141 points, 140 steps: three windows
+    for (prob, basis), b, v in ((one_centre, np.array([0.6, 2.0, 0.6]), np.array([1.0, 2.0, 0.7])),
+                                (two_centre, np.array([1.6, 1.1]), np.array([0.9, 1.4]))):
+        Cg, drift = lib.propagate_grid(basis, b, v, g, track_norm=True)
+        Cg, drift = Cg.cpu().numpy(), drift.cpu().numpy()
+        for t in range(len(b)):
+            co, do = zgrid.propagate_grid(prob, b[t], v[t], g, track_norm=True)
+            assert np.abs(Cg[t] - co).max() < PTOL, (t, np.abs(Cg[t] - co).max())
+            assert abs(drift[t] - do) < 1e-10 + 1e-4 * do
+    if True:                                                               # continuation: two calls = one call
+        prob, basis = two_centre
+        b, v = np.array([1.6, 1.1]), np.array([0.9, 1.4])
+        C1 = lib.propagate(basis, b, v, -8.0, 8.0, 40).cpu().numpy()
+        Ca = lib.propagate(basis, b, v, -8.0, -1.6, 16)
+        Cb = lib.propagate(basis, b, v, -1.6, 8.0, 24, C0=Ca).cpu().numpy()
+        assert np.abs(Cb - C1).max() < 1e-12
