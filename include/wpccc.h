@@ -210,6 +210,19 @@ int wpccc_propagate_grid(const wpccc_basis *basis, int n_traj, const double *b /
  * 1 zero pivot, 2 |S_PT| >= 1, 3 not positive definite.  Half-step index i: z = z_min + i h / 2 on the uniform grid. */
 int wpccc_last_status(const wpccc_basis *basis, int n_traj, int *traj_status /*[host]*/);
 
+/* ---- eq. (4) as the paper solves it: the explicit matrix M ---------------
+ * M = -(i/v) S^{-1} H at each position, i.e. the overlap system solved for the N_tot right-hand sides that are the
+ * columns of H -- what the paper's ZGESV call produces (Fig. 3 measures its share of the run).  The hot path
+ * (wpccc_propagate) never forms M (A14); this entry point exists for the like-for-like comparison of the solver cost and
+ * for callers who want M itself.  Route: Schur complement A = I - K K^H, its inverse by Gauss-Jordan elimination with
+ * partial pivoting, then three batched complex matrix products (Y_P -= K Y_T; W_P = A^{-1} Y_P; W_T = Y_T - K^H W_P).
+ * flags bit 0: interaction-picture phases e^{i (eps_row - eps_col) z / v} (A2).  dM [device][n_pos][N_tot][N_tot] complex.
+ * One centre: M = -(i/v) D^T (eq. (5)).  Synchronises `stream`; WPCCC_ESINGULAR names a position with a zero pivot. */
+size_t wpccc_coupling_matrix_ws_bytes(const wpccc_basis *basis, int n_pos);
+int wpccc_coupling_matrix(const wpccc_basis *basis, int n_pos, const double *b /*[host]*/, const double *z /*[host]*/,
+                          const double *v /*[host]*/, int flags, double *dM /*[device]*/,
+                          void *ws /*[device]*/, size_t ws_bytes, void *stream);
+
 /* ---- a9: observables ------------------------------------------------------------------
  * From amplitudes dC [device, n_traj][N_tot] complex:
  *   P_state [n_traj][N_tot]       |c_j|^2

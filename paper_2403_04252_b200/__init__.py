@@ -73,6 +73,10 @@ _lib.wpccc_last_status.restype = C.c_int
 _lib.wpccc_last_status.argtypes = [_vp, C.c_int, _ip]
 _lib.wpccc_set_option.restype = C.c_int
 _lib.wpccc_set_option.argtypes = [_vp, C.c_char_p, C.c_longlong]
+_lib.wpccc_coupling_matrix_ws_bytes.restype = C.c_size_t
+_lib.wpccc_coupling_matrix_ws_bytes.argtypes = [_vp, C.c_int]
+_lib.wpccc_coupling_matrix.restype = C.c_int
+_lib.wpccc_coupling_matrix.argtypes = [_vp, C.c_int, _dp, _dp, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
 _lib.wpccc_probabilities.restype = C.c_int
 _lib.wpccc_probabilities.argtypes = [_vp, C.c_int, _vp, _dp, _ip, C.c_int, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.wpccc_last_timing.restype = C.c_int
@@ -90,7 +94,7 @@ _lib.wpccc_version.restype = C.c_char_p
 
 EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
-           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
+           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_coupling_matrix_ws_bytes", "wpccc_coupling_matrix", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
            "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
 
 
@@ -245,6 +249,19 @@ def matrix_elements(basis: Basis, b, z, v, phases: bool = True, want_S: bool = T
     _check(_lib.wpccc_matrix_elements(basis._h, n, _ptr(b), _ptr(z), _ptr(v), (1 if phases else 0) | (2 if want_F else 0),
                                       p(S), p(H), p(F), ws, min(cap, need), _stream(torch)))
     return (S, H, F) if want_F else (S, H)
+
+
+def coupling_matrix(basis: Basis, b, z, v, phases: bool = True):
+    """wpccc_coupling_matrix: the explicit M = -(i/v) S^{-1} H of eq. (4) [n_pos, N, N] complex128 on the device."""
+    torch = _torch()
+    b, z, v = _f64(np.atleast_1d(b)), _f64(np.atleast_1d(z)), _f64(np.atleast_1d(v))
+    n, N = len(b), basis.n_tot
+    M = torch.empty((n, N, N), dtype=torch.complex128, device="cuda")
+    need = _lib.wpccc_coupling_matrix_ws_bytes(basis._h, max(n, 1))
+    ws, cap = basis.workspace(need)
+    _check(_lib.wpccc_coupling_matrix(basis._h, n, _ptr(b), _ptr(z), _ptr(v), 1 if phases else 0, C.c_void_p(M.data_ptr()), ws, min(cap, need),
+                                      _stream(torch)))
+    return M
 
 
 def _propagate_common(basis, b, v, n_steps, init_state, track_norm, ws_bytes, C0, drift0, allow_singular, call):

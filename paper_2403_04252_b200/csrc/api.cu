@@ -7,6 +7,7 @@
 
 #include "common.cuh"
 #include "sweep.cuh"
+#include "ptx.cuh"
 
 namespace {
 
@@ -315,6 +316,8 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
                 units.push_back(u);
             }
     }
+    int nv_max = 1;
+    for (auto &u : units) nv_max = std::max(nv_max, u.n);
     const int n_groups = two ? n_traj : (int)ub.size();
     PropPlan P = plan_propagate(B, n_traj, n_groups, (int)units.size(), n_steps);
     if (ws_bytes < plan_bytes(P, 1)) WP_FAIL(WPCCC_ENOMEM, "workspace too small: need at least %zu bytes", plan_bytes(P, 1));
@@ -417,7 +420,7 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
         } else {
             Sweep1Args a{};
             a.units = d_units; a.D = d_D[buf]; a.st_rad = B->c[0].d_st_rad; a.eps = B->c[0].d_eps; a.v = d_v; a.C = dC; a.drift = d_norm_drift;
-            a.N = N; a.n_rad = B->c[0].n_rad; a.n_idx = n_idx; a.ldD = ldD; a.nv = nv; a.rows_per_chunk = rows_per_chunk; a.ring_stages = ring_stages; a.steps = steps;
+            a.N = N; a.n_rad = B->c[0].n_rad; a.n_idx = n_idx; a.ldD = ldD; a.nv = nv_max; a.rows_per_chunk = rows_per_chunk; a.ring_stages = ring_stages; a.steps = steps;
             a.zh = d_zh + i0; a.hs = d_hs + s0;
             rc = wp_sweep_one_centre(B, (int)units.size(), a, sw);
         }
@@ -479,6 +482,156 @@ extern "C" int wpccc_propagate_grid(const wpccc_basis *Bc, int n_traj, const dou
     }
     zh[2 * (size_t)n_steps] = zgrid[n_steps];
     return propagate_impl(const_cast<wpccc_basis *>(Bc), n_traj, b, v, n_steps, zh, hs, init_state, dC, d_norm_drift, ws, ws_bytes, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------- explicit M (eq. (4))
+namespace {
+
+// Batched complex product C (+)= sign * op(A) B:  C [m][n] (ldc), B [k][n] (ldb) row-major;  TRANS: op(A) = A^H with A [k][m] (lda),
+// else A [m][k] (lda).  ACC: C += sign * ..., else C = sign * ....  grid = (n tiles, m tiles, positions), block 16 x 16, thread tile 2 x 2.
+struct ZgemmArgs { const cplx *A, *B; cplx *C; size_t a_stride, b_stride, c_stride; int m, n, k, lda, ldb, ldc; double sign; };
+template <bool TRANS, bool ACC>
+__global__ void __launch_bounds__(256) k_zgemm(const ZgemmArgs a) {
+    __shared__ cplx sA[32][17], sB[16][33];                        // [m][k], [k][n]
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4, m0 = blockIdx.y * 32, n0 = blockIdx.x * 32;
+    const cplx *A = a.A + (size_t)blockIdx.z * a.a_stride, *Bm = a.B + (size_t)blockIdx.z * a.b_stride;
+    cplx *C = a.C + (size_t)blockIdx.z * a.c_stride;
+    cplx acc[2][2] = {{{0.0, 0.0}, {0.0, 0.0}}, {{0.0, 0.0}, {0.0, 0.0}}};
+    for (int k0 = 0; k0 < a.k; k0 += 16) {
+        for (int e = threadIdx.x; e < 32 * 16; e += 256) {
+            int mi, ki;
+            if (TRANS) { mi = e & 31; ki = e >> 5; } else { ki = e & 15; mi = e >> 4; }     // consecutive threads along the contiguous index
+            cplx v = {0.0, 0.0};
+            if (m0 + mi < a.m && k0 + ki < a.k) {
+                if (TRANS) { v = A[(size_t)(k0 + ki) * a.lda + m0 + mi]; v.y = -v.y; } else v = A[(size_t)(m0 + mi) * a.lda + k0 + ki];
+            }
+            sA[mi][ki] = v;
+            const int kb = e >> 5, nb = e & 31;
+            sB[kb][nb] = (k0 + kb < a.k && n0 + nb < a.n) ? Bm[(size_t)(k0 + kb) * a.ldb + n0 + nb] : cplx{0.0, 0.0};
+        }
+        __syncthreads();
+        #pragma unroll
+        for (int kk = 0; kk < 16; ++kk) {
+            const cplx a0 = sA[ty][kk], a1 = sA[ty + 16][kk], b0 = sB[kk][tx], b1 = sB[kk][tx + 16];
+            acc[0][0].x += a0.x * b0.x - a0.y * b0.y; acc[0][0].y += a0.x * b0.y + a0.y * b0.x;
+            acc[0][1].x += a0.x * b1.x - a0.y * b1.y; acc[0][1].y += a0.x * b1.y + a0.y * b1.x;
+            acc[1][0].x += a1.x * b0.x - a1.y * b0.y; acc[1][0].y += a1.x * b0.y + a1.y * b0.x;
+            acc[1][1].x += a1.x * b1.x - a1.y * b1.y; acc[1][1].y += a1.x * b1.y + a1.y * b1.x;
+        }
+        __syncthreads();
+    }
+    #pragma unroll
+    for (int i = 0; i < 2; ++i)
+        #pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int r = m0 + ty + 16 * i, c = n0 + tx + 16 * j;
+            if (r < a.m && c < a.n) {
+                cplx *d = C + (size_t)r * a.ldc + c;
+                const cplx o = ACC ? *d : cplx{0.0, 0.0};
+                *d = cplx{o.x + a.sign * acc[i][j].x, o.y + a.sign * acc[i][j].y};
+            }
+        }
+}
+
+// M[i][j] = -(i/v) e^{i (eps_i - eps_j) z / v} W[i][j],  W rows of centre T in M itself, rows of centre P in Wp
+struct MFinalArgs { double *M; const double *Wp; const double *z, *v; const int *st_rad_T, *st_rad_P; const double *eps_T, *eps_P; int NT, NP, phases; };
+__global__ void k_m_final(const MFinalArgs a) {
+    const int p = blockIdx.x, N = a.NT + a.NP;
+    const double t = a.z[p] / a.v[p], vinv = 1.0 / a.v[p];
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < N * N; e += gridDim.y * blockDim.x) {
+        const int i = e / N, j = e % N;
+        double pr = 1.0, pi = 0.0;
+        if (a.phases) {
+            const double ei = (i < a.NT) ? a.eps_T[a.st_rad_T[i]] : a.eps_P[a.st_rad_P[i - a.NT]];
+            const double ej = (j < a.NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - a.NT]];
+            sincos((ei - ej) * t, &pi, &pr);
+        }
+        const double *w = (i < a.NT || !a.Wp) ? a.M + ((size_t)p * N * N + e) * 2 : a.Wp + (((size_t)p * a.NP + (i - a.NT)) * N + j) * 2;
+        const double wr = w[0] * pr - w[1] * pi, wi = w[0] * pi + w[1] * pr;
+        double *o = a.M + ((size_t)p * N * N + e) * 2;
+        o[0] = wi * vinv; o[1] = -wr * vinv;                   // -(i/v) (wr + i wi)
+    }
+}
+
+}  // namespace
+
+extern "C" size_t wpccc_coupling_matrix_ws_bytes(const wpccc_basis *B, int n_pos) {
+    if (!B || n_pos < 1) return 0;
+    const size_t N = B->n_tot, NT = B->c[0].n_states, NP = B->n_centres == 2 ? B->c[1].n_states : 0;
+    size_t per = 9 * 8 + (size_t)B->E_tot * 8 + 64 + 8;
+    if (NP) per += NP * NT * 16 + wp_factor_elems((int)NP) * 16 + NP * N * 16 + NP * NP * 16;
+    size_t tot = per * (size_t)n_pos + 65536;
+    if (NP) tot += align256(wp_transfer_ws_bytes(B, std::min(n_pos, wp_transfer_default_chunk(B))));
+    return tot;
+}
+
+extern "C" int wpccc_coupling_matrix(const wpccc_basis *Bc, int n_pos, const double *b, const double *z, const double *v, int flags,
+                                     double *dM, void *ws, size_t ws_bytes, void *stream) {
+    if (!Bc || !dM) WP_FAIL(WPCCC_EINVAL, "basis or dM is NULL");
+    wpccc_basis *B = const_cast<wpccc_basis *>(Bc);
+    if (n_pos < 0 || (n_pos > 0 && (!b || !z || !v))) WP_FAIL(WPCCC_EINVAL, "n_pos < 0 or position arrays NULL");
+    if (n_pos == 0) return 0;
+    if (!ws || ws_bytes < wpccc_coupling_matrix_ws_bytes(B, n_pos)) WP_FAIL(WPCCC_ENOMEM, "workspace too small: need %zu bytes", wpccc_coupling_matrix_ws_bytes(B, n_pos));
+    for (int p = 0; p < n_pos; ++p)
+        if (!(v[p] > 0.0) || !(b[p] >= 0.0) || !(b[p] * b[p] + z[p] * z[p] > 0.0)) WP_FAIL(WPCCC_EINVAL, "position %d: need v > 0, b >= 0 and R > 0", p);
+    cudaStream_t s = (cudaStream_t)stream;
+    wp_timing_reset(B);
+    B->tab_zeroed = nullptr;
+    const bool two = B->n_centres == 2;
+    const int NT = B->c[0].n_states, NP = two ? B->c[1].n_states : 0, N = NT + NP;
+    Carver cv(ws, ws_bytes);
+    const int tchunk = two ? wp_transfer_default_chunk(B) : 0;
+    const size_t tws_bytes = two ? align256(wp_transfer_ws_bytes(B, std::min(n_pos, tchunk))) : 0;
+    void *tws = two ? cv.take<char>(tws_bytes) : nullptr;
+    double *d_b = cv.take<double>(n_pos), *d_z = cv.take<double>(n_pos), *d_v = cv.take<double>(n_pos);
+    GeomOut g = carve_geom(cv, n_pos);
+    double *d_F = cv.take<double>((size_t)n_pos * B->E_tot);
+    double *d_K = two ? cv.take<double>((size_t)n_pos * NP * NT * 2) : nullptr;
+    double *d_A = two ? cv.take<double>((size_t)n_pos * wp_factor_elems(NP) * 2) : nullptr;
+    double *d_W = two ? cv.take<double>((size_t)n_pos * NP * N * 2) : nullptr;
+    void *d_fs = two ? cv.take<char>(wp_factor_scratch_bytes(B, n_pos)) : nullptr;
+    int *d_flags = cv.take<int>(n_pos);
+    if (!cv.ok) WP_FAIL(WPCCC_ENOMEM, "workspace too small (internal plan mismatch)");
+    WP_CUDA(cudaMemcpyAsync(d_b, b, n_pos * sizeof(double), cudaMemcpyHostToDevice, s));
+    WP_CUDA(cudaMemcpyAsync(d_z, z, n_pos * sizeof(double), cudaMemcpyHostToDevice, s));
+    WP_CUDA(cudaMemcpyAsync(d_v, v, n_pos * sizeof(double), cudaMemcpyHostToDevice, s));
+    k_geometry_list<<<(n_pos + 127) / 128, 128, 0, s>>>(n_pos, d_b, d_z, d_v, g);
+    int rc;
+    WP_CUDA(cudaMemsetAsync(d_flags, 0, (size_t)n_pos * sizeof(int), s));
+    if (two) {
+        WP_CUDA(cudaMemsetAsync(dM, 0, (size_t)n_pos * N * N * 16, s));
+        rc = elements_two_centre(B, n_pos, g, d_F, d_K, dM, tws, tws_bytes, tchunk, s); if (rc) return rc;
+        // the N right-hand sides of eq. (4) need A^{-1} applied to a matrix: the explicit-inverse route, whatever "solve_route" says
+        const int keep = B->opt.solve_route; B->opt.solve_route = 1;
+        rc = wp_factor(B, n_pos, d_K, d_A, d_flags, d_fs, s);
+        B->opt.solve_route = keep;
+        if (rc) return rc;
+        wp_span_begin(B, FAM_FACT, s);
+        const size_t sN = (size_t)N * N, sK = (size_t)NP * NT, sA = wp_factor_elems(NP), sW = (size_t)NP * N;
+        cplx *M = reinterpret_cast<cplx *>(dM), *K = reinterpret_cast<cplx *>(d_K), *A = reinterpret_cast<cplx *>(d_A), *W = reinterpret_cast<cplx *>(d_W);
+        for (int p0 = 0; p0 < n_pos; p0 += 32768) {
+            const int np = std::min(32768, n_pos - p0);
+            ZgemmArgs g1{K + p0 * sK, M + p0 * sN, M + p0 * sN + (size_t)NT * N, sK, sN, sN, NP, N, NT, NT, N, N, -1.0};           // Y_P -= K Y_T
+            k_zgemm<false, true><<<dim3((N + 31) / 32, (NP + 31) / 32, np), 256, 0, s>>>(g1);
+            ZgemmArgs g2{A + p0 * sA, M + p0 * sN + (size_t)NT * N, W + p0 * sW, sA, sN, sW, NP, N, NP, NP, N, N, 1.0};            // W_P = A^{-1} Y_P
+            k_zgemm<false, false><<<dim3((N + 31) / 32, (NP + 31) / 32, np), 256, 0, s>>>(g2);
+            ZgemmArgs g3{K + p0 * sK, W + p0 * sW, M + p0 * sN, sK, sW, sN, NT, N, NP, NT, N, N, -1.0};                            // W_T = Y_T - K^H W_P
+            k_zgemm<true, true><<<dim3((N + 31) / 32, (NT + 31) / 32, np), 256, 0, s>>>(g3);
+        }
+        wp_span_end(B, s, 3);
+    } else {
+        rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, s);
+        if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, dM, N, (long long)N * N, 1, s);
+        if (rc) return rc;
+    }
+    MFinalArgs f{dM, d_W, g.z, g.v, B->c[0].d_st_rad, two ? B->c[1].d_st_rad : nullptr, B->c[0].d_eps, two ? B->c[1].d_eps : nullptr, NT, NP, flags & 1};
+    k_m_final<<<dim3(n_pos, std::min(64, (N * N + 255) / 256)), 256, 0, s>>>(f);
+    WP_CUDA(cudaGetLastError());
+    std::vector<int> hf(n_pos, 0);
+    WP_CUDA(cudaMemcpyAsync(hf.data(), d_flags, n_pos * sizeof(int), cudaMemcpyDeviceToHost, s));
+    WP_CUDA(cudaStreamSynchronize(s));
+    for (int p = 0; p < n_pos; ++p) if (hf[p]) WP_FAIL(WPCCC_ESINGULAR, "overlap system singular at position %d (code %d)", p, hf[p]);
+    return 0;
 }
 
 extern "C" int wpccc_last_status(const wpccc_basis *B, int n_traj, int *traj_status) {

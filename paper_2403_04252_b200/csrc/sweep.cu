@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
         return;
     }
     // ---------------- consumers: thread tid owns rows tid + 224 t
-    int row[NTILE]; double eov[NTILE][NV];                  // eps of the row's radial function / v of the trajectory
+    int row[NTILE], rowc[NTILE]; double eov[NTILE][NV];     // eps of the row's radial function / v of the trajectory
     cplx C[NTILE][NV], Acc[NTILE][NV], ph[NTILE][NV];
     double vinv[NV];
     #pragma unroll
@@ -79,6 +79,7 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
     for (int t = 0; t < NTILE; ++t) {
         row[t] = tid + SW1_CONSUMERS * t;
         const int rc = min(row[t], N - 1);
+        rowc[t] = rc;
         const double e = a.eps[a.st_rad[rc]];
         #pragma unroll
         for (int q = 0; q < NV; ++q) {
@@ -122,42 +123,57 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
         #pragma unroll 1
         for (int st = 0; st < 4; ++st) {
             const cplx *Xc = X + (size_t)xb * NV * N;
-            cplx acc[NTILE][NV];
+            // ILP independent accumulator sets (consecutive streamed rows) when a thread has few (row, trajectory) pairs:
+            // a single set would be one dependent fma chain of N links
+            constexpr int ILP = (NTILE * NV <= 2) ? 4 : ((NTILE * NV <= 4) ? 2 : 1);
+            cplx acc[ILP][NTILE][NV];
             #pragma unroll
-            for (int t = 0; t < NTILE; ++t)
+            for (int i = 0; i < ILP; ++i)
                 #pragma unroll
-                for (int q = 0; q < NV; ++q) acc[t][q] = cplx{0.0, 0.0};
+                for (int t = 0; t < NTILE; ++t)
+                    #pragma unroll
+                    for (int q = 0; q < NV; ++q) acc[i][t][q] = cplx{0.0, 0.0};
             for (int c = 0; c < n_chunks; ++c) {
                 const int slot = (int)(g % NS);
                 mbar_wait(&full[slot], (unsigned)((g / NS) & 1));
                 if (active) {
                     const double *buf = reinterpret_cast<const double *>(ring + (size_t)slot * chunk_bytes);
                     const int c0 = c * rpc, rows = min(rpc, N - c0);
-                    #pragma unroll 2
-                    for (int rr = 0; rr < rows; ++rr) {
+                    auto one_row = [&](int rr, int set) {
                         const double *Dc = buf + (size_t)rr * ld;
                         cplx xq[NV];
                         #pragma unroll
                         for (int q = 0; q < NV; ++q) xq[q] = Xc[(q < nv ? q : 0) * N + c0 + rr];
                         #pragma unroll
                         for (int t = 0; t < NTILE; ++t) {
-                            const double d = Dc[min(row[t], N - 1)];
+                            const double d = Dc[rowc[t]];
                             #pragma unroll
-                            for (int q = 0; q < NV; ++q) { acc[t][q].x = fma(d, xq[q].x, acc[t][q].x); acc[t][q].y = fma(d, xq[q].y, acc[t][q].y); }
+                            for (int q = 0; q < NV; ++q) { acc[set][t][q].x = fma(d, xq[q].x, acc[set][t][q].x); acc[set][t][q].y = fma(d, xq[q].y, acc[set][t][q].y); }
                         }
+                    };
+                    int rr = 0;
+                    for (; rr + 4 <= rows; rr += 4) {
+                        one_row(rr, 0); one_row(rr + 1, 1 % ILP); one_row(rr + 2, 2 % ILP); one_row(rr + 3, 3 % ILP);
                     }
+                    for (; rr < rows; ++rr) one_row(rr, 0);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[slot]);
                 ++g;
             }
+            #pragma unroll
+            for (int i = 1; i < ILP; ++i)
+                #pragma unroll
+                for (int t = 0; t < NTILE; ++t)
+                    #pragma unroll
+                    for (int q = 0; q < NV; ++q) { acc[0][t][q].x += acc[i][t][q].x; acc[0][t][q].y += acc[i][t][q].y; }
             // k = -(i/v) P y; RK4 accumulation; the next stage's vector goes into the other buffer
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
             #pragma unroll
             for (int t = 0; t < NTILE; ++t)
                 #pragma unroll
                 for (int q = 0; q < NV; ++q) {
-                    const cplx y = cmul(acc[t][q], ph[t][q]);
+                    const cplx y = cmul(acc[0][t][q], ph[t][q]);
                     kk[t][q] = cplx{y.y * vinv[q], -y.x * vinv[q]};
                     Acc[t][q].x += wgt * kk[t][q].x; Acc[t][q].y += wgt * kk[t][q].y;
                     if (st == 3) { C[t][q].x += (h / 6.0) * Acc[t][q].x; C[t][q].y += (h / 6.0) * Acc[t][q].y; Acc[t][q] = cplx{0.0, 0.0}; }
@@ -896,17 +912,24 @@ static bool sweep1_shape(int N, int *ntile, int *nv) {
     for (auto &sh : shapes) if (N <= sh[0]) { *ntile = sh[1]; *nv = sh[2]; return true; }
     return false;
 }
+// kernel instance for units of at most `nmax` trajectories: the smallest NV >= nmax that is instantiated for this NTILE
+static int sweep1_nv_instance(int ntile, int nv_plan, int nmax) {
+    if (ntile <= 3 && nmax <= 1) return 1;
+    if (ntile <= 2 && nmax <= 2) return 2;
+    return nv_plan;
+}
 
 void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages) {
     (void)n_rad;
     int ntile = 1;
     if (!sweep1_shape(N, &ntile, nv)) { *nv = 1; *rows_per_chunk = 1; *stages = 2; return; }      // wp_sweep_one_centre reports the limit
-    // ring of whole rows (about 16 KB per chunk, 4 stages) + the double-buffered stage vectors within the 227 KB of a CTA
+    // ring of whole rows, 4 stages of up to 40 KB (about 160 KB in flight keep one SM's TMA stream busy), + the
+    // double-buffered stage vectors within the 227 KB of a CTA
     const int ld = wp_sweep1_ld(N);
     const size_t cap = 220 * 1024, vec = (size_t)2 * *nv * N * 16;
-    int rr = std::max(1, std::min(16, (int)(16384 / ((size_t)ld * 8)))), ss = 4;
-    while (ss > 2 && (size_t)ss * rr * ld * 8 + vec > cap) --ss;
+    int rr = std::max(1, std::min(32, (int)(40960 / ((size_t)ld * 8)))), ss = 4;
     while (rr > 1 && (size_t)ss * rr * ld * 8 + vec > cap) --rr;
+    while (ss > 2 && (size_t)ss * rr * ld * 8 + vec > cap) --ss;
     *rows_per_chunk = rr; *stages = ss;
 }
 
@@ -914,17 +937,18 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
     if (n_units <= 0 || a.steps <= 0) return 0;
     int ntile = 0, nvs = 0;
     if (!sweep1_shape(a.N, &ntile, &nvs)) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d exceeds the register-resident design (N <= 3136)", a.N);
-    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + (size_t)2 * nvs * a.N * 16;
+    const int nvi = sweep1_nv_instance(ntile, nvs, a.nv);           // a.nv: largest unit of this call
+    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + (size_t)2 * nvi * a.N * 16;
     if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
     static PerDevice attr_1;
-    const bool raise = wp_raise(attr_1, smem);
+    const bool raise = wp_raise(attr_1, 1);               // once per device: every instance gets the full shared-memory limit
     wp_span_begin(B, FAM_SWEEP, s);
-#define WP_SWEEP1(NT_, NV_) do { if (raise) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
+#define WP_SWEEP1(NT_, NV_) do { static PerDevice at_; if (raise || wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
         k_sweep1<NT_, NV_><<<n_units, SW1_CONSUMERS + 32, smem, s>>>(a); } while (0)
     switch (ntile) {
-        case 1: WP_SWEEP1(1, 4); break;
-        case 2: WP_SWEEP1(2, 4); break;
-        case 3: WP_SWEEP1(3, 3); break;
+        case 1: if (nvi == 1) WP_SWEEP1(1, 1); else if (nvi == 2) WP_SWEEP1(1, 2); else WP_SWEEP1(1, 4); break;
+        case 2: if (nvi == 1) WP_SWEEP1(2, 1); else if (nvi == 2) WP_SWEEP1(2, 2); else WP_SWEEP1(2, 4); break;
+        case 3: if (nvi == 1) WP_SWEEP1(3, 1); else WP_SWEEP1(3, 3); break;
         case 4: WP_SWEEP1(4, 2); break;
         case 6: WP_SWEEP1(6, 1); break;
         case 9: WP_SWEEP1(9, 1); break;

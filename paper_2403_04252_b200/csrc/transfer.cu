@@ -419,6 +419,7 @@ __global__ void __launch_bounds__(128 * (8 / NJ), 1) k_tcon(const TconArgs a) {
             const double *ck = sCk + 2 * (kc0 * 4 + fk);
             if (all_need && nk == TC_KCS) tcon_stage<NJ, true, true, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
             else if (all_need) tcon_stage<NJ, true, false, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
+            else if (nk == TC_KCS) tcon_stage<NJ, false, true, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);      // ragged tile: same unrolled pipeline, warp-uniform predicates
             else tcon_stage<NJ, false, false, TC_KCS>(Ab, Bb, ck, nk, need, Cre, Cim);
         }
         __syncwarp();

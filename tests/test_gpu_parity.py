@@ -323,3 +323,15 @@ def test_paper_zgrid_propagation(lib, one_centre, two_centre):
         Ca = lib.propagate(basis, b, v, -8.0, -1.6, 16)
         Cb = lib.propagate(basis, b, v, -1.6, 8.0, 24, C0=Ca).cpu().numpy()
         assert np.abs(Cb - C1).max() < 1e-12
+
+
+def test_explicit_coupling_matrix(lib, one_centre, two_centre):
+    """M = -(i/v) S^{-1} H of eq. (4) with N_tot right-hand sides (the paper's ZGESV usage)
+    against the oracle's S and H and a library solve; one centre: M = -(i/v) D^T (eq. (5))."""
+    for (prob, basis), pos in ((two_centre, POS2), (one_centre, POS1[:3])):
+        b, z, v = map(np.array, zip(*pos))
+        M = lib.coupling_matrix(basis, b, z, v).cpu().numpy()
+        for p in range(len(b)):
+            So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
+            Mo = (-1j / v[p]) * np.linalg.solve(So, Ho)
+            assert np.abs(M[p] - Mo).max() < 1e-12 + 1e-13 * np.abs(Mo).max() * np.linalg.cond(So), (p, np.abs(M[p] - Mo).max())
