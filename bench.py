@@ -135,7 +135,9 @@ def family_work(prob, b_local, n_steps, units=None):
         out["transfer_tables"] = ("hbm", 8.0 * 2 * (nqc[0] + nqc[1]) * nodes * n_tab, "byte")
         out["rotation"] = ("hbm", 16.0 * (3 * Nc[0] * Nc[1] + 6 * nqc[0] * nqc[1]) * n_pos, "byte")
         out["direct_assemble"] = ("hbm", 16.0 * (Nc[0] ** 2 + Nc[1] ** 2) * n_pos, "byte")
-        out["factor"] = ("alu", (8.0 * Nc[1] ** 2 * Nc[0] + 8.0 / 3.0 * Nc[1] ** 3) * n_pos, "flop")
+        # a7, solve_route 0: Hermitian rank-N_T update A = I - K K^H on the lower triangle (4 N_P^2 N_T flops) + complex Cholesky
+        # (4/3 N_P^3); counted against the DFMA peak (the DMMA peak of mma.m8n8k4 is the same number on this chip)
+        out["factor"] = ("alu", (4.0 * Nc[1] ** 2 * Nc[0] + 4.0 / 3.0 * Nc[1] ** 3) * n_pos, "flop")
         out["sweep"] = ("hbm", 16.0 * (N * N + 2 * Nc[0] * Nc[1] + Nc[1] ** 2) * 4 * n_steps * n_traj_local, "byte")
     else:
         out["direct_assemble"] = ("hbm", 8.0 * N * N * n_pos, "byte")
@@ -143,20 +145,28 @@ def family_work(prob, b_local, n_steps, units=None):
     return out
 
 
-# What one bench "step" is for each configuration: the whole job where that takes seconds, else one window of RK4 steps of
-# the configured size, successive steps walking through the configured z-range from z_min (amplitudes carried over,
-# WPCCC_INIT_FROM_DC); the metric trajectory*RK4-steps/s is intensive, so a window measures the rate of the whole job.
-STEP_WINDOW = {0: None, 1: None, 2: None, 3: 64, 4: None}
+# What one bench "step" is for each configuration: the whole job (every RK4 step of the configured z-range) of
+# STEP_BATCH[cfg] trajectories.  configs[3] (128 impact parameters x 3000 steps, minutes of GPU time) runs as 16 batches of 8
+# impact parameters (every 16th of the log-spaced set, so each batch spans the whole b-range): with 8 trajectories per call
+# the mirror stash (the body-frame integrals of all 3000 half-step positions beyond z = 0, 78 GB)
+# fits the 180 GB of HBM and every pair (b, -z), (b, +z) is evaluated once -- this is how the library runs that job
+# fastest; successive bench steps walk through the 16 batches.  --window-steps instead takes windows of RK4 steps of the
+# configured size walking through z from z_min (amplitudes carried over, WPCCC_INIT_FROM_DC), all trajectories at once.
+STEP_BATCH = {0: None, 1: None, 2: None, 3: 8, 4: None}
 
 
 class Job:
     """One configuration staged on the GPU and its bench step."""
 
-    def __init__(self, wp, cfg, world, rank, window=None, direct_tables=False):
+    def __init__(self, wp, cfg, world, rank, window=None, direct_tables=False, batch=None):
         self.wp, self.cfg = wp, cfg
         self.prob, run, self.mine = workload(cfg, world, rank)
         self.b_all, self.v_all, self.vg_all = run["b"], run["v"], run["vgroup"]
-        self.b, self.v = self.b_all[self.mine], self.v_all[self.mine]
+        self.b_job, self.v_job = self.b_all[self.mine], self.v_all[self.mine]          # this rank's trajectories of the whole job
+        self.b_run, self.world = self.b_all, world                                      # the whole job's global list (rank r owns r, r + world, ..)
+        self.n_batches = (len(self.b_job) // batch) if (batch and not window and len(self.b_job) > batch and len(self.b_job) % batch == 0) else 1
+        self.b, self.v = self.b_job, self.v_job
+        self.select_batch(0)
         self.n_steps_job, self.z0, self.z1 = run["n_steps"], run["z_min"], run["z_max"]
         self.hz = (self.z1 - self.z0) / self.n_steps_job
         self.window = min(window, self.n_steps_job) if window else None
@@ -167,6 +177,16 @@ class Job:
             self.basis.enable_direct_tables(True)
         self.k, self.C, self.n_singular = 0, None, 0
         self.world, self.rank = world, rank
+
+    def select_batch(self, k):
+        """Trajectories of bench step k: every n_batches-th of the job's list, starting at k mod n_batches."""
+        if self.n_batches > 1:
+            sl = slice(k % self.n_batches, None, self.n_batches)
+            self.b, self.v = self.b_job[sl], self.v_job[sl]
+            # the same batch on every rank; all ranks' trajectories of this step in the order gather_amplitudes returns them
+            self.b_all = self.b_run.reshape(-1, self.world)[sl].reshape(-1)
+            self.vg_all = np.zeros(len(self.b_all), np.int32)
+            self.v_all = np.full(len(self.b_all), self.v[0])
 
     def span(self):
         """z-range of the next step."""
@@ -186,6 +206,8 @@ class Job:
         C = wp.propagate(basis, self.b, self.v, za, zb, self.n_steps, C0=Cw if C0 == "walk" else C0, allow_singular=True)
         if C0 == "walk":
             self.C, self.k = C, self.k + 1
+            if self.n_batches > 1:
+                self.select_batch(self.k)
         Call = gather_amplitudes(C, len(self.b_all), self.rank, self.world)
         return wp.probabilities(basis, Call, b=self.b_all, vgroup=self.vg_all, n_vgroups=self.n_vg)
 
@@ -195,7 +217,11 @@ class Job:
         what = ("one window of %d RK4 steps of the configured size (h=%.4g) of all trajectories per step, successive steps walking through z from z_min=%g "
                 "(amplitudes carried over); the full job is %d such steps" % (self.window, self.hz, self.z0, self.n_steps_job)) if self.window else \
                ("the whole job per step: z in [%g, %g], %d RK4 steps" % (self.z0, self.z1, self.n_steps_job))
-        return "BASELINE.json configs[%d]: %s, N_tot=%d states, %d trajectories; %s" % (self.cfg, kind, self.basis.n_tot, len(self.b_all), what)
+        if self.n_batches > 1:
+            what += ("; the %d impact parameters run as %d batches of %d (every %dth of the log-spaced set), one batch per bench step, successive steps "
+                     "walking through the batches: with %d trajectories per call the mirror stash holds every position beyond z = 0" % (
+                         len(self.b_job), self.n_batches, len(self.b), self.n_batches, len(self.b)))
+        return "BASELINE.json configs[%d]: %s, N_tot=%d states, %d trajectories; %s" % (self.cfg, kind, self.basis.n_tot, len(self.b_job), what)
 
     def close(self):
         self.basis.close()
@@ -280,8 +306,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     import paper_2403_04252_b200 as wp
 
-    window = args.window_steps or STEP_WINDOW[args.config]
-    job = Job(wp, args.config, world, rank, window=window, direct_tables=args.direct_tables)
+    window = args.window_steps or None
+    job = Job(wp, args.config, world, rank, window=window, direct_tables=args.direct_tables, batch=STEP_BATCH[args.config])
     prob, b, v, b_all = job.prob, job.b, job.v, job.b_all
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
     sampler = ClockSampler(local_rank) if rank == 0 else None
@@ -379,8 +405,8 @@ def run_ours(args):
             if str(cfg) in per_config:
                 continue
             n_warm, n_timed = (3, 5) if cfg in (0, 1) else (1, 2)
-            j2 = Job(wp, cfg, 1, 0, window=STEP_WINDOW[cfg])
-            if STEP_WINDOW[cfg] is None and cfg in (2, 4):                  # whole jobs of several seconds: warm up on short windows first
+            j2 = Job(wp, cfg, 1, 0, batch=STEP_BATCH[cfg])
+            if cfg in (2, 4):                                               # whole jobs of several seconds: warm up on short windows first
                 jw = Job(wp, cfg, 1, 0, window=16)
                 jw.basis.close(); jw.basis = j2.basis
                 for _ in range(3):
@@ -398,12 +424,55 @@ def run_ours(args):
             wp.release_workspace()
             torch.cuda.empty_cache()
     line["per_config"] = {k: per_config[k] for k in sorted(per_config)}
+    if world == 1 and args.paper_shape:
+        line["paper_shape"] = paper_shape_sweep(wp, torch, flush)
     sampler.stop()
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config, budget_steps=args.cpu_steps or CPU_STEPS[args.config])
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def paper_shape_sweep(wp, torch, flush, lmax_1c=(0, 2, 4, 6, 8, 10), lmax_2c=(0, 1, 2, 3, 4, 5)):
+    """the paper's own workload shape: p + H at 100 keV, the 6001-point geometric
+    z-grid from -300 to 300, eight impact parameters, basis grown through l_max (1C N = 42 .. 4257, 2C N = 60 .. 1910).
+    Timed on the 128 central steps of that grid (all eight trajectories; the cost per step does not depend on z), reported
+    per RK4 step and extrapolated to the 6000 steps of a whole path."""
+    from wpccc_inputs.paper_shape import paper_problem
+    out = []
+    for two, lms in ((False, lmax_1c), (True, lmax_2c)):
+        for lm in lms:
+            rec = {"mode": "2C" if two else "1C", "l_max": lm}
+            try:
+                prob, run = paper_problem(two, lm)
+                rec["N"] = prob.n_tot
+                g = run["zgrid"]
+                mid = len(g) // 2
+                win = g[mid - 64: mid + 65]
+                basis = wp.setup_basis(prob)
+                for _ in range(2):
+                    wp.propagate_grid(basis, run["b"], run["v"], win, allow_singular=True)
+                ms = []
+                for _ in range(3):
+                    flush.fill_(1)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    wp.propagate_grid(basis, run["b"], run["v"], win, allow_singular=True)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    ms.append(e0.elapsed_time(e1))
+                per_step = sum(ms) / len(ms) / 128.0
+                rec.update({"ms_per_rk4_step_8_paths": round(per_step, 4), "trajectory_steps_per_s": round(8 * 1e3 / per_step, 1),
+                            "whole_path_6000_steps_s_extrapolated": round(per_step * 6000 / 1e3, 2),
+                            "flagged_not_positive_definite": sum(1 for x in wp.last_status(basis, 8) if x is not None)})
+                basis.close()
+            except Exception as e:                                    # a size beyond a kernel's design limit is reported, not hidden
+                rec["error"] = str(e)[:300]
+            wp.release_workspace()
+            torch.cuda.empty_cache()
+            out.append(rec)
+    return out
 
 
 CPU_STEPS = {0: 400, 1: 16, 2: 40, 3: 1, 4: 40}     # RK4 steps of one trajectory the oracle does in roughly 10-30 s
@@ -417,14 +486,12 @@ def cpu_sample(cfg_idx, n_rk4_steps):
     prob, run = build_config(cfg_idx)
     h = (run["z_max"] - run["z_min"]) / run["n_steps"]
     i = len(run["b"]) // 2
-    t0 = time.perf_counter()
+    t0, c0 = time.perf_counter(), time.process_time()
     oprop.propagate(prob, float(run["b"][i]), float(run["v"][i]), -0.5 * n_rk4_steps * h, 0.5 * n_rk4_steps * h, n_rk4_steps)
-    dt = time.perf_counter() - t0
-    try:
-        from threadpoolctl import threadpool_info
-        thr = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
-    except Exception:
-        thr = os.cpu_count() or 1
+    dt, cpu = time.perf_counter() - t0, time.process_time() - c0
+    # threads the oracle actually used: CPU time of the process (all threads) / wall time.  The oracle is numpy as it
+    # stands: its matrix products run on the BLAS thread pool, everything else is single-threaded Python
+    thr = max(1, int(round(cpu / dt)))
     sample = "configs[%d], 1 trajectory (b=%.4g, v=%.3g), %d RK4 steps of the configured size around z=0 (%d evaluations of S,H + %d solves)" % (
         cfg_idx, run["b"][i], run["v"][i], n_rk4_steps, 2 * n_rk4_steps + 1, 4 * n_rk4_steps)
     return dt, sample, thr
@@ -467,6 +534,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[i] of the headline line (default: the largest single-GPU configuration)")
     ap.add_argument("--per-config", dest="per_config", action="store_true", default=True, help="also measure the other four configurations (a few steps each) into per_config")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false")
+    ap.add_argument("--paper-shape", action="store_true", help="SURVEY.md 8(f) NEXT-3: also time the paper's own workload shape (l_max sweep on the geometric z-grid) into paper_shape")
     ap.add_argument("--cpu-steps", type=int, default=0, help="RK4 steps of the cpu_baseline sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--direct-tables", action="store_true", help="SURVEY.md 8(f) NEXT-1: radial sums from prefix/suffix tables instead of the DMMA GEMM (family direct_gemm then counts HBM bytes)")

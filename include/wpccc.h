@@ -102,6 +102,15 @@ int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_centre *cent
                       double Z_proj, int Nr, double h, const double *w /*[host]*/, int lambda_max,
                       const wpccc_quad *quad /*[host]; NULL iff n_centres == 1*/,
                       void *dev_arena /*[device]*/, size_t arena_bytes, void *stream);
+/* The same on a non-uniform radial grid r[0] = 0 < r[1] < ... < r[Nr] [host] ("The grid is denser around the origin";
+ * SURVEY.md 8(f) NEXT-3): u, g and w are tabulated on these points (w: the caller's quadrature weights, e.g. trapezoid
+ * (r[k+1] - r[k-1])/2).  Eq. (7) sums over the given points; the five-point interpolation of the two-centre node tables takes
+ * the grid point nearest to r (the lower one on a tie) as stencil centre, clamped to [2, Nr - 2], with Lagrange weights on the
+ * actual abscissae; functions vanish beyond r[Nr]. */
+int wpccc_setup_basis_grid(wpccc_basis **out, int n_centres, const wpccc_centre *centres /*[host]*/,
+                           double Z_proj, int Nr, const double *r /*[host]*/, const double *w /*[host]*/, int lambda_max,
+                           const wpccc_quad *quad /*[host]; NULL iff n_centres == 1*/,
+                           void *dev_arena /*[device]*/, size_t arena_bytes, void *stream);
 void wpccc_free_basis(wpccc_basis *basis);
 
 /* Sizes the caller needs to allocate outputs: total number of states N_tot, states on centre c,

@@ -51,6 +51,9 @@ _lib.wpccc_basis_bytes.argtypes = [C.c_int, C.POINTER(_Centre), C.c_int, C.c_int
 _lib.wpccc_setup_basis.restype = C.c_int
 _lib.wpccc_setup_basis.argtypes = [C.POINTER(_vp), C.c_int, C.POINTER(_Centre), C.c_double, C.c_int, C.c_double, _dp, C.c_int,
                                    C.POINTER(_Quad), _vp, C.c_size_t, _vp]
+_lib.wpccc_setup_basis_grid.restype = C.c_int
+_lib.wpccc_setup_basis_grid.argtypes = [C.POINTER(_vp), C.c_int, C.POINTER(_Centre), C.c_double, C.c_int, _dp, _dp, C.c_int,
+                                        C.POINTER(_Quad), _vp, C.c_size_t, _vp]
 _lib.wpccc_free_basis.restype = None
 _lib.wpccc_free_basis.argtypes = [_vp]
 for _n in ("wpccc_n_states",):
@@ -92,7 +95,7 @@ _lib.wpccc_enable_direct_tables.argtypes = [_vp, _vp, C.c_size_t, _vp]
 _lib.wpccc_last_error.restype = C.c_char_p
 _lib.wpccc_version.restype = C.c_char_p
 
-EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
+EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_setup_basis_grid", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
            "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_coupling_matrix_ws_bytes", "wpccc_coupling_matrix", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
            "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
@@ -164,8 +167,14 @@ class Basis:
         base = (self.arena.data_ptr() + 255) & ~255
         w = _f64(prob.w)
         h = C.c_void_p()
-        _check(_lib.wpccc_setup_basis(C.byref(h), len(prob.centres), cs, float(prob.Z_proj), int(prob.Nr), float(prob.h), _ptr(w),
-                                      int(prob.lambda_max), qp, C.c_void_p(base), nbytes, _stream(torch)))
+        rgrid = getattr(prob, "rgrid", None)             # non-uniform radial grid [Nr+1] (wpccc_setup_basis_grid), else uniform k h
+        if rgrid is not None:
+            rg = _f64(rgrid)
+            _check(_lib.wpccc_setup_basis_grid(C.byref(h), len(prob.centres), cs, float(prob.Z_proj), int(prob.Nr), _ptr(rg), _ptr(w),
+                                               int(prob.lambda_max), qp, C.c_void_p(base), nbytes, _stream(torch)))
+        else:
+            _check(_lib.wpccc_setup_basis(C.byref(h), len(prob.centres), cs, float(prob.Z_proj), int(prob.Nr), float(prob.h), _ptr(w),
+                                          int(prob.lambda_max), qp, C.c_void_p(base), nbytes, _stream(torch)))
         self._h = h
         self.n_centres = len(prob.centres)
         self.n_tot = _lib.wpccc_n_states(h)

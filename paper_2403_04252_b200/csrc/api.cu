@@ -132,12 +132,12 @@ GeomOut carve_geom(Carver &cv, size_t n) {
 
 // elements of one block of positions (geometry already on the device): F, then H0 / K (two-centre) or Dre (one-centre)
 int elements_two_centre(wpccc_basis *B, int n_pos, const GeomOut &g, double *d_F, double *d_K, double *d_H, void *tws, size_t tws_bytes,
-                        int chunk, cudaStream_t s, const TransferSel *sel = nullptr) {
+                        int chunk, cudaStream_t s, const TransferSel *sel = nullptr, double *d_KT = nullptr) {
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
     int rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, s); if (rc) return rc;
     rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_H, N, (long long)N * N, 1, s); if (rc) return rc;
     rc = wp_direct_assemble(B, 1, n_pos, g.cosT, d_F, B->E_tot, d_H + ((size_t)NT * N + NT) * 2, N, (long long)N * N, 1, s); if (rc) return rc;
-    return wp_transfer(B, n_pos, g.R, g.cosT, g.sinT, g.theta, g.v, d_K, d_H, tws, tws_bytes, chunk, s, sel);
+    return wp_transfer(B, n_pos, g.R, g.cosT, g.sinT, g.theta, g.v, d_K, d_H, tws, tws_bytes, chunk, s, sel, d_KT);    // d_KT: H^T and K^T for the sweep
 }
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -156,7 +156,7 @@ PropPlan plan_propagate(const wpccc_basis *B, int n_traj, int n_groups, int n_un
         P.tws = align256(wp_transfer_ws_bytes(B, wp_transfer_default_chunk(B)));
         P.fixed = P.tws + 64 * 1024 + (size_t)n_traj * 64 + grid;
         P.per_idx_single = (size_t)n_traj * (6 * 8 + (size_t)B->E_tot * 8 + NP * NP * 16) + 4096;                    // geometry + F + Schur-complement scratch
-        P.per_idx_double = (size_t)n_traj * (N * N * 16 + NP * NT * 16 + wp_factor_elems((int)NP) * 16 + 4) + 4096;  // H0, K, factor, flags
+        P.per_idx_double = (size_t)n_traj * (N * N * 16 + 2 * NP * NT * 16 + wp_factor_elems((int)NP) * 16 + 4) + 4096;  // H0^T, K, K^T, factor, flags
     } else {
         P.tws = 0;
         P.fixed = 64 * 1024 + (size_t)n_traj * 64 + (size_t)n_units * sizeof(SweepUnit) + grid;
@@ -173,7 +173,7 @@ int preferred_window(const PropPlan &P, int n_steps, size_t cap) {
     while (W > 1 && plan_bytes(P, W) > cap) --W;
     return W;
 }
-constexpr size_t WS_PREFERRED_CAP = (size_t)96 << 30;     // wpccc_workspace_bytes(.., 1) never asks for more than this (180 GB HBM)
+constexpr size_t WS_PREFERRED_CAP = (size_t)120 << 30;    // wpccc_workspace_bytes(.., 1) never asks for more than this (180 GB HBM)
 
 }  // namespace
 
@@ -192,8 +192,13 @@ extern "C" size_t wpccc_workspace_bytes(const wpccc_basis *B, int n_traj, int n_
     if (what == 2) return plan_bytes(P, 1);
     const int W = preferred_window(P, n_steps, WS_PREFERRED_CAP);
     size_t tot = plan_bytes(P, W);
-    if (P.two && W == std::min(std::max(n_steps, 1), 64) && wp_transfer_mirror_ok(B) && B->opt.mirror_pairs)     // mirror stash, at most 32 GB
-        tot += std::min((size_t)n_traj * (size_t)std::max(n_steps, 1) * wp_transfer_stash_doubles(B) * 8, (size_t)32 << 30) + 4096;
+    if (P.two && W == std::min(std::max(n_steps, 1), 64) && wp_transfer_mirror_ok(B) && B->opt.mirror_pairs) {
+        // mirror stash: the body-frame integrals of the n_steps half-step positions beyond z = 0 of
+        // every trajectory, as far as the total stays within WS_PREFERRED_CAP (then only the positions next to z = 0 are paired:
+        // run fewer trajectories per call to pair them all)
+        const size_t want = (size_t)n_traj * (size_t)std::max(n_steps, 1) * wp_transfer_stash_doubles(B) * 8;
+        tot += std::min(want, WS_PREFERRED_CAP > tot ? WS_PREFERRED_CAP - tot : 0) + 4096;
+    }
     return tot;
 }
 
@@ -334,12 +339,12 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
     GeomOut g = carve_geom(cv, npos_max);
     double *d_F = cv.take<double>(npos_max * B->E_tot);
     void *d_fscratch = two ? cv.take<char>(wp_factor_scratch_bytes(B, (int)npos_max)) : nullptr;
-    double *d_H[2] = {nullptr, nullptr}, *d_K[2] = {nullptr, nullptr}, *d_LU[2] = {nullptr, nullptr}, *d_D[2] = {nullptr, nullptr};
+    double *d_H[2] = {nullptr, nullptr}, *d_K[2] = {nullptr, nullptr}, *d_KT[2] = {nullptr, nullptr}, *d_LU[2] = {nullptr, nullptr}, *d_D[2] = {nullptr, nullptr};
     int *d_flags[2] = {nullptr, nullptr};
     const size_t NT = B->c[0].n_states, NP = two ? B->c[1].n_states : 0;
     for (int k = 0; k < 2; ++k) {
         if (two) {
-            d_H[k] = cv.take<double>(npos_max * N * N * 2); d_K[k] = cv.take<double>(npos_max * NP * NT * 2);
+            d_H[k] = cv.take<double>(npos_max * N * N * 2); d_K[k] = cv.take<double>(npos_max * NP * NT * 2); d_KT[k] = cv.take<double>(npos_max * NP * NT * 2);
             d_LU[k] = cv.take<double>(npos_max * wp_factor_elems((int)NP) * 2); d_flags[k] = cv.take<int>(npos_max);
         } else d_D[k] = cv.take<double>(npos_max * N * ldD);
     }
@@ -401,7 +406,7 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
                 sel.n_pre = (int)std::max<long long>(0, std::min<long long>(n_idx, sel.i_mid + 1 - i0));
                 sel.suf0 = (int)std::max<long long>(sel.n_pre, std::min<long long>(n_idx, sel.i_mid + sel.n_st + 1 - i0));
             }
-            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e, mirror ? &sel : nullptr);
+            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e, mirror ? &sel : nullptr, d_KT[buf]);
             if (!rc) cu(cudaMemsetAsync(d_flags[buf], 0, (size_t)n_pos * sizeof(int), e), "clear flags");
             if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], d_flags[buf], d_fscratch, e);
         } else {
@@ -412,7 +417,7 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
         if (!cu(cudaEventRecord(ev_elem[buf], e), "record") || !cu(cudaStreamWaitEvent(sw, ev_elem[buf], 0), "wait for the elements")) break;
         if (two) {
             Sweep2Args a{};
-            a.H = d_H[buf]; a.K = d_K[buf]; a.Ainv = d_LU[buf];
+            a.H = d_H[buf]; a.K = d_K[buf]; a.KT = d_KT[buf]; a.Ainv = d_LU[buf];
             a.st_rad_T = B->c[0].d_st_rad; a.st_rad_P = B->c[1].d_st_rad; a.eps_T = B->c[0].d_eps; a.eps_P = B->c[1].d_eps;
             a.v = d_v; a.C = dC; a.drift = d_norm_drift; a.NT = (int)NT; a.NP = (int)NP; a.n_idx = n_idx; a.steps = steps;
             a.zh = d_zh + i0; a.hs = d_hs + s0; a.solve = B->opt.solve_route == 0; a.flags = d_flags[buf]; a.traj_status = d_traj_status; a.i0 = i0;

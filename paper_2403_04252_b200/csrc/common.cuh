@@ -11,8 +11,8 @@
 
 #include "wpccc.h"
 
-#define WP_MAX_L 6        // largest orbital momentum supported per centre
-#define WP_MAX_LAMBDA 12  // largest multipole (2 * WP_MAX_L)
+#define WP_MAX_L 10       // largest orbital momentum supported per centre
+#define WP_MAX_LAMBDA 20  // largest multipole (2 * WP_MAX_L)
 #define WP_NFAM 8         // timing families (wpccc_last_timing)
 #define WP_SCRATCH_BYTES (1u << 20)   // index scratch of wpccc_probabilities inside the basis arena
 
@@ -94,6 +94,7 @@ struct wpccc_basis {
     double *d_rp = nullptr;    // [lambda_max+1][Kpad] r_k^lambda
     double *d_rm = nullptr;    // [lambda_max+1][Kpad] r_k^-(lambda+1)
     double *d_rk = nullptr;    // [Kpad] r_k (0 in the padding)
+    double *d_rgrid = nullptr; // [Nr+1] r_0 = 0 .. r_Nr of a non-uniform radial grid (wpccc_setup_basis_grid); nullptr: uniform r_k = k h
     GemmTile *d_tiles = nullptr;
     int *d_ent_lam = nullptr;   // [E_tot] multipole of every radial entry (both centres)
     double2 *d_dtab = nullptr;  // [Nr+1][E_tot] (P_e[g], Q_e[g]) prefix/suffix sums of eq. (7), caller-owned; nullptr: GEMM
@@ -162,7 +163,7 @@ int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes);
 // others come from sel->stash.
 int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
                 const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s,
-                const TransferSel *sel = nullptr);
+                const TransferSel *sel = nullptr, double *d_KT = nullptr);   // d_KT: also K^T [p][N_T][N_P], and the H_PT / H_TP blocks go to H^T
 size_t wp_transfer_stash_doubles(const wpccc_basis *B);   // doubles per stash slot
 bool wp_transfer_mirror_ok(const wpccc_basis *B);         // the mirror-pair contraction kernel fits shared memory
 int wp_transfer_default_chunk(const wpccc_basis *B);

@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(128) k_direct_tables_build(const TabBuildArgs 
     for (int k = a.Nr; k >= 1; --k) { acc += pp[k - 1] * rm[k - 1]; a.T[(size_t)(k - 1) * a.E_tot + e].y = acc; }
 }
 
-struct TabEvalArgs { const double2 *T; const int *ent_lam; const double *rk, *R; double *F; int E_tot, Nr, ldF, lambda_max; double h; PosMap rmap, fmap; };
+struct TabEvalArgs { const double2 *T; const int *ent_lam; const double *rk, *R; double *F; int E_tot, Nr, ldF, lambda_max, uniform; double h; PosMap rmap, fmap; };
 // grid = (positions, entry blocks of 256)
 __global__ void __launch_bounds__(256) k_direct_tables_eval(const TabEvalArgs a) {
     __shared__ double sRp[WP_MAX_LAMBDA + 1], sRm[WP_MAX_LAMBDA + 1];
@@ -293,7 +293,9 @@ __global__ void __launch_bounds__(256) k_direct_tables_eval(const TabEvalArgs a)
     const double R = a.R[pos_row(a.rmap, p)];
     if (threadIdx.x == 0) {
         // g = number of grid points r_k = rk[k-1] (k = 1..Nr) with r_k < R: the same comparison as the GEMM's operand
-        int g = (int)floor(R / a.h);
+        int g;
+        if (a.uniform) g = (int)floor(R / a.h);
+        else { int lo = 0, hi = a.Nr; while (lo < hi) { const int mid = (lo + hi) >> 1; if (a.rk[mid] < R) lo = mid + 1; else hi = mid; } g = lo; }   // bisection on a non-uniform grid
         g = max(0, min(a.Nr, g));
         while (g < a.Nr && a.rk[g] < R) ++g;
         while (g > 0 && !(a.rk[g - 1] < R)) --g;
@@ -339,7 +341,7 @@ int wp_direct_gemm(wpccc_basis *B, int n_pos, const double *d_R, double *d_F, in
         TabEvalArgs t{};
         t.rmap = rmap ? *rmap : ident; t.fmap = fmap ? *fmap : ident;
         t.T = B->d_dtab; t.ent_lam = B->d_ent_lam; t.rk = B->d_rk; t.R = d_R; t.F = d_F; t.E_tot = B->E_tot; t.Nr = B->Nr; t.ldF = ldF;
-        t.lambda_max = B->lambda_max; t.h = B->h;
+        t.lambda_max = B->lambda_max; t.h = B->h; t.uniform = B->d_rgrid == nullptr;
         wp_span_begin(B, FAM_GEMM, s);
         k_direct_tables_eval<<<dim3(n_pos, (B->E_tot + 255) / 256), 256, 0, s>>>(t);
         wp_span_end(B, s, 1);

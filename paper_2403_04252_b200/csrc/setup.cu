@@ -173,6 +173,8 @@ size_t layout(wpccc_basis &B, char *base) {
     B.d_rp = bump.take<double>((size_t)L1 * B.Kpad);
     B.d_rm = bump.take<double>((size_t)L1 * B.Kpad);
     B.d_rk = bump.take<double>(B.Kpad);
+    double *rgrid = bump.take<double>(B.Nr + 1);
+    if (B.d_rgrid || !base) B.d_rgrid = base ? rgrid : reinterpret_cast<double *>(1);   // kept only for non-uniform grids (flag set by the caller)
     B.d_tiles = bump.take<GemmTile>(B.tiles.size());
     B.d_ent_lam = bump.take<int>(B.E_tot);
     B.d_st_rad_glob = bump.take<int>(B.n_tot); B.d_rad_info = bump.take<int>(B.n_rad_tot); B.d_scratch = bump.take<char>(WP_SCRATCH_BYTES);
@@ -254,20 +256,25 @@ extern "C" size_t wpccc_basis_bytes(int n_centres, const wpccc_centre *centres, 
     return layout(B, nullptr) + (size_t)(Nr + 1) * sizeof(double) + 256;   // + scratch for the weights
 }
 
-extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_centre *centres, double Z_proj, int Nr, double h,
-                                 const double *w, int lambda_max, const wpccc_quad *quad, void *dev_arena, size_t arena_bytes,
-                                 void *stream) {
+static int setup_impl(wpccc_basis **out, int n_centres, const wpccc_centre *centres, double Z_proj, int Nr, double h, const double *rgrid,
+                      const double *w, int lambda_max, const wpccc_quad *quad, void *dev_arena, size_t arena_bytes, void *stream) {
     if (!out) WP_FAIL(WPCCC_EINVAL, "out is NULL");
     *out = nullptr;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) WP_FAIL(WPCCC_ECUDA, "no CUDA device (this library has no CPU fallback)");
-    if (!w || !(h > 0)) WP_FAIL(WPCCC_EINVAL, "w is NULL or h <= 0");
+    if (!w || (!rgrid && !(h > 0))) WP_FAIL(WPCCC_EINVAL, "w is NULL or h <= 0");
+    if (rgrid) {
+        if (rgrid[0] != 0.0) WP_FAIL(WPCCC_EINVAL, "r[0] must be 0");
+        for (int k = 0; k < Nr; ++k) if (!(rgrid[k + 1] > rgrid[k])) WP_FAIL(WPCCC_EINVAL, "radial grid must be strictly increasing (index %d)", k);
+        h = rgrid[Nr] / Nr;                            // only a scale (initial guesses of index searches)
+    }
     if (!dev_arena || ((uintptr_t)dev_arena & 255)) WP_FAIL(WPCCC_EINVAL, "dev_arena must be a 256-byte aligned device pointer");
     wpccc_basis *B = new wpccc_basis;
     int rc = describe(*B, n_centres, centres, Nr, lambda_max, quad);
     if (rc) { delete B; return rc; }
     if (n_centres == 2 && Z_proj != centres[1].Z) { delete B; WP_FAIL(WPCCC_EINVAL, "Z_proj must equal centres[1].Z with two centres"); }
     B->h = h; B->Z_proj = Z_proj;
+    B->d_rgrid = rgrid ? reinterpret_cast<double *>(1) : nullptr;     // layout() turns the flag into the arena pointer
     const size_t need = layout(*B, (char *)dev_arena);
     const size_t w_off = need;
     if (arena_bytes < need + (size_t)(Nr + 1) * sizeof(double)) { delete B; WP_FAIL(WPCCC_ENOMEM, "arena too small: need %zu bytes", need + (size_t)(Nr + 1) * 8); }
@@ -279,7 +286,7 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     const int L1 = lambda_max + 1;
     std::vector<double> rp((size_t)L1 * B->Kpad, 0.0), rm((size_t)L1 * B->Kpad, 0.0), rk(B->Kpad, 0.0);
     for (int kk = 0; kk < Nr; ++kk) {
-        const double r = h * (double)(kk + 1);
+        const double r = rgrid ? rgrid[kk + 1] : h * (double)(kk + 1);
         rk[kk] = r;
         double p = 1.0;
         for (int lam = 0; lam < L1; ++lam) { rp[(size_t)lam * B->Kpad + kk] = p; rm[(size_t)lam * B->Kpad + kk] = 1.0 / (p * r); p *= r; }
@@ -287,6 +294,7 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     std::vector<cudaError_t> errs;
     auto chk = [&](int r_) { if (r_ && !rc) rc = r_; };
     chk(upload(B->d_rp, rp, s)); chk(upload(B->d_rm, rm, s)); chk(upload(B->d_rk, rk, s));
+    if (rgrid && !rc && cudaMemcpyAsync(B->d_rgrid, rgrid, (size_t)(Nr + 1) * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess) rc = WPCCC_ECUDA;
     chk(upload(B->d_tiles, B->tiles, s));
     std::vector<int> all_lam;
     for (int ci = 0; ci < n_centres; ++ci) all_lam.insert(all_lam.end(), B->c[ci].ent_lam.begin(), B->c[ci].ent_lam.end());
@@ -365,6 +373,19 @@ extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_c
     if (rc) { delete B; return rc; }
     *out = B;
     return 0;
+}
+
+extern "C" int wpccc_setup_basis(wpccc_basis **out, int n_centres, const wpccc_centre *centres, double Z_proj, int Nr, double h,
+                                 const double *w, int lambda_max, const wpccc_quad *quad, void *dev_arena, size_t arena_bytes,
+                                 void *stream) {
+    return setup_impl(out, n_centres, centres, Z_proj, Nr, h, nullptr, w, lambda_max, quad, dev_arena, arena_bytes, stream);
+}
+
+extern "C" int wpccc_setup_basis_grid(wpccc_basis **out, int n_centres, const wpccc_centre *centres, double Z_proj, int Nr, const double *r,
+                                      const double *w, int lambda_max, const wpccc_quad *quad, void *dev_arena, size_t arena_bytes,
+                                      void *stream) {
+    if (!r) WP_FAIL(WPCCC_EINVAL, "r is NULL");
+    return setup_impl(out, n_centres, centres, Z_proj, Nr, 0.0, r, w, lambda_max, quad, dev_arena, arena_bytes, stream);
 }
 
 extern "C" void wpccc_free_basis(wpccc_basis *B) {

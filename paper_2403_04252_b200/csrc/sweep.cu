@@ -622,11 +622,11 @@ __global__ void __launch_bounds__(FR_THREADS, 1) k_factor_reg(const FactorArgs a
 // stages 0..3 each [H rows | K rows | factor | K rows], then (drift only) K rows; producer and consumers walk the same
 // loops (SweepSched gives the chunk shapes).
 struct SweepSched {
-    int N, NT, NP, rH, rK, rA, nH, nK, nA, cb;
+    int N, NT, NP, rH, rK, rA, nH, nK, nA, nKT, cb;       // rA also: rows of K^T [NT][NP] per chunk (nKT chunks)
     __device__ SweepSched(int NT_, int NP_, int chunk_bytes) {
         NT = NT_; NP = NP_; N = NT + NP; cb = chunk_bytes;
         rH = max(1, chunk_bytes / (16 * N)); rK = max(1, chunk_bytes / (16 * NT)); rA = max(1, chunk_bytes / (16 * NP));
-        nH = (N + rH - 1) / rH; nK = (NP + rK - 1) / rK; nA = (NP + rA - 1) / rA;
+        nH = (N + rH - 1) / rH; nK = (NP + rK - 1) / rK; nA = (NP + rA - 1) / rA; nKT = (NT + rA - 1) / rA;
     }
     __device__ int rows_fwd(const CholLayout &L, int j) const { return max(1, min(L.nb(j), cb / (16 * L.len(j)))); }   // rows of block row j per chunk
     __device__ int rows_bwd(const CholLayout &L, int j) const { return max(1, cb / (16 * L.nb(j))); }                  // rows below block j per chunk
@@ -641,8 +641,11 @@ __device__ __forceinline__ cplx warp_dot(const cplx *row, const cplx *x, int n, 
 
 constexpr int SW_DLD = CHOL_NB + 1;      // row stride of the staged diagonal block
 
-template <bool SOLVE>
-__global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a, const int chunk_bytes) {
+constexpr int SW_TCOLS = 4;            // columns / rows of K per consumer thread in the K^H and K products: N_T, N_P <= 1024
+constexpr int SW_TROWS = 8;            // rows of H0 per consumer thread: N <= 2048
+
+template <bool SOLVE, int TR>          // TR = ceil(N / 256): rows of H0 per consumer thread
+__global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Args a, const int chunk_bytes, const int NS) {
     extern __shared__ __align__(128) unsigned char smraw[];
     const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int t = blockIdx.x;
@@ -650,9 +653,11 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
     const SweepSched S(NT, NP, chunk_bytes);
     const CholLayout CL(NP);
     unsigned char *ring = smraw;
-    cplx *C = reinterpret_cast<cplx *>(smraw + (size_t)SW_STAGES * chunk_bytes);
-    cplx *Acc = C + N, *X = Acc + N, *Kn = X + N, *Y = Kn + N, *ph = Y + N, *Wp = ph + N, *part = Wp + NP;   // part [8][NT]
-    cplx *Tj = part + 8 * NT, *Dblk = Tj + CHOL_NB, *part2 = Dblk + CHOL_NB * SW_DLD;                          // SOLVE: [32], [32][33], [8][32]
+    // shared: the stage vectors X, Y, w_P; the state of element j = tid + 256 t (amplitude C, RK4 accumulator, last slope,
+    // phase) lives in registers of the thread that owns it
+    cplx *X = reinterpret_cast<cplx *>(smraw + (size_t)NS * chunk_bytes);
+    cplx *Y = X + N, *Wp = Y + N;
+    cplx *Tj = Wp + NP, *Dblk = Tj + CHOL_NB, *part2 = Dblk + CHOL_NB * SW_DLD;                                  // SOLVE: [32], [32][33], [8][32]
     __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
     __shared__ double red[8];
     __shared__ int redi[8];
@@ -662,6 +667,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
     }
     __syncthreads();
     const cplx *Hg = reinterpret_cast<const cplx *>(a.H), *Kg = reinterpret_cast<const cplx *>(a.K), *Ag = reinterpret_cast<const cplx *>(a.Ainv);
+    const cplx *KTg = reinterpret_cast<const cplx *>(a.KT);
     const size_t a_stride = wp_factor_elems(NP);
 
     if (warp == SW_CONSUMERS / 32) {
@@ -669,22 +675,23 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
         if (lane != 0) return;
         long long g = 0;
         auto push = [&](const cplx *src, unsigned bytes) {
-            const int slot = (int)(g % SW_STAGES); const long long use = g / SW_STAGES;
+            const int slot = (int)(g % NS); const long long use = g / NS;
             if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
             mbar_expect_tx(&full[slot], bytes);
             tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
             ++g;
         };
         auto push_K = [&](const cplx *Kp) { for (int q = 0; q < S.nK; ++q) { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); push(Kp + (size_t)r0 * NT, (unsigned)rows * NT * 16u); } };
+        auto push_KT = [&](const cplx *Kp) { for (int q = 0; q < S.nKT; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NT - r0); push(Kp + (size_t)r0 * NP, (unsigned)rows * NP * 16u); } };
         for (int s = 0; s < a.steps; ++s)
             for (int st = 0; st < (track ? 5 : 4); ++st) {
                 const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
                 const size_t pos = (size_t)t * a.n_idx + li;
-                const cplx *Kp = Kg + pos * (size_t)NP * NT;
-                if (st == 4) { push_K(Kp); break; }
+                const cplx *Kp = Kg + pos * (size_t)NP * NT, *KTp = KTg + pos * (size_t)NP * NT;
+                if (st == 4) { push_KT(KTp); break; }
                 const cplx *Hp = Hg + pos * (size_t)N * N, *Ap = Ag + pos * a_stride;
                 for (int q = 0; q < S.nH; ++q) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); push(Hp + (size_t)r0 * N, (unsigned)rows * N * 16u); }
-                push_K(Kp);
+                push_KT(KTp);
                 if (!SOLVE) {
                     for (int q = 0; q < S.nA; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NP - r0); push(Ap + (size_t)r0 * NP, (unsigned)rows * NP * 16u); }
                 } else {
@@ -704,10 +711,18 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
     }
     // ---------------- consumers (256 threads)
     const double vel = a.v[t];
-    for (int j = tid; j < N; j += SW_CONSUMERS) {
-        const double *src = a.C + ((size_t)t * N + j) * 2;
-        C[j] = {src[0], src[1]}; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0};
+    cplx C[TR], Acc[TR], Kn[TR], ph[TR]; double eov[TR];
+    #pragma unroll
+    for (int tr = 0; tr < TR; ++tr) {
+        const int j = tid + SW_CONSUMERS * tr;
+        C[tr] = Acc[tr] = Kn[tr] = ph[tr] = cplx{0.0, 0.0}; eov[tr] = 0.0;
+        if (j < N) {
+            const double *src = a.C + ((size_t)t * N + j) * 2;
+            C[tr] = cplx{src[0], src[1]};
+            eov[tr] = ((j < NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - NT]]) / vel;
+        }
     }
+    int li_ph = -1;                                          // half-step index the phases in ph[] belong to
     // first position of this window whose overlap factorisation failed (n_idx: none)
     int first_bad = a.n_idx;
     if (a.flags) {
@@ -718,13 +733,13 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
     double drift = track ? a.drift[t] : 0.0;
     long long g = 0;                                         // chunk counter, in step with the producer
     auto acquire = [&]() -> const cplx * {
-        const int slot = (int)(g % SW_STAGES);
-        mbar_wait(&full[slot], (unsigned)((g / SW_STAGES) & 1));
+        const int slot = (int)(g % NS);
+        mbar_wait(&full[slot], (unsigned)((g / NS) & 1));
         return reinterpret_cast<const cplx *>(ring + (size_t)slot * chunk_bytes);
     };
     auto release = [&]() {
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[(int)(g % SW_STAGES)]);
+        if (lane == 0) mbar_arrive(&empty[(int)(g % NS)]);
         ++g;
     };
     consumer_sync();
@@ -740,31 +755,67 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
             const double alpha = (st == 0 || st == 4) ? 0.0 : (st == 3 ? h : 0.5 * h);
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
             const double z = a.zh[li];
-            for (int j = tid; j < N; j += SW_CONSUMERS) {
-                const double e = (j < NT) ? a.eps_T[a.st_rad_T[j]] : a.eps_P[a.st_rad_P[j - NT]];
-                double sn, cs; sincos(e * z / vel, &sn, &cs);
-                ph[j] = {cs, sn};
-                const cplx x = {C[j].x + alpha * Kn[j].x, C[j].y + alpha * Kn[j].y};
-                X[j] = cmulc(x, {cs, sn});
+            #pragma unroll
+            for (int tr = 0; tr < TR; ++tr) {
+                const int j = tid + SW_CONSUMERS * tr;
+                if (li != li_ph) { double sn, cs; sincos(eov[tr] * z, &sn, &cs); ph[tr] = cplx{cs, sn}; }
+                if (j < N) X[j] = cmulc(cplx{C[tr].x + alpha * Kn[tr].x, C[tr].y + alpha * Kn[tr].y}, ph[tr]);
             }
-            for (int j = tid; j < 8 * NT; j += SW_CONSUMERS) part[j] = {0.0, 0.0};
+            li_ph = li;
             consumer_sync();
-            if (st == 4) {
-                // c^H S c = |c|^2 + 2 Re( X_P^H K X_T )
-                double acc = 0.0;
-                for (int q = 0; q < S.nK; ++q) {
+            // (K v)_r = sum_c K^T[c][r] v_c for this thread's rows r = tid + 256 t of the projectile block: the rows c of K^T stream
+            // through the ring, v_c is a broadcast, consecutive lanes read consecutive elements -- no reduction
+            // (ILP independent accumulator sets over consecutive streamed rows: one set is a dependent fma chain of N_T links)
+            auto k_times = [&](const cplx *vT, cplx (&accK)[SW_TCOLS]) {
+                constexpr int TC = (TR + 1) / 2, ILP = TC == 1 ? 4 : 2;
+                cplx ak[ILP][TC];
+                #pragma unroll
+                for (int u = 0; u < ILP; ++u)
+                    #pragma unroll
+                    for (int tc = 0; tc < TC; ++tc) ak[u][tc] = cplx{0.0, 0.0};
+                for (int q = 0; q < S.nKT; ++q) {
                     const cplx *buf = acquire();
-                    const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
-                    for (int r = warp; r < rows; r += 8) {
-                        const cplx d = warp_dot(buf + (size_t)r * NT, X, NT, lane);
-                        acc += 2.0 * (X[NT + r0 + r].x * d.x + X[NT + r0 + r].y * d.y);
+                    const int c0 = q * S.rA, rows = min(S.rA, NT - c0);
+                    auto one = [&](int rr, int u) {
+                        const cplx y = vT[c0 + rr];
+                        const cplx *Kc = buf + (size_t)rr * NP;
+                        #pragma unroll
+                        for (int tc = 0; tc < TC; ++tc) {
+                            const int r = tid + SW_CONSUMERS * tc;
+                            if (r < NP) { const cplx k = Kc[r]; ak[u][tc].x += k.x * y.x - k.y * y.y; ak[u][tc].y += k.x * y.y + k.y * y.x; }
+                        }
+                    };
+                    int rr = 0;
+                    for (; rr + ILP <= rows; rr += ILP) {
+                        #pragma unroll
+                        for (int u = 0; u < ILP; ++u) one(rr + u, u);
                     }
+                    for (; rr < rows; ++rr) one(rr, 0);
                     release();
                 }
+                #pragma unroll
+                for (int tc = 0; tc < SW_TCOLS; ++tc) {
+                    accK[tc] = cplx{0.0, 0.0};
+                    if (tc < TC) {
+                        #pragma unroll
+                        for (int u = 0; u < ILP; ++u) { accK[tc].x += ak[u][tc < TC ? tc : 0].x; accK[tc].y += ak[u][tc < TC ? tc : 0].y; }
+                    }
+                }
+            };
+            if (st == 4) {
+                // c^H S c = |c|^2 + 2 Re( X_P^H K X_T )
+                cplx accK[SW_TCOLS];
+                k_times(X, accK);
                 double nrm = 0.0;
-                for (int j = tid; j < N; j += SW_CONSUMERS) nrm += X[j].x * X[j].x + X[j].y * X[j].y;
+                #pragma unroll
+                for (int tc = 0; tc < SW_TCOLS; ++tc) {
+                    const int r = tid + SW_CONSUMERS * tc;
+                    if (r < NP) nrm += 2.0 * (X[NT + r].x * accK[tc].x + X[NT + r].y * accK[tc].y);
+                }
+                #pragma unroll
+                for (int tr = 0; tr < TR; ++tr) { const int j = tid + SW_CONSUMERS * tr; if (j < N) nrm += X[j].x * X[j].x + X[j].y * X[j].y; }
                 nrm = warp_sum(nrm);
-                if (lane == 0) red[warp] = acc + nrm;
+                if (lane == 0) red[warp] = nrm;
                 consumer_sync();
                 double tot = 0.0;
                 for (int w = 0; w < 8; ++w) tot += red[w];
@@ -772,26 +823,50 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
                 consumer_sync();
                 break;
             }
-            // y = H0 x
-            for (int q = 0; q < S.nH; ++q) {
-                const cplx *buf = acquire();
-                const int r0 = q * S.rH, rows = min(S.rH, N - r0);
-                for (int r = warp; r < rows; r += 8) {
-                    const cplx d = warp_dot(buf + (size_t)r * N, X, N, lane);
-                    if (lane == 0) Y[r0 + r] = d;
+            // y = H0 x from the streamed rows c of H0^T: y_r = sum_c H0^T[c][r] x_c, thread tid owns the rows r = tid + 256 t
+            {
+                constexpr int ILP = TR == 1 ? 4 : (TR <= 3 ? 2 : 1);
+                cplx accY[ILP][TR];
+                #pragma unroll
+                for (int u = 0; u < ILP; ++u)
+                    #pragma unroll
+                    for (int tr = 0; tr < TR; ++tr) accY[u][tr] = cplx{0.0, 0.0};
+                for (int q = 0; q < S.nH; ++q) {
+                    const cplx *buf = acquire();
+                    const int c0 = q * S.rH, rows = min(S.rH, N - c0);
+                    auto one = [&](int rr, int u) {
+                        const cplx x = X[c0 + rr];
+                        const cplx *Hc = buf + (size_t)rr * N;
+                        #pragma unroll
+                        for (int tr = 0; tr < TR; ++tr) {
+                            const int r = tid + SW_CONSUMERS * tr;
+                            if (r < N) { const cplx hh = Hc[r]; accY[u][tr].x += hh.x * x.x - hh.y * x.y; accY[u][tr].y += hh.x * x.y + hh.y * x.x; }
+                        }
+                    };
+                    int rr = 0;
+                    for (; rr + ILP <= rows; rr += ILP) {
+                        #pragma unroll
+                        for (int u = 0; u < ILP; ++u) one(rr + u, u);
+                    }
+                    for (; rr < rows; ++rr) one(rr, 0);
+                    release();
                 }
-                release();
+                #pragma unroll
+                for (int tr = 0; tr < TR; ++tr) {
+                    const int r = tid + SW_CONSUMERS * tr;
+                    cplx y = accY[0][tr];
+                    #pragma unroll
+                    for (int u = 1; u < ILP; ++u) { y.x += accY[u][tr].x; y.y += accY[u][tr].y; }
+                    if (r < N) Y[r] = y;
+                }
             }
             consumer_sync();
             // y_P -= K y_T
-            for (int q = 0; q < S.nK; ++q) {
-                const cplx *buf = acquire();
-                const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
-                for (int r = warp; r < rows; r += 8) {
-                    const cplx d = warp_dot(buf + (size_t)r * NT, Y, NT, lane);
-                    if (lane == 0) { Y[NT + r0 + r].x -= d.x; Y[NT + r0 + r].y -= d.y; }
-                }
-                release();
+            {
+                cplx accK[SW_TCOLS];
+                k_times(Y, accK);
+                #pragma unroll
+                for (int tc = 0; tc < SW_TCOLS; ++tc) { const int r = tid + SW_CONSUMERS * tc; if (r < NP) { Y[NT + r].x -= accK[tc].x; Y[NT + r].y -= accK[tc].y; } }
             }
             consumer_sync();
             if (!SOLVE) {
@@ -866,28 +941,39 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
                     consumer_sync();
                 }
             }
-            // w_T = y_T - K^H w_P: per-warp partial sums over its rows of K
+            // w_T = y_T - K^H w_P: thread c owns the columns c, c + 256, .. of K (consecutive lanes, conflict-free), reads
+            // w_P[r] as a broadcast and accumulates over the streamed rows in registers: no partial sums, no reduction
+            cplx accT[SW_TCOLS];
+            #pragma unroll
+            for (int tc = 0; tc < SW_TCOLS; ++tc) accT[tc] = cplx{0.0, 0.0};
             for (int q = 0; q < S.nK; ++q) {
                 const cplx *buf = acquire();
                 const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
-                for (int r = warp; r < rows; r += 8) {
+                for (int r = 0; r < rows; ++r) {
                     const cplx x = Wp[r0 + r];
                     const cplx *Kr = buf + (size_t)r * NT;
-                    cplx *pw = part + warp * NT;
-                    for (int c = lane; c < NT; c += 32) { const cplx k = Kr[c]; pw[c].x += k.x * x.x + k.y * x.y; pw[c].y += k.x * x.y - k.y * x.x; }
+                    #pragma unroll
+                    for (int tc = 0; tc < SW_TCOLS; ++tc) {
+                        const int c = tid + SW_CONSUMERS * tc;
+                        if (c < NT) { const cplx k = Kr[c]; accT[tc].x += k.x * x.x + k.y * x.y; accT[tc].y += k.x * x.y - k.y * x.x; }
+                    }
                 }
                 release();
             }
-            consumer_sync();
             // k = -(i/v) P w
-            for (int j = tid; j < N; j += SW_CONSUMERS) {
+            #pragma unroll
+            for (int tr = 0; tr < TR; ++tr) {
+                const int j = tid + SW_CONSUMERS * tr;
+                if (j >= N) continue;
                 cplx w;
-                if (j < NT) { w = Y[j]; for (int q = 0; q < 8; ++q) { w.x -= part[q * NT + j].x; w.y -= part[q * NT + j].y; } }
-                else w = Wp[j - NT];
-                const cplx y = cmul(w, ph[j]);
+                if (j < NT) {                                   // the column sums of K^H w_P for j = tid + 256 tr are this thread's own
+                    w = Y[j];
+                    if (tr < SW_TCOLS) { w.x -= accT[tr < SW_TCOLS ? tr : 0].x; w.y -= accT[tr < SW_TCOLS ? tr : 0].y; }
+                } else w = Wp[j - NT];
+                const cplx y = cmul(w, ph[tr]);
                 const cplx k = {y.y / vel, -y.x / vel};
-                Kn[j] = k; Acc[j].x += wgt * k.x; Acc[j].y += wgt * k.y;
-                if (st == 3) { C[j].x += (h / 6.0) * Acc[j].x; C[j].y += (h / 6.0) * Acc[j].y; Acc[j] = {0.0, 0.0}; Kn[j] = {0.0, 0.0}; }
+                Kn[tr] = k; Acc[tr].x += wgt * k.x; Acc[tr].y += wgt * k.y;
+                if (st == 3) { C[tr].x += (h / 6.0) * Acc[tr].x; C[tr].y += (h / 6.0) * Acc[tr].y; Acc[tr] = cplx{0.0, 0.0}; Kn[tr] = cplx{0.0, 0.0}; }
             }
             consumer_sync();
         }
@@ -896,9 +982,10 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
     // first failed half-step index is kept in traj_status (wpccc_last_status)
     const bool dead = first_bad < a.n_idx || (a.traj_status && a.traj_status[t] != 0);
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-    for (int j = tid; j < N; j += SW_CONSUMERS) {
-        double *dst = a.C + ((size_t)t * N + j) * 2;
-        dst[0] = dead ? qnan : C[j].x; dst[1] = dead ? qnan : C[j].y;
+    #pragma unroll
+    for (int tr = 0; tr < TR; ++tr) {
+        const int j = tid + SW_CONSUMERS * tr;
+        if (j < N) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = dead ? qnan : C[tr].x; dst[1] = dead ? qnan : C[tr].y; }
     }
     if (tid == 0 && a.traj_status && a.traj_status[t] == 0 && first_bad < a.n_idx)
         a.traj_status[t] = (a.flags[(size_t)t * a.n_idx + first_bad] << 28) | ((int)(a.i0 + first_bad) + 1);
@@ -908,7 +995,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32) k_sweep2(const Sweep2Args a
 
 // (rows per thread, trajectories per unit) of the one-centre sweep for N states: 224 NTILE >= N, state in registers
 static bool sweep1_shape(int N, int *ntile, int *nv) {
-    static const int shapes[][3] = {{224, 1, 4}, {448, 2, 4}, {672, 3, 3}, {896, 4, 2}, {1344, 6, 1}, {2016, 9, 1}, {3136, 14, 1}};
+    static const int shapes[][3] = {{224, 1, 4}, {448, 2, 4}, {672, 3, 3}, {896, 4, 2}, {1344, 6, 1}, {2016, 9, 1}, {3136, 14, 1}, {4480, 20, 1}};
     for (auto &sh : shapes) if (N <= sh[0]) { *ntile = sh[1]; *nv = sh[2]; return true; }
     return false;
 }
@@ -923,11 +1010,12 @@ void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages)
     (void)n_rad;
     int ntile = 1;
     if (!sweep1_shape(N, &ntile, nv)) { *nv = 1; *rows_per_chunk = 1; *stages = 2; return; }      // wp_sweep_one_centre reports the limit
-    // ring of whole rows, 4 stages of up to 40 KB (about 160 KB in flight keep one SM's TMA stream busy), + the
-    // double-buffered stage vectors within the 227 KB of a CTA
+    // ring of whole rows + the double-buffered stage vectors within the 227 KB of a CTA.  One SM's TMA bulk-copy stream
+    // delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s, 32 KB 88, 48 KB 107, 64 KB 133 GB/s):
+    // three stages of up to 56 KB
     const int ld = wp_sweep1_ld(N);
     const size_t cap = 220 * 1024, vec = (size_t)2 * *nv * N * 16;
-    int rr = std::max(1, std::min(32, (int)(40960 / ((size_t)ld * 8)))), ss = 4;
+    int rr = std::max(1, std::min(64, (int)(57344 / ((size_t)ld * 8)))), ss = 3;
     while (rr > 1 && (size_t)ss * rr * ld * 8 + vec > cap) --rr;
     while (ss > 2 && (size_t)ss * rr * ld * 8 + vec > cap) --ss;
     *rows_per_chunk = rr; *stages = ss;
@@ -936,7 +1024,7 @@ void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages)
 int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s) {
     if (n_units <= 0 || a.steps <= 0) return 0;
     int ntile = 0, nvs = 0;
-    if (!sweep1_shape(a.N, &ntile, &nvs)) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d exceeds the register-resident design (N <= 3136)", a.N);
+    if (!sweep1_shape(a.N, &ntile, &nvs)) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d exceeds the register-resident design (N <= 4480)", a.N);
     const int nvi = sweep1_nv_instance(ntile, nvs, a.nv);           // a.nv: largest unit of this call
     const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + (size_t)2 * nvi * a.N * 16;
     if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
@@ -952,7 +1040,8 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
         case 4: WP_SWEEP1(4, 2); break;
         case 6: WP_SWEEP1(6, 1); break;
         case 9: WP_SWEEP1(9, 1); break;
-        default: WP_SWEEP1(14, 1); break;
+        case 14: WP_SWEEP1(14, 1); break;
+        default: WP_SWEEP1(20, 1); break;
     }
 #undef WP_SWEEP1
     wp_span_end(B, s, 1);
@@ -963,22 +1052,29 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaSt
 int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStream_t s) {
     if (n_traj <= 0 || a.steps <= 0) return 0;
     const int N = a.NT + a.NP;
-    const size_t vec = ((size_t)6 * N + a.NP + (size_t)8 * a.NT + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB) * 16;
-    // ring chunk: at least one row of H0 (16 N bytes), about 40 KB, so that four of them and the vectors fit 220 KB
-    size_t chunk = 40 * 1024;
-    while (chunk > (size_t)16 * N && SW_STAGES * chunk + vec > 220 * 1024) chunk -= 1024;
-    chunk = std::max(chunk, std::max((size_t)16 * N, (size_t)16 * CHOL_NB * CHOL_NB));     // a row of H0, a diagonal block of the factor
-    chunk = (chunk + 127) & ~(size_t)127;
-    const size_t smem = SW_STAGES * chunk + vec;
+    if (a.NT > SW_CONSUMERS * SW_TCOLS || a.NP > SW_CONSUMERS * SW_TCOLS) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N_T = %d or N_P = %d exceeds %d", a.NT, a.NP, SW_CONSUMERS * SW_TCOLS);
+    if (N > SW_CONSUMERS * 8) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d exceeds %d", N, SW_CONSUMERS * 8);
+    const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB) * 16;
+    // TMA ring: one SM's bulk-copy stream delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s,
+    // 32 KB 88, 48 KB 107, 64 KB 133 GB/s), so the chunks are as large as the shared memory allows: three stages of up to 64 KB,
+    // two stages when three would be smaller than 48 KB each
+    const size_t chunk_min = std::max((size_t)16 * N, (size_t)16 * CHOL_NB * CHOL_NB), room = (size_t)220 * 1024 - vec;
+    int NS = 3;
+    size_t chunk = std::min<size_t>(64 * 1024, room / 3);
+    if (chunk < 48 * 1024) { NS = 2; chunk = std::min<size_t>(96 * 1024, room / 2); }
+    chunk &= ~(size_t)127;
+    if (chunk < chunk_min) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
+    const size_t smem = NS * chunk + vec;
     if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
-    static PerDevice attr_2;
-    if (wp_raise(attr_2, smem)) {
-        WP_CUDA(cudaFuncSetAttribute(k_sweep2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        WP_CUDA(cudaFuncSetAttribute(k_sweep2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
+    const int tr = (N + SW_CONSUMERS - 1) / SW_CONSUMERS;
     wp_span_begin(B, FAM_SWEEP, s);
-    if (a.solve) k_sweep2<true><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
-    else k_sweep2<false><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk);
+#define WP_SWEEP2(SOLVE_, TR_) do { static PerDevice at_; if (wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep2<SOLVE_, TR_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
+        k_sweep2<SOLVE_, TR_><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk, NS); } while (0)
+#define WP_SWEEP2_TR(SOLVE_) do { if (tr <= 1) WP_SWEEP2(SOLVE_, 1); else if (tr == 2) WP_SWEEP2(SOLVE_, 2); else if (tr == 3) WP_SWEEP2(SOLVE_, 3); \
+        else if (tr == 4) WP_SWEEP2(SOLVE_, 4); else WP_SWEEP2(SOLVE_, 8); } while (0)
+    if (a.solve) WP_SWEEP2_TR(true); else WP_SWEEP2_TR(false);
+#undef WP_SWEEP2_TR
+#undef WP_SWEEP2
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;

@@ -26,8 +26,9 @@ void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages)
 int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s);
 
 struct Sweep2Args {          // two-centre: S = [[I, K^H], [K, I]], H full (eq. (1)-(4))
-    const double *H;         // [traj][n_idx][N][N] complex, no time phase
+    const double *H;         // [traj][n_idx][N][N] complex H0^T (the TRANSPOSE: row c holds column c of H0), no time phase
     const double *K;         // [traj][n_idx][NP][NT] complex S_PT, no time phase
+    const double *KT;        // [traj][n_idx][NT][NP] complex S_PT^T
     const double *Ainv;      // [traj][n_idx][NP][NP] complex (I - K K^H)^{-1}, row-major
     const int *st_rad_T, *st_rad_P; const double *eps_T, *eps_P;
     const double *v;

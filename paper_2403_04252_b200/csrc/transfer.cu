@@ -111,6 +111,7 @@ struct TtabArgs {
     double Zother[2];                        // side 0 (T functions): Z_P;  side 1: Z_T
     double h; int Nr, KC;                    // KC: z' nodes per CTA (multiple of 4)
     int sph;                                 // 1: spheroidal nodes: ring = eta_i (pos[off_rho]), axial node = tau_k (pos[off_zq])
+    const double *rgrid;                     // [Nr+1] non-uniform radial grid, or nullptr (uniform r_k = k h)
     double *out[2]; size_t pos_stride[2];    // doubles per position for each side
     int lmax[2];
     SelDev sel; int q0;
@@ -156,16 +157,37 @@ __global__ void __launch_bounds__(256) k_ttab(const TtabArgs a) {
             rs = side ? rP : rT; ro = side ? rT : rP;
             c = (side ? zP : zk) / rs;
         }
-        int j = (int)floor(rs / a.h + 0.5);
-        j = max(2, min(a.Nr - 2, j));
-        const double t = rs / a.h - (double)j;
-        // Lagrange basis on offsets -2..2
-        sLag[0 * KC + tid] = (t + 1.0) * t * (t - 1.0) * (t - 2.0) / 24.0;
-        sLag[1 * KC + tid] = -(t + 2.0) * t * (t - 1.0) * (t - 2.0) / 6.0;
-        sLag[2 * KC + tid] = (t + 2.0) * (t + 1.0) * (t - 1.0) * (t - 2.0) / 4.0;
-        sLag[3 * KC + tid] = -(t + 2.0) * (t + 1.0) * t * (t - 2.0) / 6.0;
-        sLag[4 * KC + tid] = (t + 2.0) * (t + 1.0) * t * (t - 1.0) / 24.0;
-        sJ[tid] = (rs > a.Nr * a.h) ? -1 : j;
+        int j;
+        if (a.rgrid) {
+            // non-uniform grid ("denser around the origin"): stencil centre = the nearest grid point (the lower one on a
+            // tie), by bisection; five-point Lagrange weights on the actual abscissae
+            int lo = 0, hi = a.Nr;                               // invariant: r[lo] <= rs (or lo == 0), r[hi] > rs (or hi == Nr)
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (a.rgrid[mid] <= rs) lo = mid; else hi = mid; }
+            j = (__dsub_rn(rs, a.rgrid[lo]) <= __dsub_rn(a.rgrid[hi], rs)) ? lo : hi;
+            j = max(2, min(a.Nr - 2, j));
+            double x[5];
+            #pragma unroll
+            for (int q = 0; q < 5; ++q) x[q] = a.rgrid[j - 2 + q];
+            #pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                double L = 1.0;
+                #pragma unroll
+                for (int c = 0; c < 5; ++c) if (c != q) L = L * (rs - x[c]) / (x[q] - x[c]);
+                sLag[q * KC + tid] = L;
+            }
+            sJ[tid] = (rs > a.rgrid[a.Nr]) ? -1 : j;
+        } else {
+            j = (int)floor(rs / a.h + 0.5);
+            j = max(2, min(a.Nr - 2, j));
+            const double t = rs / a.h - (double)j;
+            // Lagrange basis on offsets -2..2
+            sLag[0 * KC + tid] = (t + 1.0) * t * (t - 1.0) * (t - 2.0) / 24.0;
+            sLag[1 * KC + tid] = -(t + 2.0) * t * (t - 1.0) * (t - 2.0) / 6.0;
+            sLag[2 * KC + tid] = (t + 2.0) * (t + 1.0) * (t - 1.0) * (t - 2.0) / 4.0;
+            sLag[3 * KC + tid] = -(t + 2.0) * (t + 1.0) * t * (t - 2.0) / 6.0;
+            sLag[4 * KC + tid] = (t + 2.0) * (t + 1.0) * t * (t - 1.0) / 24.0;
+            sJ[tid] = (rs > a.Nr * a.h) ? -1 : j;
+        }
         sRinv[tid] = 1.0 / rs;
         sPot[tid] = -a.Zother[side] / ro;
         // Theta~_{lq}(c), q >= 0
@@ -708,6 +730,7 @@ struct TrotArgs {
     const TrotChunk *chunks; const int *rowbase;   // rowbase[b]: first local body row of radial function b inside its chunk
     int NT, NP, lmax, max_rows;
     double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex (p: window position)
+    double *KT; int ht;                      // optional K^T [p][NT][NP]; ht: write the H_PT, H_TP blocks of H^T instead of H
     // block z: evaluated position (fetch == 0): window position sel_pos(sel, q0 + z), integrals part[z];
     //          fetched position (fetch == 1): z = g * n_fetch + lf -> window position g * n_idx + n_pre + lf,
     //          integrals in stash slot g * n_st + slot0 + lf
@@ -740,7 +763,8 @@ __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
 //   times (-1)^q for q < 0 and (-1)^q' for q' < 0.
 __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     extern __shared__ __align__(16) double sd[];     // [lmax+1][W][W] Wigner d, W = 2 lmax + 1; then body rows [2][max_rows][nq8T] complex
-    const int prod = blockIdx.y, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
+    // blockIdx.y: 0 S_PT -> K, 1 H_PT, 2 H_TP, 3 (only with a.KT) S_PT once more -> K^T
+    const int yid = blockIdx.y, prod = yid == 3 ? 0 : yid, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
     const TrotChunk ch = a.chunks[blockIdx.x];
     int p; const double2 *part;              // window position (geometry, outputs) and its body-frame integrals
     {
@@ -814,8 +838,10 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     // stage 2: contract the projectile-side index
     const int NP = a.NP, N = NT + NP;
     for (int e = tid; e < ch.nst * NT; e += blockDim.x) {
-        // products 0, 1 are written row-major in (beta, alpha); product 2 (H_TP) in (alpha, beta): coalesced stores
-        const int ibl = (prod < 2) ? e / NT : e % ch.nst, ia = (prod < 2) ? e % NT : e / ch.nst;
+        // loop order = the order of the output rows (coalesced stores): K and H_PT row-major in (beta, alpha), H_TP and K^T in
+        // (alpha, beta); with a.ht the H blocks are written transposed (H^T is what the RK4 sweep streams), so the two swap
+        const bool beta_major = (yid == 0) || (yid == 1 && !a.ht) || (yid == 2 && a.ht);
+        const int ibl = beta_major ? e / NT : e % ch.nst, ia = beta_major ? e % NT : e / ch.nst;
         const int ib = ch.st0 + ibl;
         const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
         const double *dB = sd + (lb * W + mb + L) * W + L;
@@ -826,9 +852,10 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
             sr += dB[pq] * xp.x + dB[-pq] * xm.x; si += dB[pq] * xp.y + dB[-pq] * xm.y;
         }
         double *o;
-        if (prod == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
-        else if (prod == 1) o = a.H + (((size_t)p * N + NT + ib) * N + ia) * 2;            // H_PT
-        else { o = a.H + (((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
+        if (yid == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
+        else if (yid == 3) o = a.KT + (((size_t)p * NT + ia) * NP + ib) * 2;
+        else if (yid == 1) o = a.H + (a.ht ? ((size_t)p * N + ia) * N + NT + ib : ((size_t)p * N + NT + ib) * N + ia) * 2;             // H_PT
+        else { o = a.H + (a.ht ? ((size_t)p * N + NT + ib) * N + ia : ((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
         o[0] = sr; o[1] = si;
     }
 }
@@ -901,11 +928,12 @@ int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes) {
 }
 
 int wp_transfer_default_chunk(const wpccc_basis *B) {
-    // a multiple of the SM count (every tile CTA has the same work, so launches are whole waves), node tables <= 6 GB
+    // a multiple of the SM count (every tile CTA has the same work, so launches are whole waves), node tables <= 17 GB
+    // (configs[3]: 113 MB per position: 148 positions = 16.7 GB; halving the chunk leaves a ragged last wave)
     TransferPlan P = make_plan(B, 1);
     const size_t tab = (P.stride[0] + P.stride[1]) * 8;
     int c = 148;
-    while (c > 1 && (size_t)c * tab > ((size_t)6 << 30)) c /= 2;
+    while (c > 1 && (size_t)c * tab > ((size_t)17 << 30)) c /= 2;
     return c;
 }
 
@@ -917,7 +945,7 @@ bool wp_transfer_mirror_ok(const wpccc_basis *B) { return B->quad.kind == 0 && d
 
 int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_cos, const double *d_sin, const double *d_theta,
                 const double *d_v, double *d_K, double *d_H, void *ws, size_t ws_bytes, int chunk, cudaStream_t s,
-                const TransferSel *sel) {
+                const TransferSel *sel, double *d_KT) {
     if (n_pos <= 0) return 0;
     SelDev sd{0, 0, 0, 0};
     int n_eval = n_pos, n_fetch = 0;                 // evaluated positions of this call; fetched indices per group
@@ -961,7 +989,9 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     {
         const CentreTab &C = B->c[1];
         const size_t rot_fixed = rot_nd + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
-        const size_t rot_target = 48 * 1024;       // four CTAs per SM hide the staging latency (cfg 1: 36.8 ms at 100 KB, 26.6 ms at 48 KB)
+        // four CTAs per SM hide the staging latency (cfg 1: 36.8 ms at 100 KB, 26.6 ms at 48 KB; cfg 3: 395 ms per batch with
+        // one radial function per chunk at 48 KB, 459 ms with 16 body rows per chunk at 100 KB)
+        const size_t rot_target = 48 * 1024;
         const int cap = std::min(256, std::max(C.l_max + 1, (int)((rot_target - rot_fixed) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
         TrotChunk cur{0, 0, 0, 0, 0};
         for (int b = 0; b < C.n_rad; ++b) {
@@ -1021,7 +1051,8 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     tr.radT = B->c[0].d_st_rad; tr.lT_st = B->c[0].d_st_l; tr.mT_st = B->c[0].d_st_m;
     tr.radP = B->c[1].d_st_rad; tr.lP_st = B->c[1].d_st_l; tr.mP_st = B->c[1].d_st_m;
     tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
-    tr.lmax = lmx; tr.K = d_K; tr.H = d_H;
+    tr.lmax = lmx; tr.K = d_K; tr.H = d_H; tr.KT = d_KT; tr.ht = d_KT != nullptr;
+    const unsigned n_prod = d_KT ? 4 : 3;
     tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
     tr.sel = sd;
     for (int p0 = 0; p0 < n_eval; p0 += chunk) {
@@ -1035,7 +1066,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
             ts.eta_scale = B->quad.eta_scale; ts.out = d_pos; ts.wd = d_wd; ts.wd_stride = P.wd_stride; ts.q0 = p0;
             k_tpos_sph<<<dim3(P.L.n_rho, np), std::min(256, (P.L.n_z + 31) / 32 * 32), 0, s>>>(ts);
         } else k_tpos<<<np, 128, 0, s>>>(ta);
-        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R; tb.sel = sd; tb.q0 = p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC; tb.sph = sph;
+        TtabArgs tb{}; tb.L = P.L; tb.pos = d_pos; tb.R = d_R; tb.sel = sd; tb.q0 = p0; tb.h = B->h; tb.Nr = B->Nr; tb.KC = KC; tb.sph = sph; tb.rgrid = B->d_rgrid;
         for (int c = 0; c < 2; ++c) {
             tb.Ut[c] = B->c[c].d_Ut; tb.lrad[c] = B->c[c].d_l; tb.n_rad[c] = B->c[c].n_rad; tb.nf_pad[c] = B->c[c].nf_pad;
             tb.nq8[c] = P.nq8[c]; tb.ntile[c] = P.ntile[c]; tb.colidx[c] = d_colidx[c]; tb.out[c] = d_tab[c]; tb.pos_stride[c] = P.stride[c];
@@ -1068,7 +1099,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
 
         tr.part = d_part; tr.q0 = p0; tr.fetch = 0;
         wp_span_begin(B, FAM_ROT, s);
-        k_trot<<<dim3((unsigned)rchunks.size(), 3, np), 256, rot_smem, s>>>(tr);
+        k_trot<<<dim3((unsigned)rchunks.size(), n_prod, np), 256, rot_smem, s>>>(tr);
         wp_span_end(B, s, 1);
         B->units[FAM_ROT] += np;
         WP_CUDA(cudaGetLastError());
@@ -1080,7 +1111,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         for (int z0 = 0; z0 < total; z0 += 32768) {
             tr.q0 = z0;                      // fetch mode: first (g, lf) pair of this launch
             wp_span_begin(B, FAM_ROT, s);
-            k_trot<<<dim3((unsigned)rchunks.size(), 3, (unsigned)std::min(32768, total - z0)), 256, rot_smem, s>>>(tr);
+            k_trot<<<dim3((unsigned)rchunks.size(), n_prod, (unsigned)std::min(32768, total - z0)), 256, rot_smem, s>>>(tr);
             wp_span_end(B, s, 1);
             WP_CUDA(cudaGetLastError());
         }

@@ -335,3 +335,38 @@ def test_explicit_coupling_matrix(lib, one_centre, two_centre):
             So, Ho = assemble.S_and_H(prob, b[p], z[p], v[p])
             Mo = (-1j / v[p]) * np.linalg.solve(So, Ho)
             assert np.abs(M[p] - Mo).max() < 1e-12 + 1e-13 * np.abs(Mo).max() * np.linalg.cond(So), (p, np.abs(M[p] - Mo).max())
+
+
+def test_nonuniform_radial_grid(lib):
+    """wpccc_setup_basis_grid (radial grid denser around the origin): eq. (7) sums over the given
+    points, the node tables interpolate on the actual abscissae; elements (GEMM and table routes) and a propagation against
+    oracle/nonuniform.py, one and two centres."""
+    from oracle import nonuniform as nu
+    from wpccc_inputs.paper_shape import exponential_grid, resample_problem
+    g = exponential_grid(437, 40.0, 4.0)                                        # ragged Nr
+    for two in (False, True):
+        fine = tiny_problem(two, l_max=2, n_max=3, bins=2, k_max=2.0, Nr=2000, h=0.02, Z_P=2.0 if two else 1.0, quad=dict(QUAD) if two else None, seed=11 if two else None)
+        prob = resample_problem(fine, g)
+        basis = lib.setup_basis(prob)
+        pos = POS2 + [(0.03, 0.01, 1.0), (3.0, 38.5, 1.0)] if two else POS1      # incl. R below r_1-ish and nodes beyond r_max
+        b, z, v = map(np.array, zip(*pos))
+        S, H = lib.matrix_elements(basis, b, z, v, phases=True)
+        S, H = S.cpu().numpy(), H.cpu().numpy()
+        for p in range(len(b)):
+            So, Ho = nu.S_and_H_grid(prob, g, b[p], z[p], v[p])
+            assert_elements(S[p], So, "S on the non-uniform grid, position %d" % p)
+            assert_elements(H[p], Ho, "H on the non-uniform grid, position %d" % p)
+        if not two:
+            basis.enable_direct_tables(True)
+            _, Ht = lib.matrix_elements(basis, b, z, v, phases=True)
+            basis.enable_direct_tables(False)
+            for p in range(len(b)):
+                assert_elements(Ht[p].cpu().numpy(), nu.S_and_H_grid(prob, g, b[p], z[p], v[p])[1], "D^T (tables) on the non-uniform grid, position %d" % p)
+        bt, vt, n_steps = np.array([1.6, 0.9]), np.array([1.0, 1.3]), 30
+        basis.set_option("solve_route", 1)
+        Cg = lib.propagate(basis, bt, vt, -6.0, 6.0, n_steps).cpu().numpy()
+        h = 12.0 / n_steps
+        for t in range(2):
+            co = oprop.propagate(prob, bt[t], vt[t], -6.0, 6.0, n_steps, matrices=lambda i, t=t: nu.S_and_H_grid(prob, g, bt[t], -6.0 + 0.5 * i * h, vt[t]))
+            assert np.abs(Cg[t] - co).max() < PTOL, (two, t, np.abs(Cg[t] - co).max())
+        basis.close()
