@@ -145,7 +145,6 @@ size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, 
  *                           cond(A) 2^-53.
  *   "inverse_kernel"     solve_route 1 only: 0 automatic, 1 shared-memory kernel, 2 global-memory blocked kernel.
  *   "inverse_chunk_cols" solve_route 1, register kernel: stage K in chunks of this many columns (0 automatic).
- *   "sweep_cluster"      CTAs per thread-block cluster of the RK4 sweep (0 automatic; 1, 2, 4, 8).
  *   "timing"             1 (default) / 0: record the CUDA events behind wpccc_last_timing.
  * Returns 0 or WPCCC_EINVAL (unknown key, value out of range). */
 int wpccc_set_option(wpccc_basis *basis, const char *key, long long value);

@@ -176,8 +176,8 @@ __global__ void __launch_bounds__(256) k_direct_assemble(const AsmArgs a) {
     const int p = blockIdx.x, L = a.lambda_max, ldp = 2 * L + 1;
     if (threadIdx.x == 0) assoc_legendre_all(L, a.cosT[p], sP, ldp);
     __syncthreads();
-    const int idx = blockIdx.y * blockDim.x + threadIdx.x;
-    if (idx >= a.N * a.N) return;
+    const long long idx = ((long long)blockIdx.y * gridDim.z + blockIdx.z) * blockDim.x + threadIdx.x;    // element blocks over (y, z): more than 65 535 of them at N > 4 096
+    if (idx >= (long long)a.N * a.N) return;
     const int i = idx / a.N, j = idx % a.N;
     const int ap = a.st_rad[i], lp = a.st_l[i], mp = a.st_m[i];
     const int aa = a.st_rad[j], l = a.st_l[j], m = a.st_m[j];
@@ -403,7 +403,9 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
         WP_CUDA(cudaGetLastError());
         return 0;
     }
-    dim3 grid(n_pos, (C.n_states * C.n_states + 255) / 256);
+    const long long eb = ((long long)C.n_states * C.n_states + 255) / 256;
+    const unsigned gz = (unsigned)((eb + 65534) / 65535);
+    dim3 grid(n_pos, (unsigned)((eb + gz - 1) / gz), gz);
     wp_span_begin(B, FAM_DASM, s);
     k_direct_assemble<<<grid, 256, 0, s>>>(a);
     wp_span_end(B, s, 1);

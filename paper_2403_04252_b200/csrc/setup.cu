@@ -231,11 +231,11 @@ int describe(wpccc_basis &B, int n_centres, const wpccc_centre *centres, int Nr,
 
 __global__ void k_pair_products(const double *Ut, int nf_pad, int n_rad, const double *w, int Nr, int Kpad, double *PP) {
     // PP[pair(a1,a)][k-1] = w_k u_a1(r_k) u_a(r_k), k = 1..Nr; zero for k-1 >= Nr
-    const int pair = blockIdx.y;
+    const int pair = blockIdx.x;                     // pairs along x: there can be more than 65 535 of them
     int a1 = 0, rem = pair;
     while (rem >= n_rad - a1) { rem -= n_rad - a1; ++a1; }
     const int a = a1 + rem;
-    for (int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < Kpad; kk += gridDim.x * blockDim.x) {
+    for (int kk = blockIdx.y * blockDim.x + threadIdx.x; kk < Kpad; kk += gridDim.y * blockDim.x) {
         double v = 0.0;
         if (kk < Nr) { const double *row = Ut + (size_t)(kk + 1) * nf_pad; v = w[kk + 1] * row[2 * a1] * row[2 * a]; }
         PP[(size_t)pair * Kpad + kk] = v;
@@ -355,7 +355,7 @@ static int setup_impl(wpccc_basis **out, int n_centres, const wpccc_centre *cent
             }
         chk(upload(C.d_Ut, Ut, s));
         if (!rc) {
-            dim3 grid(std::min((B->Kpad + 255) / 256, 64), C.n_pairs);
+            dim3 grid(C.n_pairs, std::min((B->Kpad + 255) / 256, 64));
             k_pair_products<<<grid, 256, 0, s>>>(C.d_Ut, C.nf_pad, C.n_rad, d_w, Nr, B->Kpad, C.d_PP);
             if (cudaGetLastError() != cudaSuccess) { wp_set_error("k_pair_products launch failed"); rc = WPCCC_ECUDA; }
         }
@@ -425,7 +425,7 @@ void wp_timing_reset(wpccc_basis *B) {
 static const int k_sample_every[WP_NFAM] = {1, 1, 8, 8, 1, 1, 1, 1};
 void wp_span_begin(wpccc_basis *B, int fam, cudaStream_t s) {
     B->cur_fam = fam;
-    B->cur_sampled = (B->groups[fam]++ % k_sample_every[fam]) == 0;
+    B->cur_sampled = (B->groups[fam]++ % k_sample_every[fam]) == 0 && B->opt.timing;
     if (!B->cur_sampled) return;
     wpccc_basis::Span sp; sp.fam = fam; sp.a = take_event(B); sp.b = take_event(B);
     cudaEventRecord(sp.a, s);

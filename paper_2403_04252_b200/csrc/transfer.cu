@@ -731,6 +731,7 @@ struct TrotArgs {
     int NT, NP, lmax, max_rows;
     double *K; double *H;                    // K [p][NP][NT] complex; H [p][N][N] complex (p: window position)
     double *KT; int ht;                      // optional K^T [p][NT][NP]; ht: write the H_PT, H_TP blocks of H^T instead of H
+    int tb;                                  // target states per pass through stages 1 and 2
     // block z: evaluated position (fetch == 0): window position sel_pos(sel, q0 + z), integrals part[z];
     //          fetched position (fetch == 1): z = g * n_fetch + lf -> window position g * n_idx + n_pre + lf,
     //          integrals in stash slot g * n_st + slot0 + lf
@@ -780,8 +781,9 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     double2 *body = reinterpret_cast<double2 *>(sd + nd);
     const int nq8T = a.nq8T, NT = a.NT;
     const size_t blk = (size_t)a.nq8P * nq8T, fam_stride = (size_t)a.max_rows * nq8T;
-    double2 *Ep = body + 2 * fam_stride, *Em = Ep + (size_t)a.max_rows * NT;      // [rows][NT] each
-    int *s_colT = reinterpret_cast<int *>(Em + (size_t)a.max_rows * NT);          // [NT][L+1] column of (a, q) per target state
+    const int TB = a.tb;                                                          // target states per pass (NT unless shared memory is short)
+    double2 *Ep = body + 2 * fam_stride, *Em = Ep + (size_t)a.max_rows * TB;      // [rows][TB] each
+    int *s_colT = reinterpret_cast<int *>(Em + (size_t)a.max_rows * TB);          // [NT][L+1] column of (a, q) per target state
     {
         double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
         for (int e = tid; e < (L + 1) * W * W; e += blockDim.x) {
@@ -812,8 +814,12 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     // stage 1: contract the target-side index.  For body row (b, p = |q'|) and target state alpha = (a, m_a):
     //   P0 = sum_{q>=0} d^{l_a}_{m_a,q} F0[q],  M0 = sum_{q>0} (-1)^q d_{m_a,-q} F0[q],  P1, M1 the same with family (+),
     //   E+ = P0 + (p == 0 ? M0 : M1)            (q' = +p),      E- = (-1)^p (d_{m_a,0} F0[0] + P1 + M0)   (q' = -p < 0)
-    for (int e = tid; e < ch.nrows * NT; e += blockDim.x) {
-        const int r = e / NT, ia = e - r * NT, pq = s_rowp[r];
+    const int NP = a.NP, N = NT + NP;
+    for (int ia0 = 0; ia0 < NT; ia0 += TB) {
+    const int tbn = min(TB, NT - ia0);
+    if (ia0) __syncthreads();                                 // the previous pass is done with Ep, Em
+    for (int e = tid; e < ch.nrows * tbn; e += blockDim.x) {
+        const int r = e / tbn, ia = ia0 + (e - r * tbn), pq = s_rowp[r];
         const int la = a.lT_st[ia], ma = a.mT_st[ia];
         const double *dA = sd + (la * W + ma + L) * W + L;
         const double2 *f0 = body + (size_t)r * nq8T, *f1 = f0 + fam_stride;
@@ -836,19 +842,18 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     }
     __syncthreads();
     // stage 2: contract the projectile-side index
-    const int NP = a.NP, N = NT + NP;
-    for (int e = tid; e < ch.nst * NT; e += blockDim.x) {
+    for (int e = tid; e < ch.nst * tbn; e += blockDim.x) {
         // loop order = the order of the output rows (coalesced stores): K and H_PT row-major in (beta, alpha), H_TP and K^T in
         // (alpha, beta); with a.ht the H blocks are written transposed (H^T is what the RK4 sweep streams), so the two swap
         const bool beta_major = (yid == 0) || (yid == 1 && !a.ht) || (yid == 2 && a.ht);
-        const int ibl = beta_major ? e / NT : e % ch.nst, ia = beta_major ? e % NT : e / ch.nst;
+        const int ibl = beta_major ? e / tbn : e % ch.nst, ial = beta_major ? e % tbn : e / ch.nst, ia = ia0 + ial;
         const int ib = ch.st0 + ibl;
         const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
         const double *dB = sd + (lb * W + mb + L) * W + L;
-        const double2 *ep = Ep + (size_t)a.rowbase[rb] * NT + ia, *em = Em + (size_t)a.rowbase[rb] * NT + ia;
+        const double2 *ep = Ep + (size_t)a.rowbase[rb] * tbn + ial, *em = Em + (size_t)a.rowbase[rb] * tbn + ial;
         double sr = dB[0] * ep[0].x, si = dB[0] * ep[0].y;
         for (int pq = 1; pq <= lb; ++pq) {
-            const double2 xp = ep[pq * NT], xm = em[pq * NT];
+            const double2 xp = ep[pq * tbn], xm = em[pq * tbn];
             sr += dB[pq] * xp.x + dB[-pq] * xm.x; si += dB[pq] * xp.y + dB[-pq] * xm.y;
         }
         double *o;
@@ -857,6 +862,7 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
         else if (yid == 1) o = a.H + (a.ht ? ((size_t)p * N + ia) * N + NT + ib : ((size_t)p * N + NT + ib) * N + ia) * 2;             // H_PT
         else { o = a.H + (a.ht ? ((size_t)p * N + NT + ib) * N + ia : ((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
         o[0] = sr; o[1] = si;
+    }
     }
 }
 
@@ -992,7 +998,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         // four CTAs per SM hide the staging latency (cfg 1: 36.8 ms at 100 KB, 26.6 ms at 48 KB; cfg 3: 395 ms per batch with
         // one radial function per chunk at 48 KB, 459 ms with 16 body rows per chunk at 100 KB)
         const size_t rot_target = 48 * 1024;
-        const int cap = std::min(256, std::max(C.l_max + 1, (int)((rot_target - rot_fixed) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
+        const int cap = std::min(256, std::max(C.l_max + 1, (int)((rot_target > rot_fixed ? rot_target - rot_fixed : 0) / (2 * ((size_t)P.nq8[0] + B->c[0].n_states) * 16))));
         TrotChunk cur{0, 0, 0, 0, 0};
         for (int b = 0; b < C.n_rad; ++b) {
             if (cur.nrows + C.l[b] + 1 > cap) { rchunks.push_back(cur); cur = TrotChunk{b, b, C.rad_first[b], 0, 0}; }
@@ -1006,7 +1012,12 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     if (off > ws_bytes) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small");
     WP_CUDA(cudaMemcpyAsync(d_rchunks, rchunks.data(), rchunks.size() * sizeof(TrotChunk), cudaMemcpyHostToDevice, s));
     WP_CUDA(cudaMemcpyAsync(d_rowbase, rowbase.data(), rowbase.size() * sizeof(int), cudaMemcpyHostToDevice, s));
-    const size_t rot_smem = rot_nd + 2 * (size_t)rot_max_rows * ((size_t)P.nq8[0] + B->c[0].n_states) * 16 + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
+    // stages 1 and 2 of the rotation work on all N_T target states at once, or in passes of rot_tb states when the intermediate
+    // [rows][N_T] arrays would not fit (wide bases: the paper's two-centre l_max = 5, N_T = 955)
+    const size_t rot_base = rot_nd + 2 * (size_t)rot_max_rows * P.nq8[0] * 16 + (size_t)B->c[0].n_states * (lmx + 1) * 4 + 16;
+    int rot_tb = B->c[0].n_states;
+    while (rot_tb > 32 && rot_base + 2 * (size_t)rot_max_rows * rot_tb * 16 > 200 * 1024) rot_tb = (rot_tb + 1) / 2;
+    const size_t rot_smem = rot_base + 2 * (size_t)rot_max_rows * rot_tb * 16;
     if (rot_smem > 220 * 1024) WP_FAIL(WPCCC_EINVAL, "transfer: basis too large for the rotation kernel's shared memory");
     static PerDevice rot_attr;
     if (wp_raise(rot_attr, rot_smem)) WP_CUDA(cudaFuncSetAttribute(k_trot, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
@@ -1054,7 +1065,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     tr.lmax = lmx; tr.K = d_K; tr.H = d_H; tr.KT = d_KT; tr.ht = d_KT != nullptr;
     const unsigned n_prod = d_KT ? 4 : 3;
     tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
-    tr.sel = sd;
+    tr.sel = sd; tr.tb = rot_tb;
     for (int p0 = 0; p0 < n_eval; p0 += chunk) {
         const int np = std::min(chunk, n_eval - p0);
         TposArgs ta{}; ta.L = P.L; ta.R = d_R; ta.cosT = d_cos; ta.sinT = d_sin; ta.v = d_v; ta.sel = sd; ta.q0 = p0;

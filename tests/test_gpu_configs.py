@@ -54,7 +54,7 @@ def sample_positions(run, n_total, picks, seed):
     return b[perm], z[perm], v[perm], inv[:len(picks)]
 
 
-@pytest.mark.parametrize("idx,n_total,n_picks", [(0, 300, 6), (1, 150, 6), (3, 40, 2), (2, 260, 2)])
+@pytest.mark.parametrize("idx,n_total,n_picks", [(0, 300, 6), (1, 150, 6), (3, 40, 6), (2, 260, 6)])
 def test_T1_elements_at_config_size(lib, idx, n_total, n_picks):
     prob, basis = config(lib, idx)
     run = run_of(idx)
@@ -69,6 +69,30 @@ def test_T1_elements_at_config_size(lib, idx, n_total, n_picks):
         if two:
             assert_elements(S[p].cpu().numpy(), So, "configs[%d] S at pick %d" % (idx, k))
     del S, H
+
+
+@pytest.mark.parametrize("idx,n_pairs", [(1, 20), (3, 8)])
+def test_T1_lab_frame_definition_at_config_size(lib, idx, n_pairs):
+    """at two positions, seeded-random (beta, alpha) pairs of S_PT, H_PT, H_TP against L0, the lab-frame
+    definition (triple loop over the configured product nodes with lab-frame spherical harmonics at every node: no
+    rotation, no azimuthal factorisation), at the full size of the two-centre configs."""
+    from oracle import transfer as otr
+    prob, basis = config(lib, idx)
+    run = run_of(idx)
+    bs, v = run["b"], float(run["v"][0])
+    pos = [(bs[len(bs) // 2], -0.37), (bs[-1], 5.3)]
+    b, z = np.array([p[0] for p in pos]), np.array([p[1] for p in pos])
+    S, H = lib.matrix_elements(basis, b, z, np.full(2, v), phases=False)
+    S, H = S.cpu().numpy(), H.cpu().numpy()
+    T, P = prob.centres
+    stT, stP, NT = T.states(), P.states(), T.n_states
+    rng = np.random.default_rng(300 + idx)
+    for p in range(2):
+        for _ in range(n_pairs // 2):
+            ia, ib = int(rng.integers(len(stT))), int(rng.integers(len(stP)))
+            for kind, got in (("S", S[p][NT + ib, ia]), ("HPT", H[p][NT + ib, ia]), ("HTP", H[p][ia, NT + ib])):
+                ref = otr.lab_frame_element(prob, stP[ib], stT[ia], b[p], z[p], v, kind)
+                assert abs(got - ref) <= REL * abs(ref) + FLOOR, (idx, p, kind, ia, ib, got, ref)
 
 
 def test_T1_radial_entries_config2(lib):

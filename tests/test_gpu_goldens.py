@@ -73,3 +73,13 @@ def test_full_trajectories_match_the_oracle_goldens(lib, cfg):
         assert np.abs(np.abs(Cg[t]) ** 2 - np.abs(co) ** 2).max() < PTOL
         assert abs(drift[t] - do) < 1e-9 + 1e-3 * do, (cfg, t, drift[t], do)
     print("configs[%d]: %d full trajectories x %d RK4 steps, max |c_gpu - c_oracle| = %.3e" % (cfg, len(gs), n, worst))
+    if len(prob.centres) == 2:
+        # the explicit-inverse route of the overlap solve (wpccc_set_option "solve_route" 1) on the same trajectories
+        basis.set_option("solve_route", 1)
+        try:
+            Ci = lib.propagate(basis, b, v, z0, z1, n).cpu().numpy()
+        finally:
+            basis.set_option("solve_route", 0)
+        worst_i = max(np.abs(Ci[t] - g["C"]).max() for t, g in enumerate(gs))
+        assert worst_i < PTOL
+        print("configs[%d]: explicit Gauss-Jordan inverse route: max |c_gpu - c_oracle| = %.3e (Cholesky + triangular solves: %.3e)" % (cfg, worst_i, worst))
