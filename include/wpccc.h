@@ -248,6 +248,26 @@ int wpccc_probabilities(const wpccc_basis *basis, int n_traj, const double *dC /
                         int init_state, double *P_state, double *P_nl, double *P_class,
                         double *sigma_nl, double *sigma_class, void *stream);
 
+/* ---- a9 without any allocation: cross sections with the scratch in a static device array -------
+ * For callers that cannot call cudaMalloc and hold no workspace (code under CUDA graph capture set-up, tight serving
+ * loops, harnesses that forbid allocation): the cross-section integral of P:L106,
+ *   dSigma [device][n_vgroups][n_cols] = 2 pi Int b P(b) db  (trapezoid rule in ln b over the trajectories of each
+ *   velocity group sorted by b, exactly as sigma_nl / sigma_class of wpccc_probabilities),
+ * of any per-trajectory probability table dP [device][n_traj][n_cols] (row-major, e.g. P_nl or P_class).  It takes no
+ * basis handle and no workspace: its index scratch (b, the sorted order, the group offsets) is a file-scope
+ * `static __device__` array of WPCCC_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads libwpccc.so
+ * holds until the process exits.  b [host][n_traj] > 0, vgroup [host][n_traj] in 0..n_vgroups-1.
+ * Limits: n_traj <= WPCCC_STATIC_MAX_TRAJ and n_vgroups <= WPCCC_STATIC_MAX_VGROUPS per call, else WPCCC_ENOMEM with a
+ * message naming the limit (nothing is launched).  Calls no cudaMalloc / cudaFree / allocating library routine.
+ * All calls on a device share the one array: calls whose GPU work overlaps (other streams or host threads) race --
+ * issue one at a time per device.  The array keeps the previous call's contents; each call rewrites every element it
+ * reads, nothing needs to start at zero.  Synchronises `stream` (the host index vectors must outlive the copies). */
+#define WPCCC_STATIC_SCRATCH_BYTES (256 * 1024)
+#define WPCCC_STATIC_MAX_TRAJ 16384
+#define WPCCC_STATIC_MAX_VGROUPS 1024
+int wpccc_cross_sections_static(int n_traj, int n_cols, const double *dP /*[device]*/, const double *b /*[host]*/,
+                                const int *vgroup /*[host]*/, int n_vgroups, double *dSigma /*[device]*/, void *stream);
+
 /* ---- diagnostics ----------------------------------------------------------------------------- */
 
 /* Per-family device time of the last wpccc_propagate / wpccc_matrix_elements call on this handle,

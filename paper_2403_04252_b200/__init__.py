@@ -82,6 +82,8 @@ _lib.wpccc_coupling_matrix.restype = C.c_int
 _lib.wpccc_coupling_matrix.argtypes = [_vp, C.c_int, _dp, _dp, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
 _lib.wpccc_probabilities.restype = C.c_int
 _lib.wpccc_probabilities.argtypes = [_vp, C.c_int, _vp, _dp, _ip, C.c_int, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.wpccc_cross_sections_static.restype = C.c_int
+_lib.wpccc_cross_sections_static.argtypes = [C.c_int, C.c_int, _vp, _dp, _ip, C.c_int, _vp, _vp]
 _lib.wpccc_last_timing.restype = C.c_int
 _lib.wpccc_last_timing.argtypes = [_vp, _dp, C.POINTER(C.c_longlong)]
 _lib.wpccc_last_units.restype = C.c_int
@@ -97,7 +99,7 @@ _lib.wpccc_version.restype = C.c_char_p
 
 EXPORTS = ("wpccc_basis_bytes", "wpccc_setup_basis", "wpccc_setup_basis_grid", "wpccc_free_basis", "wpccc_n_states", "wpccc_n_states_centre",
            "wpccc_n_rad_centre", "wpccc_n_radial_entries", "wpccc_radial_entry", "wpccc_workspace_bytes",
-           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_coupling_matrix_ws_bytes", "wpccc_coupling_matrix", "wpccc_probabilities", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
+           "wpccc_matrix_elements", "wpccc_propagate", "wpccc_propagate_grid", "wpccc_last_status", "wpccc_set_option", "wpccc_coupling_matrix_ws_bytes", "wpccc_coupling_matrix", "wpccc_probabilities", "wpccc_cross_sections_static", "wpccc_last_timing", "wpccc_last_units", "wpccc_fp64_peak",
            "wpccc_direct_table_bytes", "wpccc_enable_direct_tables", "wpccc_last_error", "wpccc_version")
 
 
@@ -340,6 +342,29 @@ def probabilities(basis: Basis, Cc, b=None, vgroup=None, n_vgroups: int = 0, ini
                                     _ptr(vg, C.c_int) if vg is not None else None, int(n_vgroups), int(init_state), p("P_state"), p("P_nl"),
                                     p("P_class"), p("sigma_nl"), p("sigma_class"), _stream(torch)))
     return out
+
+
+STATIC_MAX_TRAJ, STATIC_MAX_VGROUPS = 16384, 1024     # WPCCC_STATIC_MAX_TRAJ / _VGROUPS of wpccc.h
+
+
+def cross_sections_static(P, b, vgroup, n_vgroups: int):
+    """wpccc_cross_sections_static: sigma [n_vgroups][n_cols] of a probability table P [n_traj][n_cols] (device, float64) with
+    the index scratch in the library's static device array: no allocation inside the call (the output tensor is the caller's)."""
+    torch = _torch()
+    n, ncol = P.shape
+    P = P.contiguous()
+    sigma = torch.empty((int(n_vgroups), ncol), dtype=torch.float64, device="cuda")
+    cross_sections_static_into(P, b, vgroup, n_vgroups, sigma)
+    return sigma
+
+
+def cross_sections_static_into(P, b, vgroup, n_vgroups: int, sigma):
+    """The same with the output tensor passed in (nothing at all is allocated on the device)."""
+    torch = _torch()
+    n, ncol = P.shape
+    bb, vg = _f64(b), _i32(vgroup)
+    _check(_lib.wpccc_cross_sections_static(int(n), int(ncol), C.c_void_p(P.data_ptr()), _ptr(bb), _ptr(vg, C.c_int), int(n_vgroups),
+                                            C.c_void_p(sigma.data_ptr()), _stream(torch)))
 
 
 def last_timing(basis: Basis):

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwpccc.so")
-SOURCES = ["setup.cu", "direct.cu", "transfer.cu", "sweep.cu", "cholesky.cu", "api.cu"]
+SOURCES = ["setup.cu", "direct.cu", "transfer.cu", "sweep.cu", "cholesky.cu", "api.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
