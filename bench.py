@@ -122,7 +122,9 @@ def family_work(prob, b_local, n_steps, units=None):
             for a1 in range(len(l)):
                 ok = (np.abs(l[a1] - l[a1:]) <= lam) & (lam <= l[a1] + l[a1:]) & (((l[a1] + l[a1:] + lam) % 2) == 0)
                 E += int(ok.sum())
-    out = {"direct_gemm": ("tensor", 2.0 * prob.Nr * E * n_pos, "flop")}
+    # a z-grid symmetric about 0: F(R) is contracted once per mirror pair (b, -z), (b, +z) (wpccc_last_units)
+    n_gemm = (units or {}).get("direct_gemm") or n_pos
+    out = {"direct_gemm": ("tensor", 2.0 * prob.Nr * E * n_gemm, "flop")}
     if two:
         q = prob.quad
         nodes = q["n_rho"] * q["n_z"]
@@ -419,6 +421,17 @@ def run_ours(args):
                                     "workload": j2.describe(), "dominant": d2, "frac": f2[d2]["frac"], "kernel_families": f2,
                                     "matrix_elements_per_s": round(elements_per_position(j2.prob) * len(j2.b_all) * (2 * j2.n_steps + 1) / (ms2 * 1e-3), 1)}
             line["gpu_launches"] += int(ln2)
+            if cfg in (2, 4):
+                # the same job with the radial sums of eq. (7) read from prefix/suffix tables instead of the
+                # DMMA GEMM (wpccc_enable_direct_tables; exact, parity-tested): the step is then bound by the RK4 sweep
+                j2.basis.enable_direct_tables(True)
+                ms3, fam3, ln3, un3, _ = measure(j2, torch, dist, 1, 1, 2, flush)
+                f3 = families(j2, fam3, 2, un3, pk, dmma, dfma, direct_tables=True)
+                d3 = max(f3, key=lambda k: f3[k]["ms_per_step"])
+                per_config[str(cfg)]["table_route"] = {"value": round(len(j2.b_all) * j2.n_steps / (ms3 * 1e-3), 3), "ms_per_step": round(ms3, 3), "steps": 2, "warmup": 1,
+                                                       "direct": "prefix/suffix tables (NEXT-1)", "dominant": d3, "frac": f3[d3]["frac"], "kernel_families": f3}
+                line["gpu_launches"] += int(ln3)
+                j2.basis.enable_direct_tables(False)
             j2.close()
             del j2
             wp.release_workspace()

@@ -132,7 +132,8 @@ size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, 
  * Selects between CUDA routes that compute the same thing (never a CPU path); takes effect from the
  * next call on this handle.  Keys:
  *   "mirror_pairs"       1 (default) / 0: on a z-grid symmetric about 0, evaluate the body-frame integrals of
- *                        eq. (9) at (b, -z) and (b, +z) together (see wpccc_last_units).
+ *                        eq. (9) at (b, -z) and (b, +z) together, and the direct radial entries of eq. (7), which
+ *                        depend on the position through R only, once per pair (see wpccc_last_units).
  *   "solve_route"        how S(R) x = y is solved in every RK4 stage (role of ZGESV), with
  *                        S = [[I, K^H], [K, I]] reduced to its Schur complement A = I - K K^H (Hermitian,
  *                        positive definite whenever S is):
@@ -278,12 +279,18 @@ int wpccc_cross_sections_static(int n_traj, int n_cols, const double *dP /*[devi
 int wpccc_last_timing(const wpccc_basis *basis, double *ms /*[host][8]*/, long long *launches /*[host][8]*/);
 
 /* Positions processed by each family (same order) in the last wpccc_propagate / wpccc_matrix_elements
- * call, for the families that count them (2 node tables, 3 contraction, 4 rotation; 0 otherwise).
+ * call, for the families that count them (0 direct GEMM / tables in wpccc_propagate, 2 node tables,
+ * 3 contraction, 4 rotation; 0 otherwise).
  * wpccc_propagate on a z-grid symmetric about 0 (z_min = -z_max) evaluates the body-frame integrals of
  * eq. (9) once per mirror pair (b, -z), (b, +z) -- they differ only by the complex conjugation of the
  * axial phase -- as far as the workspace beyond wpccc_workspace_bytes(.., 2) can hold the second
  * member's integrals until the sweep reaches it; units[3] is then smaller
- * than the number of positions.  wpccc_set_option(basis, "mirror_pairs", 0) disables this.
+ * than the number of positions.  The direct radial entries F^c_lambda(a', a; R) of eq. (7) are the same at
+ * (b, -z) and (b, +z) (same R): on such a grid, when the workspace can hold F of the half-step positions up to
+ * z = 0 of every distinct b ((n_steps + 1) x n_entries doubles each; included in wpccc_workspace_bytes(.., 1)
+ * up to its cap), the contraction of a2 runs for z <= 0 only and units[0] is about half the positions; the
+ * assembly a3 (which differs through P_lambda^mu(cos Theta)) runs everywhere.
+ * wpccc_set_option(basis, "mirror_pairs", 0) disables both.
  * Returns the number of families (8) or WPCCC_EINVAL. */
 int wpccc_last_units(const wpccc_basis *basis, long long *units /*[host][8]*/);
 

@@ -131,12 +131,43 @@ GeomOut carve_geom(Carver &cv, size_t n) {
 }
 
 // elements of one block of positions (geometry already on the device): F, then H0 / K (two-centre) or Dre (one-centre)
+// Mirror of the direct radial entries on a z-grid symmetric about 0: F^c_lambda(a', a; R) of eq. (7) depends on the position
+// through R = |R| only, so (b, -z) and (b, +z) share it.  F then lives in a per-group table over the half-step positions up to
+// z = 0 ([group][n_steps + 1][E_tot], PosMap fold): the GEMM runs for the first n_gemm_idx positions of a window only (those
+// with z <= 0) and the assembly (which differs between -z and +z through P_lambda^mu(cos Theta)) reads the folded row.
+struct DirectMirror { double *F; int n_gemm_idx; PosMap rmap, fmap_gemm, fmap_asm; };
+DirectMirror direct_mirror(double *d_Fst, int n_steps, long long i0, int n_idx) {
+    DirectMirror m{};
+    m.F = d_Fst;
+    m.n_gemm_idx = (int)std::max<long long>(0, std::min<long long>(n_idx, (long long)n_steps + 1 - i0));
+    m.rmap = PosMap{m.n_gemm_idx, n_idx, 0, -1};
+    m.fmap_gemm = PosMap{m.n_gemm_idx, n_steps + 1, (int)i0, 2 * n_steps};
+    m.fmap_asm = PosMap{n_idx, n_steps + 1, (int)i0, 2 * n_steps};
+    return m;
+}
+// F of a window of n_groups x n_idx positions: plain (d_F [n_pos][E_tot]) or through the mirror table; *F_out, *fmap_out are
+// what the assembly reads
+int direct_entries(wpccc_basis *B, int n_groups, int n_idx, const double *d_R, double *d_F, const DirectMirror *dm, cudaStream_t s,
+                   const double **F_out, const PosMap **fmap_out) {
+    if (!dm) {
+        B->units[FAM_GEMM] += (long long)n_groups * n_idx;
+        *F_out = d_F; *fmap_out = nullptr;
+        return wp_direct_gemm(B, n_groups * n_idx, d_R, d_F, B->E_tot, s);
+    }
+    *F_out = dm->F; *fmap_out = &dm->fmap_asm;
+    if (dm->n_gemm_idx == 0) return 0;
+    B->units[FAM_GEMM] += (long long)n_groups * dm->n_gemm_idx;
+    return wp_direct_gemm(B, n_groups * dm->n_gemm_idx, d_R, dm->F, B->E_tot, s, &dm->rmap, &dm->fmap_gemm);
+}
+
 int elements_two_centre(wpccc_basis *B, int n_pos, const GeomOut &g, double *d_F, double *d_K, double *d_H, void *tws, size_t tws_bytes,
-                        int chunk, cudaStream_t s, const TransferSel *sel = nullptr, double *d_KT = nullptr) {
+                        int chunk, cudaStream_t s, const TransferSel *sel = nullptr, double *d_KT = nullptr,
+                        const DirectMirror *dm = nullptr, int n_idx = 0) {
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
-    int rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, s); if (rc) return rc;
-    rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_H, N, (long long)N * N, 1, s); if (rc) return rc;
-    rc = wp_direct_assemble(B, 1, n_pos, g.cosT, d_F, B->E_tot, d_H + ((size_t)NT * N + NT) * 2, N, (long long)N * N, 1, s); if (rc) return rc;
+    const double *F = d_F; const PosMap *fm = nullptr;
+    int rc = direct_entries(B, dm ? n_pos / n_idx : n_pos, dm ? n_idx : 1, g.R, d_F, dm, s, &F, &fm); if (rc) return rc;
+    rc = wp_direct_assemble(B, 0, n_pos, g.cosT, F, B->E_tot, d_H, N, (long long)N * N, 1, s, fm); if (rc) return rc;
+    rc = wp_direct_assemble(B, 1, n_pos, g.cosT, F, B->E_tot, d_H + ((size_t)NT * N + NT) * 2, N, (long long)N * N, 1, s, fm); if (rc) return rc;
     return wp_transfer(B, n_pos, g.R, g.cosT, g.sinT, g.theta, g.v, d_K, d_H, tws, tws_bytes, chunk, s, sel, d_KT);    // d_KT: H^T and K^T for the sweep
 }
 
@@ -192,6 +223,11 @@ extern "C" size_t wpccc_workspace_bytes(const wpccc_basis *B, int n_traj, int n_
     if (what == 2) return plan_bytes(P, 1);
     const int W = preferred_window(P, n_steps, WS_PREFERRED_CAP);
     size_t tot = plan_bytes(P, W);
+    if (B->opt.mirror_pairs) {
+        // mirror table of the direct radial entries (z-grid symmetric about 0): F of the half-step positions up to z = 0
+        const size_t fs = align256((size_t)n_traj * ((size_t)std::max(n_steps, 1) + 1) * (size_t)B->E_tot * 8) + 8192;
+        if (tot + fs <= WS_PREFERRED_CAP) tot += fs;
+    }
     if (P.two && W == std::min(std::max(n_steps, 1), 64) && wp_transfer_mirror_ok(B) && B->opt.mirror_pairs) {
         // mirror stash: the body-frame integrals of the n_steps half-step positions beyond z = 0 of
         // every trajectory, as far as the total stays within WS_PREFERRED_CAP (then only the positions next to z = 0 are paired:
@@ -325,7 +361,25 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
     const int n_groups = two ? n_traj : (int)ub.size();
     PropPlan P = plan_propagate(B, n_traj, n_groups, (int)units.size(), n_steps);
     if (ws_bytes < plan_bytes(P, 1)) WP_FAIL(WPCCC_ENOMEM, "workspace too small: need at least %zu bytes", plan_bytes(P, 1));
-    const int W = preferred_window(P, n_steps, ws_bytes);
+    // z-grid symmetric about 0 (z_k = -z_{2n-k} for the half-step positions): mirror pairs (b, -z), (b, +z)
+    bool sym_grid = B->opt.mirror_pairs != 0;
+    if (sym_grid) {
+        double zmax = 0.0;
+        for (double z : zh) zmax = std::max(zmax, std::fabs(z));
+        for (size_t k = 0; k < zh.size() && sym_grid; ++k) if (std::fabs(zh[k] + zh[zh.size() - 1 - k]) > 1e-14 * zmax) sym_grid = false;
+    }
+    // mirror table of the direct radial entries (DirectMirror above): [group][n_steps + 1][E_tot], all or nothing; the window is
+    // shortened (not below 16 steps) if that is what it takes to hold it
+    size_t fst_bytes = 0;
+    int W = 0;
+    if (sym_grid) {
+        const size_t want = align256((size_t)n_groups * ((size_t)n_steps + 1) * (size_t)B->E_tot * 8) + 4096;
+        if (ws_bytes > want && ws_bytes - want >= plan_bytes(P, 1)) {
+            const int Wm = preferred_window(P, n_steps, ws_bytes - want);
+            if (Wm >= std::min(n_steps, 16)) { fst_bytes = want; W = Wm; }
+        }
+    }
+    if (!fst_bytes) W = preferred_window(P, n_steps, ws_bytes);
     const int n_idx_max = 2 * W + 1;
 
     Carver cv(ws, ws_bytes);
@@ -347,16 +401,12 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
             d_LU[k] = cv.take<double>(npos_max * wp_factor_elems((int)NP) * 2); d_flags[k] = cv.take<int>(npos_max);
         } else d_D[k] = cv.take<double>(npos_max * N * ldD);
     }
+    double *d_Fst = fst_bytes ? cv.take<double>((fst_bytes - 4096) / 8) : nullptr;
     if (!cv.ok) WP_FAIL(WPCCC_ENOMEM, "workspace too small (internal plan mismatch)");
     // Mirror stash: on a z-grid symmetric about 0 the body-frame two-centre integrals at (b, +z) are written by the
     // launch that evaluates (b, -z) (TransferSel, common.cuh); whatever the workspace has left beyond the window
     // buffers holds the n_st half-step positions per trajectory that follow z = 0.
-    bool symmetric = two && B->opt.mirror_pairs && wp_transfer_mirror_ok(B);
-    if (symmetric) {
-        double zmax = 0.0;
-        for (double z : zh) zmax = std::max(zmax, std::fabs(z));
-        for (size_t k = 0; k < zh.size() && symmetric; ++k) if (std::fabs(zh[k] + zh[zh.size() - 1 - k]) > 1e-14 * zmax) symmetric = false;
-    }
+    const bool symmetric = two && sym_grid && wp_transfer_mirror_ok(B);
     TransferSel sel{}; bool mirror = false;
     if (symmetric) {
         const size_t slot = wp_transfer_stash_doubles(B) * 8, left = ws_bytes > cv.off + 4096 ? ws_bytes - cv.off - 4096 : 0;
@@ -397,6 +447,8 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
         wp_span_begin(B, FAM_OTHER, e);
         k_geometry_grid<<<(n_pos + 127) / 128, 128, 0, e>>>(n_groups, n_idx, d_b, two ? d_v : nullptr, d_zh + i0, g);
         wp_span_end(B, e, 1);
+        const DirectMirror dmir = direct_mirror(d_Fst, n_steps, i0, n_idx);
+        const DirectMirror *dm = d_Fst ? &dmir : nullptr;
         if (two) {
             // no clearing of d_H[buf]: the assembly kernels write every element of D^T, D^P and the rotation kernel every
             // element of H_PT, H_TP at every position of the window (evaluated or fetched from the mirror stash)
@@ -405,12 +457,13 @@ int propagate_impl(wpccc_basis *B, int n_traj, const double *b, const double *v,
                 sel.n_pre = (int)std::max<long long>(0, std::min<long long>(n_idx, sel.i_mid + 1 - i0));
                 sel.suf0 = (int)std::max<long long>(sel.n_pre, std::min<long long>(n_idx, sel.i_mid + sel.n_st + 1 - i0));
             }
-            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e, mirror ? &sel : nullptr, d_KT[buf]);
+            rc = elements_two_centre(B, n_pos, g, d_F, d_K[buf], d_H[buf], tws, P.tws, tchunk, e, mirror ? &sel : nullptr, d_KT[buf], dm, n_idx);
             if (!rc) cu(cudaMemsetAsync(d_flags[buf], 0, (size_t)n_pos * sizeof(int), e), "clear flags");
             if (!rc) rc = wp_factor(B, n_pos, d_K[buf], d_LU[buf], d_flags[buf], d_fscratch, e);
         } else {
-            rc = wp_direct_gemm(B, n_pos, g.R, d_F, B->E_tot, e);
-            if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, d_F, B->E_tot, d_D[buf], ldD, (long long)N * ldD, 0, e);
+            const double *F = d_F; const PosMap *fm = nullptr;
+            rc = direct_entries(B, n_groups, n_idx, g.R, d_F, dm, e, &F, &fm);
+            if (!rc) rc = wp_direct_assemble(B, 0, n_pos, g.cosT, F, B->E_tot, d_D[buf], ldD, (long long)N * ldD, 0, e, fm);
         }
         if (rc) break;
         if (!cu(cudaEventRecord(ev_elem[buf], e), "record") || !cu(cudaStreamWaitEvent(sw, ev_elem[buf], 0), "wait for the elements")) break;

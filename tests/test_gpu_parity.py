@@ -125,6 +125,41 @@ def test_one_centre_windows_do_not_change_the_result(lib, one_centre):
     assert np.abs(big - small).max() < 1e-14
 
 
+def test_one_centre_mirror_of_the_radial_entries(lib, one_centre):
+    """On a z-grid symmetric about 0 the direct radial entries F(R) of eq. (7) are contracted for z <= 0 only and reused at
+    +z (same R; wpccc.h, wpccc_last_units): several windows (150 steps > 64), repeated b, GEMM and table routes, against the
+    run with the mirror switched off and against the oracle; an asymmetric grid switches it off by itself."""
+    prob, basis = one_centre
+    b, v = np.array([0.6, 2.0, 0.6]), np.array([1.0, 1.3, 0.8])          # two distinct b
+    n_steps = 150
+    n_pos = 2 * (2 * n_steps + 3)          # windows of 64, 64, 22 steps; consecutive windows share their boundary position
+    Cm = lib.propagate(basis, b, v, -12.0, 12.0, n_steps).cpu().numpy()
+    assert lib.last_units(basis)["direct_gemm"] == 2 * (n_steps + 2), lib.last_units(basis)
+    small_ws = lib._lib.wpccc_workspace_bytes(basis._h, 3, n_steps, 2) + (1 << 20)                 # short windows
+    Cs = lib.propagate(basis, b, v, -12.0, 12.0, n_steps, ws_bytes=small_ws).cpu().numpy()
+    assert lib.last_units(basis)["direct_gemm"] >= 2 * (n_steps + 2)                               # short windows, with or without the table
+    basis.set_option("mirror_pairs", 0)
+    try:
+        C0 = lib.propagate(basis, b, v, -12.0, 12.0, n_steps).cpu().numpy()
+        assert lib.last_units(basis)["direct_gemm"] == n_pos
+    finally:
+        basis.set_option("mirror_pairs", 1)
+    assert np.abs(Cm - C0).max() < 1e-13 and np.abs(Cs - C0).max() < 1e-13, (np.abs(Cm - C0).max(), np.abs(Cs - C0).max())
+    for t in (0, 1):
+        co = oprop.propagate(prob, b[t], v[t], -12.0, 12.0, n_steps)
+        assert np.abs(Cm[t] - co).max() < PTOL
+    basis.enable_direct_tables(True)
+    try:
+        Ct = lib.propagate(basis, b, v, -12.0, 12.0, n_steps).cpu().numpy()
+        assert lib.last_units(basis)["direct_gemm"] == 2 * (n_steps + 2)
+    finally:
+        basis.enable_direct_tables(False)
+    assert np.abs(Ct - C0).max() < 1e-11
+    Ca = lib.propagate(basis, b[:1], v[:1], -6.0, 4.0, 25).cpu().numpy()
+    assert lib.last_units(basis)["direct_gemm"] == 51
+    assert np.abs(Ca[0] - oprop.propagate(prob, b[0], v[0], -6.0, 4.0, 25)).max() < PTOL
+
+
 # ------------------------------------------------------------------------------------------------ two centres
 QUAD = dict(n_rho=24, n_phi=8, n_z=48, rho_max=30.0, z_pad=30.0, phi_rule=0)
 POS2 = [(1.3, -0.8, 1.0), (0.4, 2.2, 1.5), (2.5, 0.0, 0.8), (0.2, -6.0, 1.0)]
@@ -199,6 +234,7 @@ def test_two_centre_mirror_pairs(lib, two_centre):
     Cm = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
     um = lib.last_units(basis)
     assert um["transfer_contraction"] == 3 * (n_steps + 2) and um["rotation"] == n_pos, um       # z <= 0 evaluated, z > 0 fetched
+    assert um["direct_gemm"] == 3 * (n_steps + 2), um                                            # F(R) of eq. (7): the same at -z and +z
     base = lib._lib.wpccc_workspace_bytes(basis._h, 3, n_steps, 1)
     part = lib._lib.wpccc_workspace_bytes(basis._h, 3, 64, 1)                                   # room for 64 of the 150 mirror indices
     Cp = lib.propagate(basis, b, v, -9.0, 9.0, n_steps, ws_bytes=part).cpu().numpy()
@@ -207,7 +243,7 @@ def test_two_centre_mirror_pairs(lib, two_centre):
     basis.set_option("mirror_pairs", 0)
     try:
         C0 = lib.propagate(basis, b, v, -9.0, 9.0, n_steps).cpu().numpy()
-        assert lib.last_units(basis)["transfer_contraction"] == n_pos
+        assert lib.last_units(basis)["transfer_contraction"] == n_pos and lib.last_units(basis)["direct_gemm"] == n_pos
     finally:
         basis.set_option("mirror_pairs", 1)
     assert np.abs(Cm - C0).max() < 1e-12 and np.abs(Cp - C0).max() < 1e-12, (np.abs(Cm - C0).max(), np.abs(Cp - C0).max())
