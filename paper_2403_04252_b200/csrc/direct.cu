@@ -213,7 +213,91 @@ struct Asm2Args {
     PosMap fmap;
 };
 
-__global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
+// One column j of D over a run of radial functions a_i = a0 .. a1-1 that share l_i (2 l_i + 1 rows each, CNT multipoles
+// lambda = lam0, lam0 + 2, .. with this column's l_j), rows mi0 .. mi0 + NMB - 1 of every a_i: the angular factors ang[m_i][k]
+// are the same for the whole run and live in registers; per a_i the CNT values F_lambda(a_i, a_j) come from the staged F.
+// `ang`, `o` point at row mi0 of the run's first radial function; blockstride = (2 l_i + 1) ostride.
+template <int CNT, int NMB, bool CPLX>
+__device__ __forceinline__ void asm_run(const double *sF, const int *sOff, const double *ang, int nlm, int nlm2, int a0, int a1, int aj,
+                                        int colbase, int n_rad, double *o, size_t ostride, size_t blockstride) {
+    double av[NMB][CNT];
+    #pragma unroll
+    for (int mi = 0; mi < NMB; ++mi)
+        #pragma unroll
+        for (int k = 0; k < CNT; ++k) av[mi][k] = ang[mi * nlm + k * nlm2];
+    int rowbase = a0 * n_rad - a0 * (a0 - 1) / 2 - a0;                            // pair(a_i, a_j) - a_j for a_i <= a_j
+    #pragma unroll 1
+    for (int ai = a0; ai < a1; ++ai) {
+        const double *f = sF + sOff[(ai <= aj) ? rowbase + aj : colbase + ai];
+        double fv[CNT];
+        #pragma unroll
+        for (int k = 0; k < CNT; ++k) fv[k] = f[k];
+        double *oo = o;
+        #pragma unroll
+        for (int mi = 0; mi < NMB; ++mi) {
+            double acc = av[mi][0] * fv[0];
+            #pragma unroll
+            for (int k = 1; k < CNT; ++k) acc = fma(av[mi][k], fv[k], acc);
+            if (CPLX) *reinterpret_cast<double2 *>(oo) = make_double2(acc, 0.0); else *oo = acc;
+            oo += ostride;
+        }
+        o += blockstride;
+        rowbase += n_rad - ai - 1;
+    }
+}
+// the same for any number of multipoles and rows (angular factors read from shared memory)
+template <bool CPLX>
+__device__ __forceinline__ void asm_run_any(const double *sF, const int *sOff, const double *ang, int nlm, int nlm2, int cnt, int nmb, int a0, int a1,
+                                            int aj, int colbase, int n_rad, double *o, size_t ostride, size_t blockstride) {
+    int rowbase = a0 * n_rad - a0 * (a0 - 1) / 2 - a0;
+    for (int ai = a0; ai < a1; ++ai) {
+        const double *f = sF + sOff[(ai <= aj) ? rowbase + aj : colbase + ai];
+        double *oo = o;
+        for (int mi = 0; mi < nmb; ++mi) {
+            double acc = 0.0;
+            for (int k = 0; k < cnt; ++k) acc = fma(ang[mi * nlm + k * nlm2], f[k], acc);
+            if (CPLX) *reinterpret_cast<double2 *>(oo) = make_double2(acc, 0.0); else *oo = acc;
+            oo += ostride;
+        }
+        o += blockstride;
+        rowbase += n_rad - ai - 1;
+    }
+}
+#define WP_ASM_ARGS sF, sOff, ang, nlm, nlm2, a0, a1, aj, colbase, n_rad, o, ostride, blockstride
+template <int NMB, bool CPLX>
+__device__ __forceinline__ void asm_run_rows(int cnt, const double *sF, const int *sOff, const double *ang, int nlm, int nlm2, int a0, int a1, int aj,
+                                             int colbase, int n_rad, double *o, size_t ostride, size_t blockstride) {
+    switch (cnt) {
+        case 1: asm_run<1, NMB, CPLX>(WP_ASM_ARGS); break;
+        case 2: asm_run<2, NMB, CPLX>(WP_ASM_ARGS); break;
+        case 3: asm_run<3, NMB, CPLX>(WP_ASM_ARGS); break;
+        case 4: asm_run<4, NMB, CPLX>(WP_ASM_ARGS); break;
+        case 5: asm_run<5, NMB, CPLX>(WP_ASM_ARGS); break;
+        case 6: asm_run<6, NMB, CPLX>(WP_ASM_ARGS); break;
+        default: asm_run_any<CPLX>(sF, sOff, ang, nlm, nlm2, cnt, NMB, a0, a1, aj, colbase, n_rad, o, ostride, blockstride);
+    }
+}
+// all 2 l_i + 1 rows of the run, in blocks of up to four rows
+template <bool CPLX>
+__device__ __forceinline__ void asm_run_all(int cnt, int nm, const double *sF, const int *sOff, const double *ang, int nlm, int nlm2, int a0, int a1, int aj,
+                                            int colbase, int n_rad, double *o, size_t ostride) {
+    const size_t blockstride = (size_t)nm * ostride;
+    for (int mi0 = 0; mi0 < nm; mi0 += 4) {
+        switch (min(4, nm - mi0)) {
+            case 1: asm_run_rows<1, CPLX>(cnt, WP_ASM_ARGS); break;
+            case 2: asm_run_rows<2, CPLX>(cnt, WP_ASM_ARGS); break;
+            case 3: asm_run_rows<3, CPLX>(cnt, WP_ASM_ARGS); break;
+            default: asm_run_rows<4, CPLX>(cnt, WP_ASM_ARGS); break;
+        }
+        ang += 4 * nlm; o += 4 * ostride;
+    }
+}
+#undef WP_ASM_ARGS
+
+constexpr int ASM2_THREADS = 640;          // at most: 102 registers per thread for the register-resident angular factors
+
+template <bool CPLX>
+__global__ void __launch_bounds__(ASM2_THREADS) k_direct_assemble2(const Asm2Args a) {
     extern __shared__ __align__(16) double sm2[];
     const int L = a.lambda_max, ldp = 2 * L + 1, nlm = (a.Lc + 1) * (a.Lc + 1), tid = threadIdx.x, nt = blockDim.x;
     double *sF = sm2;                                    // [E] pair-major
@@ -221,13 +305,46 @@ __global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
     double *sP = sAng + (size_t)(L + 1) * nlm * nlm;     // [(L+1)][2L+1]
     int *sOff = reinterpret_cast<int *>(sP + (L + 1) * ldp + 1);   // [n_pairs]
     int *sSt = sOff + a.n_pairs;                         // [N]
+    int *sRun = sSt + a.N;                               // [n_rad + 1][4]: runs of consecutive radial functions with equal l: a0, a1, l, first row
+    __shared__ int s_nrun;
     for (int i = tid; i < a.n_pairs; i += nt) sOff[i] = a.pair_off[i];
     for (int i = tid; i < a.N; i += nt) sSt[i] = a.st_pack[i];
-    const int N = a.N, di = nt / N, dj = nt - di * N;
+    const int N = a.N, n_rad = a.n_rad;
+    __syncthreads();
+    if (tid == 0) {
+        int nr = 0, i = 0, ai = 0;
+        while (ai < n_rad) {
+            const int l = (sSt[i] >> 16) & 15, a0 = ai, row0 = i;
+            while (ai < n_rad && ((sSt[i] >> 16) & 15) == l) { ++ai; i += 2 * l + 1; if (i >= N) { ai = (i == N) ? ai : n_rad; break; } }
+            sRun[4 * nr] = a0; sRun[4 * nr + 1] = ai; sRun[4 * nr + 2] = l; sRun[4 * nr + 3] = row0; ++nr;
+            if (i >= N) break;
+        }
+        s_nrun = nr;
+    }
     for (int p = blockIdx.x; p < a.n_pos; p += gridDim.x) {
-        __syncthreads();                                 // previous position done with sF / sAng
-        if (tid == 0) assoc_legendre_all(L, a.cosT[p], sP, ldp);
+        __syncthreads();                                 // previous position done with sF / sAng; run table visible
+        // P_lambda^mu(cos Theta), one thread per |mu| (independent recurrences in lambda)
+        if (tid <= L) {
+            const int m = tid;
+            const double x = a.cosT[p], sn = sqrt(fmax(0.0, 1.0 - x * x));
+            double pmm = 1.0;
+            for (int q = 1; q <= m; ++q) pmm = -pmm * (2 * q - 1) * sn;
+            double p0 = pmm, p1 = x * (2 * m + 1) * pmm;
+            for (int lam = m; lam <= L; ++lam) {
+                double val;
+                if (lam == m) val = p0;
+                else if (lam == m + 1) val = p1;
+                else { val = ((2 * lam - 1) * x * p1 - (lam + m - 1) * p0) / (lam - m); p0 = p1; p1 = val; }
+                sP[lam * ldp + m + L] = val;
+                if (m > 0) {
+                    double ratio = 1.0;                      // (lam-m)!/(lam+m)!
+                    for (int q = lam - m + 1; q <= lam + m; ++q) ratio /= q;
+                    sP[lam * ldp - m + L] = ((m & 1) ? -ratio : ratio) * val;
+                }
+            }
+        }
         const double *Fp = a.F + pos_row(a.fmap, p) * a.ldF + a.f_off;
+        #pragma unroll 4
         for (int e = tid; e < a.E; e += nt) sF[a.ent_perm[e]] = Fp[e];
         __syncthreads();
         for (int e = tid; e < (L + 1) * nlm * nlm; e += nt) {
@@ -245,21 +362,22 @@ __global__ void __launch_bounds__(1024) k_direct_assemble2(const Asm2Args a) {
             sAng[e] = v;
         }
         __syncthreads();
-        int i = tid / N, j = tid - i * N;
-        double *outp = a.out + (size_t)p * a.pos_stride * (a.complex_out ? 2 : 1);
-        for (int idx = tid; idx < N * N; idx += nt) {
-            const int si = sSt[i], sj = sSt[j];
-            const int ai = si & 0xffff, aj = sj & 0xffff, li = (si >> 16) & 15, lj = (sj >> 16) & 15;
-            const int alo = min(ai, aj), ahi = max(ai, aj);
-            const double *f = sF + sOff[alo * a.n_rad - alo * (alo - 1) / 2 + (ahi - alo)];
-            const int lam0 = abs(li - lj), lam1 = min(li + lj, L);
-            const double *ang = sAng + ((size_t)lam0 * nlm + (si >> 20)) * nlm + (sj >> 20);
-            double acc = 0.0;
-            for (int lam = lam0; lam <= lam1; lam += 2) { acc += ang[0] * f[0]; ang += 2 * nlm * nlm; ++f; }
-            const size_t o = (size_t)i * a.ld_out + j;
-            if (a.complex_out) *reinterpret_cast<double2 *>(outp + 2 * o) = make_double2(acc, 0.0);
-            else outp[o] = acc;
-            i += di; j += dj; if (j >= N) { j -= N; ++i; }
+        // thread = column j; all threads walk the rows in step, so every store instruction writes one contiguous run of a row of D
+        double *outp = a.out + (size_t)p * a.pos_stride * (CPLX ? 2 : 1);
+        const int nlm2 = 2 * nlm * nlm, nrun = s_nrun;
+        const size_t ostride = (size_t)a.ld_out * (CPLX ? 2 : 1);
+        for (int j = tid; j < N; j += nt) {
+            const int sj = sSt[j], aj = sj & 0xffff, lj = (sj >> 16) & 15;
+            const int colbase = aj * n_rad - aj * (aj - 1) / 2 - aj;              // pair(a_j, a_i) - a_i for a_i >= a_j
+            const double *angj = sAng + (sj >> 20);
+            double *oj = outp + (size_t)j * (CPLX ? 2 : 1);
+            for (int r = 0; r < nrun; ++r) {
+                const int a0 = sRun[4 * r], a1 = sRun[4 * r + 1], li = sRun[4 * r + 2], row0 = sRun[4 * r + 3];
+                const int lam0 = abs(li - lj), cnt = (min(li + lj, L) - lam0) / 2 + 1;
+                const double *ang = angj + (lam0 * nlm + li * li) * nlm;           // lm index of (l_i, -l_i) = l_i^2
+                double *o = oj + (size_t)row0 * ostride;
+                asm_run_all<CPLX>(cnt, 2 * li + 1, sF, sOff, ang, nlm, nlm2, a0, a1, aj, colbase, n_rad, o, ostride);
+            }
         }
     }
 }
@@ -385,7 +503,7 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
     // fast path when the per-position operands fit shared memory
     const int nlm = (C.l_max + 1) * (C.l_max + 1), L1 = B->lambda_max + 1;
     const size_t smem2 = ((size_t)((C.E + 1) & ~1) + (size_t)L1 * nlm * nlm + (size_t)L1 * (2 * B->lambda_max + 1) + 1) * 8 +
-                         ((size_t)C.n_pairs + C.n_states) * 4 + 16;
+                         ((size_t)C.n_pairs + C.n_states + 4 * ((size_t)C.n_rad + 1)) * 4 + 16;
     if (smem2 <= 220 * 1024) {
         Asm2Args b{};
         b.G = C.d_G; b.pair_off = C.d_pair_off; b.ent_perm = C.d_ent_perm; b.st_pack = C.d_st_pack;
@@ -394,11 +512,17 @@ int wp_direct_assemble(wpccc_basis *B, int c, int n_pos, const double *d_cos, co
         b.f_off = a.f_off; b.ld_out = ld_out; b.complex_out = complex_out; b.n_pos = n_pos; b.pos_stride = pos_stride;
         b.charge = a.charge; b.alt_sign = a.alt_sign; b.fmap = a.fmap;
         static PerDevice attr2;
-        if (wp_raise(attr2, smem2)) WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-        const int per_sm = smem2 <= 100 * 1024 ? 2 : 1;
-        const int threads = (C.n_states * C.n_states >= 64 * 1024) ? 1024 : 512;
+        if (wp_raise(attr2, smem2)) {
+            WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+            WP_CUDA(cudaFuncSetAttribute(k_direct_assemble2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+        }
+        // one thread per column of D; CTAs of a few positions each, so that the hardware scheduler balances them over whatever
+        // SMs the concurrent sweep kernel leaves free
+        const int threads = std::min(ASM2_THREADS, (C.n_states + 31) & ~31);
+        const int grid = std::max(1, std::min(n_pos, std::max(148 * 8, (n_pos + 3) / 4)));
         wp_span_begin(B, FAM_DASM, s);
-        k_direct_assemble2<<<std::min(n_pos, 148 * per_sm), threads, smem2, s>>>(b);
+        if (complex_out) k_direct_assemble2<true><<<grid, threads, smem2, s>>>(b);
+        else k_direct_assemble2<false><<<grid, threads, smem2, s>>>(b);
         wp_span_end(B, s, 1);
         WP_CUDA(cudaGetLastError());
         return 0;
