@@ -726,6 +726,7 @@ struct TrotArgs {
     const int *radT, *lT_st, *mT_st;         // per target state: radial function, l, m
     const int *radP, *lP_st, *mP_st;         // per projectile state
     const int *colT, *colP;                  // [n_rad][WP_MAX_L+1] column of (a, |q|)
+    const int *colTst;                       // [NT][lmax+1] column of (radial function of target state ia, q), 0 beyond l
     const int *lradP;                        // [n_rad_P] l of each projectile radial function
     const TrotChunk *chunks; const int *rowbase;   // rowbase[b]: first local body row of radial function b inside its chunk
     int NT, NP, lmax, max_rows;
@@ -755,17 +756,17 @@ __device__ double wigner_d(int l, int mp, int m, double cb, double sb) {
     return tot;
 }
 
-// grid = (chunk of projectile radial functions, product, position); block 256.  The body-frame rows the chunk needs
-// (both families, ring splits summed in order) are staged in shared memory with coalesced loads; then one thread per
-// lab-frame output element (beta, alpha), eq. (8):
+// grid = (chunk of projectile radial functions, 1, position); block 256.  A CTA handles every product of its chunk in turn
+// (S_PT -> K and K^T, H_PT, H_TP), so that the Wigner matrices and the index tables are set up once.  The body-frame rows
+// the chunk needs (both families, ring splits summed in order) are staged in shared memory with coalesced loads; then one
+// thread per lab-frame output element (beta, alpha), eq. (8):
 //   X_lab[beta, alpha] = sum_{q', q} d^{l_b}_{m_b q'}(Theta) d^{l_a}_{m_a q}(Theta) X_body[(b, q'), (a, q)],
 // where the signed body-frame element comes from the two q >= 0 families of the contraction:
 //   family (-) (weights Phi_{|q-q'|}) when q, q' have the same sign or one is 0, family (+) (Phi_{q+q'}) otherwise,
 //   times (-1)^q for q < 0 and (-1)^q' for q' < 0.
 __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     extern __shared__ __align__(16) double sd[];     // [lmax+1][W][W] Wigner d, W = 2 lmax + 1; then body rows [2][max_rows][nq8T] complex
-    // blockIdx.y: 0 S_PT -> K, 1 H_PT, 2 H_TP, 3 (only with a.KT) S_PT once more -> K^T
-    const int yid = blockIdx.y, prod = yid == 3 ? 0 : yid, tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
+    const int tid = threadIdx.x, L = a.lmax, W = 2 * L + 1;
     const TrotChunk ch = a.chunks[blockIdx.x];
     int p; const double2 *part;              // window position (geometry, outputs) and its body-frame integrals
     {
@@ -784,6 +785,11 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
     const int TB = a.tb;                                                          // target states per pass (NT unless shared memory is short)
     double2 *Ep = body + 2 * fam_stride, *Em = Ep + (size_t)a.max_rows * TB;      // [rows][TB] each
     int *s_colT = reinterpret_cast<int *>(Em + (size_t)a.max_rows * TB);          // [NT][L+1] column of (a, q) per target state
+    // stage the rows (b, q'), b in [b0, b1), q' = 0..l_b: local row = rowbase[b] + q'
+    __shared__ int s_rowsrc[256], s_rowp[256];       // body row (column index of centre P) and q' of each local row
+    for (int b = ch.b0 + tid; b < ch.b1; b += blockDim.x)
+        for (int r = 0; r <= a.lradP[b]; ++r) { s_rowsrc[a.rowbase[b] + r] = a.colP[b * (WP_MAX_L + 1) + r]; s_rowp[a.rowbase[b] + r] = r; }
+    for (int e = tid; e < NT * (L + 1); e += blockDim.x) s_colT[e] = a.colTst[e];
     {
         double sb, cb; sincos(0.5 * a.theta[p], &sb, &cb);
         for (int e = tid; e < (L + 1) * W * W; e += blockDim.x) {
@@ -791,78 +797,99 @@ __global__ void __launch_bounds__(256) k_trot(const TrotArgs a) {
             sd[e] = (abs(mp) <= l && abs(m) <= l) ? wigner_d(l, mp, m, cb, sb) : 0.0;
         }
     }
-    // stage the rows (b, q'), b in [b0, b1), q' = 0..l_b: local row = rowbase[b] + q'
-    __shared__ int s_rowsrc[256], s_rowp[256];       // body row (column index of centre P) and q' of each local row
-    for (int b = ch.b0 + tid; b < ch.b1; b += blockDim.x)
-        for (int r = 0; r <= a.lradP[b]; ++r) { s_rowsrc[a.rowbase[b] + r] = a.colP[b * (WP_MAX_L + 1) + r]; s_rowp[a.rowbase[b] + r] = r; }
-    for (int e = tid; e < NT * (L + 1); e += blockDim.x) {
-        const int ia = e / (L + 1), q = e - ia * (L + 1);
-        s_colT[e] = (q <= a.lT_st[ia]) ? a.colT[a.radT[ia] * (WP_MAX_L + 1) + q] : 0;
-    }
-    __syncthreads();
-    {
-        const int per_fam = ch.nrows * nq8T;
-        for (int e = tid; e < 2 * per_fam; e += blockDim.x) {
-            const int fam = e >= per_fam, r2 = e - fam * per_fam, r = r2 / nq8T, c = r2 - r * nq8T;
-            const double2 *src = part + ((size_t)fam * 3 + prod) * blk + (size_t)s_rowsrc[r] * nq8T + c;
-            double2 v = {0.0, 0.0};
-            for (int sp = 0; sp < a.n_split; ++sp) { const double2 x = src[(size_t)sp * 6 * blk]; v.x += x.x; v.y += x.y; }
-            body[fam * fam_stride + (size_t)r * nq8T + c] = v;
-        }
-    }
-    __syncthreads();
-    // stage 1: contract the target-side index.  For body row (b, p = |q'|) and target state alpha = (a, m_a):
-    //   P0 = sum_{q>=0} d^{l_a}_{m_a,q} F0[q],  M0 = sum_{q>0} (-1)^q d_{m_a,-q} F0[q],  P1, M1 the same with family (+),
-    //   E+ = P0 + (p == 0 ? M0 : M1)            (q' = +p),      E- = (-1)^p (d_{m_a,0} F0[0] + P1 + M0)   (q' = -p < 0)
     const int NP = a.NP, N = NT + NP;
-    for (int ia0 = 0; ia0 < NT; ia0 += TB) {
-    const int tbn = min(TB, NT - ia0);
-    if (ia0) __syncthreads();                                 // the previous pass is done with Ep, Em
-    for (int e = tid; e < ch.nrows * tbn; e += blockDim.x) {
-        const int r = e / tbn, ia = ia0 + (e - r * tbn), pq = s_rowp[r];
-        const int la = a.lT_st[ia], ma = a.mT_st[ia];
-        const double *dA = sd + (la * W + ma + L) * W + L;
-        const double2 *f0 = body + (size_t)r * nq8T, *f1 = f0 + fam_stride;
-        const int *ct = s_colT + ia * (L + 1);
-        const double2 x00 = f0[ct[0]];
-        const double d0 = dA[0];
-        double2 P0 = {d0 * x00.x, d0 * x00.y}, M0 = {0.0, 0.0}, P1 = {0.0, 0.0}, M1 = {0.0, 0.0};
-        const double2 Z0 = P0;
-        for (int q = 1; q <= la; ++q) {
-            const int c = ct[q];
-            const double dp = dA[q], dm = (q & 1) ? -dA[-q] : dA[-q];
-            const double2 x0 = f0[c], x1 = f1[c];
-            P0.x += dp * x0.x; P0.y += dp * x0.y; M0.x += dm * x0.x; M0.y += dm * x0.y;
-            P1.x += dp * x1.x; P1.y += dp * x1.y; M1.x += dm * x1.x; M1.y += dm * x1.y;
+    const int per_fam = ch.nrows * nq8T;
+    // outputs in turn: 0 S_PT -> K, 3 S_PT -> K^T (same staged rows and stage 1 as 0; only with a.KT), 1 H_PT, 2 H_TP
+    for (int oi = 0; oi < 4; ++oi) {
+        const int yid = (oi == 0) ? 0 : (oi == 1 ? 3 : oi - 1), prod = yid == 3 ? 0 : yid;
+        if (yid == 3 && !a.KT) continue;
+        __syncthreads();                             // tables ready / the previous output is done with body, Ep, Em
+        if (yid != 3) {
+            const double2 *src0 = part + (size_t)prod * blk;
+            if (a.n_split == 1) {
+                // four independent 16-byte loads in flight per thread
+                for (int e0 = tid; e0 < 2 * per_fam; e0 += 4 * 256) {
+                    double2 v[4]; int dst[4];
+                    #pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int e = e0 + 256 * u;
+                        dst[u] = -1;
+                        if (e < 2 * per_fam) {
+                            const int fam = e >= per_fam, r2 = e - fam * per_fam, r = r2 / nq8T, c = r2 - r * nq8T;
+                            v[u] = src0[(size_t)fam * 3 * blk + (size_t)s_rowsrc[r] * nq8T + c];
+                            dst[u] = fam * (int)fam_stride + r * nq8T + c;
+                        }
+                    }
+                    #pragma unroll
+                    for (int u = 0; u < 4; ++u) if (dst[u] >= 0) body[dst[u]] = v[u];
+                }
+            } else {
+                for (int e = tid; e < 2 * per_fam; e += blockDim.x) {
+                    const int fam = e >= per_fam, r2 = e - fam * per_fam, r = r2 / nq8T, c = r2 - r * nq8T;
+                    const double2 *src = src0 + (size_t)fam * 3 * blk + (size_t)s_rowsrc[r] * nq8T + c;
+                    double2 v = {0.0, 0.0};
+                    for (int sp = 0; sp < a.n_split; ++sp) { const double2 x = src[(size_t)sp * 6 * blk]; v.x += x.x; v.y += x.y; }
+                    body[fam * fam_stride + (size_t)r * nq8T + c] = v;
+                }
+            }
+            __syncthreads();
         }
-        const double2 mm = (pq == 0) ? M0 : M1;
-        const double sg = (pq & 1) ? -1.0 : 1.0;
-        Ep[e] = {P0.x + mm.x, P0.y + mm.y};
-        Em[e] = {sg * (Z0.x + P1.x + M0.x), sg * (Z0.y + P1.y + M0.y)};
-    }
-    __syncthreads();
-    // stage 2: contract the projectile-side index
-    for (int e = tid; e < ch.nst * tbn; e += blockDim.x) {
-        // loop order = the order of the output rows (coalesced stores): K and H_PT row-major in (beta, alpha), H_TP and K^T in
-        // (alpha, beta); with a.ht the H blocks are written transposed (H^T is what the RK4 sweep streams), so the two swap
-        const bool beta_major = (yid == 0) || (yid == 1 && !a.ht) || (yid == 2 && a.ht);
-        const int ibl = beta_major ? e / tbn : e % ch.nst, ial = beta_major ? e % tbn : e / ch.nst, ia = ia0 + ial;
-        const int ib = ch.st0 + ibl;
-        const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
-        const double *dB = sd + (lb * W + mb + L) * W + L;
-        const double2 *ep = Ep + (size_t)a.rowbase[rb] * tbn + ial, *em = Em + (size_t)a.rowbase[rb] * tbn + ial;
-        double sr = dB[0] * ep[0].x, si = dB[0] * ep[0].y;
-        for (int pq = 1; pq <= lb; ++pq) {
-            const double2 xp = ep[pq * tbn], xm = em[pq * tbn];
-            sr += dB[pq] * xp.x + dB[-pq] * xm.x; si += dB[pq] * xp.y + dB[-pq] * xm.y;
+        // stage 1: contract the target-side index.  For body row (b, p = |q'|) and target state alpha = (a, m_a):
+        //   P0 = sum_{q>=0} d^{l_a}_{m_a,q} F0[q],  M0 = sum_{q>0} (-1)^q d_{m_a,-q} F0[q],  P1, M1 the same with family (+),
+        //   E+ = P0 + (p == 0 ? M0 : M1)            (q' = +p),      E- = (-1)^p (d_{m_a,0} F0[0] + P1 + M0)   (q' = -p < 0)
+        // (with all target states in one pass, output 3 reuses E+, E- of output 0)
+        for (int ia0 = 0; ia0 < NT; ia0 += TB) {
+            const int tbn = min(TB, NT - ia0);
+            if (!(yid == 3 && TB >= NT)) {
+                if (ia0) __syncthreads();                                 // the previous pass is done with Ep, Em
+                for (int e = tid; e < ch.nrows * tbn; e += blockDim.x) {
+                    const int r = e / tbn, ia = ia0 + (e - r * tbn), pq = s_rowp[r];
+                    const int la = a.lT_st[ia], ma = a.mT_st[ia];
+                    const double *dA = sd + (la * W + ma + L) * W + L;
+                    const double2 *f0 = body + (size_t)r * nq8T, *f1 = f0 + fam_stride;
+                    const int *ct = s_colT + ia * (L + 1);
+                    const double2 x00 = f0[ct[0]];
+                    const double d0 = dA[0];
+                    double2 P0 = {d0 * x00.x, d0 * x00.y}, M0 = {0.0, 0.0}, P1 = {0.0, 0.0}, M1 = {0.0, 0.0};
+                    const double2 Z0 = P0;
+                    for (int q = 1; q <= la; ++q) {
+                        const int c = ct[q];
+                        const double dp = dA[q], dm = (q & 1) ? -dA[-q] : dA[-q];
+                        const double2 x0 = f0[c], x1 = f1[c];
+                        P0.x += dp * x0.x; P0.y += dp * x0.y; M0.x += dm * x0.x; M0.y += dm * x0.y;
+                        P1.x += dp * x1.x; P1.y += dp * x1.y; M1.x += dm * x1.x; M1.y += dm * x1.y;
+                    }
+                    const double2 mm = (pq == 0) ? M0 : M1;
+                    const double sg = (pq & 1) ? -1.0 : 1.0;
+                    Ep[e] = {P0.x + mm.x, P0.y + mm.y};
+                    Em[e] = {sg * (Z0.x + P1.x + M0.x), sg * (Z0.y + P1.y + M0.y)};
+                }
+                __syncthreads();
+            }
+            // stage 2: contract the projectile-side index
+            for (int e = tid; e < ch.nst * tbn; e += blockDim.x) {
+                // loop order = the order of the output rows (coalesced stores): K and H_PT row-major in (beta, alpha), H_TP and K^T in
+                // (alpha, beta); with a.ht the H blocks are written transposed (H^T is what the RK4 sweep streams), so the two swap
+                const bool beta_major = (yid == 0) || (yid == 1 && !a.ht) || (yid == 2 && a.ht);
+                const int ibl = beta_major ? e / tbn : e % ch.nst, ial = beta_major ? e % tbn : e / ch.nst, ia = ia0 + ial;
+                const int ib = ch.st0 + ibl;
+                const int rb = a.radP[ib], lb = a.lP_st[ib], mb = a.mP_st[ib];
+                const double *dB = sd + (lb * W + mb + L) * W + L;
+                const double2 *ep = Ep + (size_t)a.rowbase[rb] * tbn + ial, *em = Em + (size_t)a.rowbase[rb] * tbn + ial;
+                double sr = dB[0] * ep[0].x, si = dB[0] * ep[0].y;
+                for (int pq = 1; pq <= lb; ++pq) {
+                    const double2 xp = ep[pq * tbn], xm = em[pq * tbn];
+                    sr += dB[pq] * xp.x + dB[-pq] * xm.x; si += dB[pq] * xp.y + dB[-pq] * xm.y;
+                }
+                double *o;
+                if (yid == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
+                else if (yid == 3) o = a.KT + (((size_t)p * NT + ia) * NP + ib) * 2;
+                else if (yid == 1) o = a.H + (a.ht ? ((size_t)p * N + ia) * N + NT + ib : ((size_t)p * N + NT + ib) * N + ia) * 2;             // H_PT
+                else { o = a.H + (a.ht ? ((size_t)p * N + NT + ib) * N + ia : ((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
+                *reinterpret_cast<double2 *>(o) = make_double2(sr, si);
+            }
+            if (yid == 3 && TB < NT) __syncthreads();
         }
-        double *o;
-        if (yid == 0) o = a.K + (((size_t)p * NP + ib) * NT + ia) * 2;
-        else if (yid == 3) o = a.KT + (((size_t)p * NT + ia) * NP + ib) * 2;
-        else if (yid == 1) o = a.H + (a.ht ? ((size_t)p * N + ia) * N + NT + ib : ((size_t)p * N + NT + ib) * N + ia) * 2;             // H_PT
-        else { o = a.H + (a.ht ? ((size_t)p * N + NT + ib) * N + ia : ((size_t)p * N + ia) * N + NT + ib) * 2; si = -si; }            // H_TP = conj(rot Tb)^T
-        o[0] = sr; o[1] = si;
-    }
     }
 }
 
@@ -923,7 +950,7 @@ size_t wp_transfer_ws_bytes(const wpccc_basis *B, int n_pos_chunk) {
     return P.per_pos_bytes() * (size_t)n_pos_chunk + P.tiles.size() * sizeof(int2) + 4096 +
            2 * (size_t)(B->c[0].n_rad + B->c[1].n_rad) * (WP_MAX_L + 1) * sizeof(int) +
            2 * (size_t)(P.nq8[0] + P.nq8[1]) * sizeof(int) +
-           (size_t)B->c[1].n_rad * (sizeof(TrotChunk) + sizeof(int)) + 1024;
+           (size_t)B->c[1].n_rad * (sizeof(TrotChunk) + sizeof(int)) + (size_t)B->c[0].n_states * (WP_MAX_L + 1) * sizeof(int) + 2048;
 }
 
 int wp_transfer_chunk_positions(const wpccc_basis *B, size_t ws_bytes) {
@@ -1009,6 +1036,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     }
     TrotChunk *d_rchunks = (TrotChunk *)take(rchunks.size() * sizeof(TrotChunk));
     int *d_rowbase = (int *)take(rowbase.size() * sizeof(int));
+    int *d_colTst = (int *)take((size_t)B->c[0].n_states * (lmx + 1) * sizeof(int));
     if (off > ws_bytes) WP_FAIL(WPCCC_ENOMEM, "transfer workspace too small");
     WP_CUDA(cudaMemcpyAsync(d_rchunks, rchunks.data(), rchunks.size() * sizeof(TrotChunk), cudaMemcpyHostToDevice, s));
     WP_CUDA(cudaMemcpyAsync(d_rowbase, rowbase.data(), rowbase.size() * sizeof(int), cudaMemcpyHostToDevice, s));
@@ -1058,12 +1086,17 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
     if (dual && wp_raise(dual_attr, dual_smem)) WP_CUDA(cudaFuncSetAttribute(k_tcon<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dual_smem));
 
     const int NT = B->c[0].n_states, NP = B->c[1].n_states, N = NT + NP;
+    {   // column of (radial function of target state ia, q) for q <= l, position-independent
+        std::vector<int> cst((size_t)NT * (lmx + 1), 0);
+        for (int ia = 0; ia < NT; ++ia)
+            for (int q = 0; q <= B->c[0].st_l[ia]; ++q) cst[(size_t)ia * (lmx + 1) + q] = hcol[0][(size_t)B->c[0].st_rad[ia] * (WP_MAX_L + 1) + q];
+        WP_CUDA(cudaMemcpyAsync(d_colTst, cst.data(), cst.size() * 4, cudaMemcpyHostToDevice, s));
+    }
     TrotArgs tr{}; tr.n_split = n_split; tr.nq8T = P.nq8[0]; tr.nq8P = P.nq8[1]; tr.theta = d_theta;
     tr.radT = B->c[0].d_st_rad; tr.lT_st = B->c[0].d_st_l; tr.mT_st = B->c[0].d_st_m;
     tr.radP = B->c[1].d_st_rad; tr.lP_st = B->c[1].d_st_l; tr.mP_st = B->c[1].d_st_m;
-    tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.NT = NT; tr.NP = NP;
+    tr.colT = d_colidx[0]; tr.colP = d_colidx[1]; tr.colTst = d_colTst; tr.NT = NT; tr.NP = NP;
     tr.lmax = lmx; tr.K = d_K; tr.H = d_H; tr.KT = d_KT; tr.ht = d_KT != nullptr;
-    const unsigned n_prod = d_KT ? 4 : 3;
     tr.lradP = B->c[1].d_l; tr.chunks = d_rchunks; tr.rowbase = d_rowbase; tr.max_rows = rot_max_rows;
     tr.sel = sd; tr.tb = rot_tb;
     for (int p0 = 0; p0 < n_eval; p0 += chunk) {
@@ -1110,7 +1143,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
 
         tr.part = d_part; tr.q0 = p0; tr.fetch = 0;
         wp_span_begin(B, FAM_ROT, s);
-        k_trot<<<dim3((unsigned)rchunks.size(), n_prod, np), 256, rot_smem, s>>>(tr);
+        k_trot<<<dim3((unsigned)rchunks.size(), 1, np), 256, rot_smem, s>>>(tr);
         wp_span_end(B, s, 1);
         B->units[FAM_ROT] += np;
         WP_CUDA(cudaGetLastError());
@@ -1122,7 +1155,7 @@ int wp_transfer(wpccc_basis *B, int n_pos, const double *d_R, const double *d_co
         for (int z0 = 0; z0 < total; z0 += 32768) {
             tr.q0 = z0;                      // fetch mode: first (g, lf) pair of this launch
             wp_span_begin(B, FAM_ROT, s);
-            k_trot<<<dim3((unsigned)rchunks.size(), n_prod, (unsigned)std::min(32768, total - z0)), 256, rot_smem, s>>>(tr);
+            k_trot<<<dim3((unsigned)rchunks.size(), 1, (unsigned)std::min(32768, total - z0)), 256, rot_smem, s>>>(tr);
             wp_span_end(B, s, 1);
             WP_CUDA(cudaGetLastError());
         }
