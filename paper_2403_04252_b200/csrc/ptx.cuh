@@ -49,5 +49,28 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
+// ---- thread-block clusters: rank, cluster-wide barrier, mbarrier hand-shake and loads across the CTAs of a cluster
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {          // every thread of every CTA of the cluster
+    asm volatile("barrier.cluster.arrive.release;\n barrier.cluster.wait.acquire;\n" ::: "memory");
+}
+// arrive (release at cluster scope) on the mbarrier at the same shared-memory offset in CTA `peer` of the cluster
+__device__ __forceinline__ void mbar_arrive_peer(unsigned long long *bar, unsigned peer) {
+    asm volatile("{\n .reg .b32 ra;\n mapa.shared::cluster.u32 ra, %0, %1;\n mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n}\n"
+                 ::"r"(smem_u32(bar)), "r"(peer) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(unsigned long long *bar, unsigned parity) {      // acquire at cluster scope
+    asm volatile(
+        "{\n .reg .pred p;\n WAITC_%=:\n mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n @p bra DONEC_%=;\n bra WAITC_%=;\n DONEC_%=:\n}\n"
+        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// the complex number at the same shared-memory offset as `p` in CTA `peer` of the cluster (distributed shared memory)
+__device__ __forceinline__ cplx ld_peer(const cplx *p, unsigned peer) {
+    unsigned ra; cplx v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(ra) : "r"(smem_u32(p)), "r"(peer));
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(ra) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;\n" ::"r"(id), "r"(count) : "memory"); }

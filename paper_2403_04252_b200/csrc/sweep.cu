@@ -644,11 +644,17 @@ constexpr int SW_DLD = CHOL_NB + 1;      // row stride of the staged diagonal bl
 constexpr int SW_TCOLS = 4;            // columns / rows of K per consumer thread in the K^H and K products: N_T, N_P <= 1024
 constexpr int SW_TROWS = 8;            // rows of H0 per consumer thread: N <= 2048
 
-template <bool SOLVE, int TR>          // TR = ceil(N / 256): rows of H0 per consumer thread
+// NC = 2: a cluster of two CTAs per trajectory.  Both hold the whole state and walk the same stages; the three matrix-vector
+// products of a stage (H0 x, K y_T, K^H w_P) are split by streamed rows -- each CTA streams and multiplies one half of H0^T, K^T
+// and K, i.e. half of the bytes that bound a single SM (its TMA stream and its shared-memory port) -- and the partial sums are
+// exchanged through distributed shared memory (one mbarrier hand-shake per product; a + b = b + a, so both CTAs carry bit-identical
+// vectors).  The triangular solves are done by both (no exchange inside the block recurrences).
+template <bool SOLVE, int TR, int NC>  // TR = ceil(N / 256): rows of H0 per consumer thread
 __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Args a, const int chunk_bytes, const int NS) {
     extern __shared__ __align__(128) unsigned char smraw[];
     const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int t = blockIdx.x;
+    const int t = blockIdx.x / NC;
+    const unsigned rank = NC > 1 ? cluster_ctarank() : 0u, peer = rank ^ 1u;
     const bool track = a.drift != nullptr;
     const SweepSched S(NT, NP, chunk_bytes);
     const CholLayout CL(NP);
@@ -658,21 +664,29 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     cplx *X = reinterpret_cast<cplx *>(smraw + (size_t)NS * chunk_bytes);
     cplx *Y = X + N, *Wp = Y + N;
     cplx *Tj = Wp + NP, *Dblk = Tj + CHOL_NB, *part2 = Dblk + CHOL_NB * SW_DLD;                                  // SOLVE: [32], [32][33], [8][32]
-    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
+    cplx *Ypart = part2 + 8 * CHOL_NB, *Kpart = Ypart + N, *Tpart = Kpart + NP;                                  // NC = 2: this CTA's partial sums [N], [NP], [NT]
+    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES], xbar[3];
     __shared__ double red[8];
     __shared__ int redi[8];
     if (tid == 0) {
         for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
+        for (int s = 0; s < 3; ++s) mbar_init(&xbar[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
+    if (NC > 1) cluster_sync_all();                  // the peer's mbarriers exist before anything arrives on them
+    // chunk ranges of this CTA in the three split products
+    const int hH = NC > 1 ? (S.nH + 1) / 2 : S.nH, hKT = NC > 1 ? (S.nKT + 1) / 2 : S.nKT, hK = NC > 1 ? (S.nK + 1) / 2 : S.nK;
+    const int qH0 = rank ? hH : 0, qH1 = (NC > 1 && rank == 0) ? hH : S.nH;
+    const int qT0 = rank ? hKT : 0, qT1 = (NC > 1 && rank == 0) ? hKT : S.nKT;
+    const int qK0 = rank ? hK : 0, qK1 = (NC > 1 && rank == 0) ? hK : S.nK;
     const cplx *Hg = reinterpret_cast<const cplx *>(a.H), *Kg = reinterpret_cast<const cplx *>(a.K), *Ag = reinterpret_cast<const cplx *>(a.Ainv);
     const cplx *KTg = reinterpret_cast<const cplx *>(a.KT);
     const size_t a_stride = wp_factor_elems(NP);
 
     if (warp == SW_CONSUMERS / 32) {
         // ---------------- producer: one lane streams the chunk sequence of the whole window
-        if (lane != 0) return;
+        if (lane != 0) { if (NC > 1) cluster_sync_all(); return; }
         long long g = 0;
         auto push = [&](const cplx *src, unsigned bytes) {
             const int slot = (int)(g % NS); const long long use = g / NS;
@@ -681,17 +695,17 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
             tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
             ++g;
         };
-        auto push_K = [&](const cplx *Kp) { for (int q = 0; q < S.nK; ++q) { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); push(Kp + (size_t)r0 * NT, (unsigned)rows * NT * 16u); } };
-        auto push_KT = [&](const cplx *Kp) { for (int q = 0; q < S.nKT; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NT - r0); push(Kp + (size_t)r0 * NP, (unsigned)rows * NP * 16u); } };
+        auto push_K = [&](const cplx *Kp) { for (int q = qK0; q < qK1; ++q) { const int r0 = q * S.rK, rows = min(S.rK, NP - r0); push(Kp + (size_t)r0 * NT, (unsigned)rows * NT * 16u); } };
+        auto push_KT = [&](const cplx *Kp, int q0, int q1) { for (int q = q0; q < q1; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NT - r0); push(Kp + (size_t)r0 * NP, (unsigned)rows * NP * 16u); } };
         for (int s = 0; s < a.steps; ++s)
             for (int st = 0; st < (track ? 5 : 4); ++st) {
                 const int li = 2 * s + (st == 0 ? 0 : (st >= 3 ? 2 : 1));
                 const size_t pos = (size_t)t * a.n_idx + li;
                 const cplx *Kp = Kg + pos * (size_t)NP * NT, *KTp = KTg + pos * (size_t)NP * NT;
-                if (st == 4) { push_KT(KTp); break; }
+                if (st == 4) { push_KT(KTp, 0, S.nKT); break; }             // the norm is formed by both CTAs in full
                 const cplx *Hp = Hg + pos * (size_t)N * N, *Ap = Ag + pos * a_stride;
-                for (int q = 0; q < S.nH; ++q) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); push(Hp + (size_t)r0 * N, (unsigned)rows * N * 16u); }
-                push_KT(KTp);
+                for (int q = qH0; q < qH1; ++q) { const int r0 = q * S.rH, rows = min(S.rH, N - r0); push(Hp + (size_t)r0 * N, (unsigned)rows * N * 16u); }
+                push_KT(KTp, qT0, qT1);
                 if (!SOLVE) {
                     for (int q = 0; q < S.nA; ++q) { const int r0 = q * S.rA, rows = min(S.rA, NP - r0); push(Ap + (size_t)r0 * NP, (unsigned)rows * NP * 16u); }
                 } else {
@@ -707,6 +721,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
                 }
                 push_K(Kp);
             }
+        if (NC > 1) cluster_sync_all();
         return;
     }
     // ---------------- consumers (256 threads)
@@ -744,6 +759,16 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     };
     consumer_sync();
     if (a.flags) { for (int w = 0; w < 8; ++w) first_bad = min(first_bad, redi[w]); }
+    // NC = 2: add the peer CTA's partial sums to this thread's (elements tid + 256 k < n); `buf` is this CTA's copy of them
+    unsigned xphase = 0;                                     // bit w: parity of the next wait on xbar[w]
+    auto exchange = [&](cplx *val, int nval, int n, cplx *buf, int which) {
+        for (int k = 0; k < nval; ++k) { const int j = tid + SW_CONSUMERS * k; if (j < n) buf[j] = val[k]; }
+        consumer_sync();                                     // every partial sum of this CTA is in `buf` (and every read of the previous exchange is done)
+        if (tid == 0) mbar_arrive_peer(&xbar[which], peer);
+        mbar_wait_cluster(&xbar[which], (xphase >> which) & 1u);
+        xphase ^= 1u << which;
+        for (int k = 0; k < nval; ++k) { const int j = tid + SW_CONSUMERS * k; if (j < n) { const cplx o = ld_peer(buf + j, peer); val[k].x += o.x; val[k].y += o.y; } }
+    };
 
     for (int s = 0; s < a.steps; ++s) {
         const double h = a.hs[s];
@@ -766,14 +791,14 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
             // (K v)_r = sum_c K^T[c][r] v_c for this thread's rows r = tid + 256 t of the projectile block: the rows c of K^T stream
             // through the ring, v_c is a broadcast, consecutive lanes read consecutive elements -- no reduction
             // (ILP independent accumulator sets over consecutive streamed rows: one set is a dependent fma chain of N_T links)
-            auto k_times = [&](const cplx *vT, cplx (&accK)[SW_TCOLS]) {
+            auto k_times = [&](const cplx *vT, cplx (&accK)[SW_TCOLS], int q0, int q1) {
                 constexpr int TC = (TR + 1) / 2, ILP = TC == 1 ? 4 : 2;
                 cplx ak[ILP][TC];
                 #pragma unroll
                 for (int u = 0; u < ILP; ++u)
                     #pragma unroll
                     for (int tc = 0; tc < TC; ++tc) ak[u][tc] = cplx{0.0, 0.0};
-                for (int q = 0; q < S.nKT; ++q) {
+                for (int q = q0; q < q1; ++q) {
                     const cplx *buf = acquire();
                     const int c0 = q * S.rA, rows = min(S.rA, NT - c0);
                     auto one = [&](int rr, int u) {
@@ -805,7 +830,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
             if (st == 4) {
                 // c^H S c = |c|^2 + 2 Re( X_P^H K X_T )
                 cplx accK[SW_TCOLS];
-                k_times(X, accK);
+                k_times(X, accK, 0, S.nKT);
                 double nrm = 0.0;
                 #pragma unroll
                 for (int tc = 0; tc < SW_TCOLS; ++tc) {
@@ -831,7 +856,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
                 for (int u = 0; u < ILP; ++u)
                     #pragma unroll
                     for (int tr = 0; tr < TR; ++tr) accY[u][tr] = cplx{0.0, 0.0};
-                for (int q = 0; q < S.nH; ++q) {
+                for (int q = qH0; q < qH1; ++q) {
                     const cplx *buf = acquire();
                     const int c0 = q * S.rH, rows = min(S.rH, N - c0);
                     auto one = [&](int rr, int u) {
@@ -853,18 +878,19 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
                 }
                 #pragma unroll
                 for (int tr = 0; tr < TR; ++tr) {
-                    const int r = tid + SW_CONSUMERS * tr;
-                    cplx y = accY[0][tr];
                     #pragma unroll
-                    for (int u = 1; u < ILP; ++u) { y.x += accY[u][tr].x; y.y += accY[u][tr].y; }
-                    if (r < N) Y[r] = y;
+                    for (int u = 1; u < ILP; ++u) { accY[0][tr].x += accY[u][tr].x; accY[0][tr].y += accY[u][tr].y; }
                 }
+                if (NC > 1) exchange(accY[0], TR, N, Ypart, 0);
+                #pragma unroll
+                for (int tr = 0; tr < TR; ++tr) { const int r = tid + SW_CONSUMERS * tr; if (r < N) Y[r] = accY[0][tr]; }
             }
             consumer_sync();
             // y_P -= K y_T
             {
                 cplx accK[SW_TCOLS];
-                k_times(Y, accK);
+                k_times(Y, accK, qT0, qT1);
+                if (NC > 1) exchange(accK, SW_TCOLS, NP, Kpart, 1);
                 #pragma unroll
                 for (int tc = 0; tc < SW_TCOLS; ++tc) { const int r = tid + SW_CONSUMERS * tc; if (r < NP) { Y[NT + r].x -= accK[tc].x; Y[NT + r].y -= accK[tc].y; } }
             }
@@ -946,7 +972,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
             cplx accT[SW_TCOLS];
             #pragma unroll
             for (int tc = 0; tc < SW_TCOLS; ++tc) accT[tc] = cplx{0.0, 0.0};
-            for (int q = 0; q < S.nK; ++q) {
+            for (int q = qK0; q < qK1; ++q) {
                 const cplx *buf = acquire();
                 const int r0 = q * S.rK, rows = min(S.rK, NP - r0);
                 for (int r = 0; r < rows; ++r) {
@@ -960,6 +986,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
                 }
                 release();
             }
+            if (NC > 1) exchange(accT, SW_TCOLS, NT, Tpart, 2);
             // k = -(i/v) P w
             #pragma unroll
             for (int tr = 0; tr < TR; ++tr) {
@@ -982,14 +1009,17 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     // first failed half-step index is kept in traj_status (wpccc_last_status)
     const bool dead = first_bad < a.n_idx || (a.traj_status && a.traj_status[t] != 0);
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-    #pragma unroll
-    for (int tr = 0; tr < TR; ++tr) {
-        const int j = tid + SW_CONSUMERS * tr;
-        if (j < N) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = dead ? qnan : C[tr].x; dst[1] = dead ? qnan : C[tr].y; }
+    if (NC > 1) cluster_sync_all();                  // neither CTA leaves (nor rank 0 touches traj_status) while the other may still read
+    if (rank == 0) {
+        #pragma unroll
+        for (int tr = 0; tr < TR; ++tr) {
+            const int j = tid + SW_CONSUMERS * tr;
+            if (j < N) { double *dst = a.C + ((size_t)t * N + j) * 2; dst[0] = dead ? qnan : C[tr].x; dst[1] = dead ? qnan : C[tr].y; }
+        }
+        if (tid == 0 && a.traj_status && a.traj_status[t] == 0 && first_bad < a.n_idx)
+            a.traj_status[t] = (a.flags[(size_t)t * a.n_idx + first_bad] << 28) | ((int)(a.i0 + first_bad) + 1);
+        if (track && tid == 0) a.drift[t] = dead ? qnan : drift;
     }
-    if (tid == 0 && a.traj_status && a.traj_status[t] == 0 && first_bad < a.n_idx)
-        a.traj_status[t] = (a.flags[(size_t)t * a.n_idx + first_bad] << 28) | ((int)(a.i0 + first_bad) + 1);
-    if (track && tid == 0) a.drift[t] = dead ? qnan : drift;
 }
 }  // namespace
 
@@ -1054,7 +1084,9 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     const int N = a.NT + a.NP;
     if (a.NT > SW_CONSUMERS * SW_TCOLS || a.NP > SW_CONSUMERS * SW_TCOLS) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N_T = %d or N_P = %d exceeds %d", a.NT, a.NP, SW_CONSUMERS * SW_TCOLS);
     if (N > SW_CONSUMERS * 8) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d exceeds %d", N, SW_CONSUMERS * 8);
-    const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB) * 16;
+    // a cluster of two CTAs per trajectory where the streams of one SM are what bounds a stage (wide bases)
+    const int cl = (N >= 384) ? 2 : 1;
+    const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB + (cl > 1 ? 2 * (size_t)N : 0)) * 16;
     // TMA ring: one SM's bulk-copy stream delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s,
     // 32 KB 88, 48 KB 107, 64 KB 133 GB/s), so the chunks are as large as the shared memory allows: three stages of up to 64 KB,
     // two stages when three would be smaller than 48 KB each
@@ -1068,10 +1100,16 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
     const int tr = (N + SW_CONSUMERS - 1) / SW_CONSUMERS;
     wp_span_begin(B, FAM_SWEEP, s);
-#define WP_SWEEP2(SOLVE_, TR_) do { static PerDevice at_; if (wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep2<SOLVE_, TR_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
-        k_sweep2<SOLVE_, TR_><<<n_traj, SW_CONSUMERS + 32, smem, s>>>(a, (int)chunk, NS); } while (0)
-#define WP_SWEEP2_TR(SOLVE_) do { if (tr <= 1) WP_SWEEP2(SOLVE_, 1); else if (tr == 2) WP_SWEEP2(SOLVE_, 2); else if (tr == 3) WP_SWEEP2(SOLVE_, 3); \
-        else if (tr == 4) WP_SWEEP2(SOLVE_, 4); else WP_SWEEP2(SOLVE_, 8); } while (0)
+    cudaLaunchConfig_t lc{};
+    cudaLaunchAttribute lattr[1];
+    lc.gridDim = dim3((unsigned)(n_traj * cl)); lc.blockDim = dim3(SW_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
+    lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)cl; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
+    lc.attrs = lattr; lc.numAttrs = 1;
+    const int chunk_i = (int)chunk;
+#define WP_SWEEP2(SOLVE_, TR_, NC_) do { static PerDevice at_; if (wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep2<SOLVE_, TR_, NC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
+        WP_CUDA(cudaLaunchKernelEx(&lc, k_sweep2<SOLVE_, TR_, NC_>, a, chunk_i, NS)); } while (0)
+#define WP_SWEEP2_TR(SOLVE_) do { if (cl == 1) { if (tr <= 1) WP_SWEEP2(SOLVE_, 1, 1); else WP_SWEEP2(SOLVE_, 2, 1); } \
+        else if (tr == 2) WP_SWEEP2(SOLVE_, 2, 2); else if (tr == 3) WP_SWEEP2(SOLVE_, 3, 2); else if (tr == 4) WP_SWEEP2(SOLVE_, 4, 2); else WP_SWEEP2(SOLVE_, 8, 2); } while (0)
     if (a.solve) WP_SWEEP2_TR(true); else WP_SWEEP2_TR(false);
 #undef WP_SWEEP2_TR
 #undef WP_SWEEP2
