@@ -36,37 +36,46 @@ constexpr int SW1_CONSUMERS = 224;
 // vector x_c as a broadcast, and accumulates in registers -- no reductions, no re-reading of x per matrix row.  The
 // state (C, RK4 accumulator, phases) of a thread's rows lives in registers; only the stage vector X is shared
 // (double-buffered: one block barrier per RK4 stage).  Dynamic smem: ring, then X [2][NV][N] complex.
-template <int NTILE, int NV>
+// NC = 2 (few units, wide basis): a cluster of two CTAs per unit, each streaming one half of the rows of D and multiplying it;
+// the partial sums are exchanged through distributed shared memory once per stage (as in k_sweep2).
+template <int NTILE, int NV, int NC>
 __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args a) {
     extern __shared__ __align__(128) unsigned char smraw1[];
-    const SweepUnit u = a.units[blockIdx.x];
+    const SweepUnit u = a.units[blockIdx.x / NC];
+    const unsigned rank = NC > 1 ? cluster_ctarank() : 0u, peer = rank ^ 1u;
     const int N = a.N, ld = a.ldD, nv = u.n, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int rpc = a.rows_per_chunk, n_chunks = (N + rpc - 1) / rpc;
+    const int q0 = (NC > 1 && rank) ? (n_chunks + 1) / 2 : 0, q1 = (NC > 1 && !rank) ? (n_chunks + 1) / 2 : n_chunks, my_chunks = q1 - q0;
     const size_t chunk_bytes = (size_t)rpc * ld * 8;
     const int NS = a.ring_stages;
     unsigned char *ring = smraw1;
     cplx *X = reinterpret_cast<cplx *>(smraw1 + (size_t)NS * chunk_bytes);           // [2][NV][N]
-    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES];
+    cplx *Ypart = X + (size_t)2 * NV * N;                                            // NC = 2: this CTA's partial sums [NV][N]
+    __shared__ __align__(8) unsigned long long full[SW_STAGES], empty[SW_STAGES], xbar;
     __shared__ double red[SWEEP_NV][8];
     if (tid == 0) {
         for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW1_CONSUMERS / 32); }
+        mbar_init(&xbar, 1);
         mbar_fence_init();
     }
     __syncthreads();
+    if (NC > 1) cluster_sync_all();                  // the peer's mbarrier exists before anything arrives on it
     if (warp == SW1_CONSUMERS / 32) {
-        if (lane != 0) return;
-        const long long total = (long long)a.steps * 4 * n_chunks;
-        for (long long g = 0; g < total; ++g) {
-            const int slot = (int)(g % NS); const long long use = g / NS;
-            if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
-            const int sst = (int)(g / n_chunks), q = (int)(g - (long long)sst * n_chunks), s = sst >> 2, st = sst & 3;
-            const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));
-            const int r0 = q * rpc, rows = min(rpc, N - r0);
-            const double *src = a.D + ((size_t)u.group * a.n_idx + li) * (size_t)N * ld + (size_t)r0 * ld;
-            const unsigned bytes = (unsigned)rows * ld * 8u;
-            mbar_expect_tx(&full[slot], bytes);
-            tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
+        if (lane == 0) {
+            const long long total = (long long)a.steps * 4 * my_chunks;
+            for (long long g = 0; g < total; ++g) {
+                const int slot = (int)(g % NS); const long long use = g / NS;
+                if (use > 0) mbar_wait(&empty[slot], (unsigned)((use - 1) & 1));
+                const int sst = (int)(g / my_chunks), q = q0 + (int)(g - (long long)sst * my_chunks), s = sst >> 2, st = sst & 3;
+                const int li = 2 * s + (st == 0 ? 0 : (st == 3 ? 2 : 1));
+                const int r0 = q * rpc, rows = min(rpc, N - r0);
+                const double *src = a.D + ((size_t)u.group * a.n_idx + li) * (size_t)N * ld + (size_t)r0 * ld;
+                const unsigned bytes = (unsigned)rows * ld * 8u;
+                mbar_expect_tx(&full[slot], bytes);
+                tma_bulk_g2s(ring + (size_t)slot * chunk_bytes, src, bytes, &full[slot]);
+            }
         }
+        if (NC > 1) cluster_sync_all();
         return;
     }
     // ---------------- consumers: thread tid owns rows tid + 224 t
@@ -133,7 +142,7 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
                 for (int t = 0; t < NTILE; ++t)
                     #pragma unroll
                     for (int q = 0; q < NV; ++q) acc[i][t][q] = cplx{0.0, 0.0};
-            for (int c = 0; c < n_chunks; ++c) {
+            for (int c = q0; c < q1; ++c) {
                 const int slot = (int)(g % NS);
                 mbar_wait(&full[slot], (unsigned)((g / NS) & 1));
                 if (active) {
@@ -167,6 +176,24 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
                 for (int t = 0; t < NTILE; ++t)
                     #pragma unroll
                     for (int q = 0; q < NV; ++q) { acc[0][t][q].x += acc[i][t][q].x; acc[0][t][q].y += acc[i][t][q].y; }
+            if (NC > 1) {
+                // add the peer CTA's partial sums (a + b = b + a: both CTAs carry bit-identical vectors)
+                #pragma unroll
+                for (int t = 0; t < NTILE; ++t)
+                    if (row[t] < N) {
+                        #pragma unroll
+                        for (int q = 0; q < NV; ++q) Ypart[q * N + row[t]] = acc[0][t][q];
+                    }
+                bar_sync(1, SW1_CONSUMERS);                  // every partial sum of this CTA is written; every read of the previous stage is done
+                if (tid == 0) mbar_arrive_peer(&xbar, peer);
+                mbar_wait_cluster(&xbar, (unsigned)((s * 4 + st) & 1));
+                #pragma unroll
+                for (int t = 0; t < NTILE; ++t)
+                    if (row[t] < N) {
+                        #pragma unroll
+                        for (int q = 0; q < NV; ++q) { const cplx o = ld_peer(Ypart + q * N + row[t], peer); acc[0][t][q].x += o.x; acc[0][t][q].y += o.y; }
+                    }
+            }
             // k = -(i/v) P y; RK4 accumulation; the next stage's vector goes into the other buffer
             const double wgt = (st == 0 || st == 3) ? 1.0 : 2.0;
             #pragma unroll
@@ -210,6 +237,8 @@ __global__ void __launch_bounds__(SW1_CONSUMERS + 32) k_sweep1(const Sweep1Args 
             bar_sync(1, SW1_CONSUMERS);
         }
     }
+    if (NC > 1) cluster_sync_all();                  // neither CTA leaves while the other may still read its partial sums
+    if (rank != 0) return;
     #pragma unroll
     for (int q = 0; q < NV; ++q)
         if (q < nv) {
@@ -1051,29 +1080,46 @@ void wp_sweep1_plan(int N, int n_rad, int *nv, int *rows_per_chunk, int *stages)
     *rows_per_chunk = rr; *stages = ss;
 }
 
-int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a, cudaStream_t s) {
-    if (n_units <= 0 || a.steps <= 0) return 0;
+int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a_in, cudaStream_t s) {
+    if (n_units <= 0 || a_in.steps <= 0) return 0;
+    Sweep1Args a = a_in;
     int ntile = 0, nvs = 0;
     if (!sweep1_shape(a.N, &ntile, &nvs)) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d exceeds the register-resident design (N <= 4480)", a.N);
     const int nvi = sweep1_nv_instance(ntile, nvs, a.nv);           // a.nv: largest unit of this call
-    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + (size_t)2 * nvi * a.N * 16;
+    // a cluster of two CTAs per unit when the units leave more than half of the SMs idle and a stage is bound by one SM's streams
+    int nc = (a.N >= 384 && ntile >= 2 && ntile <= 4 && 2 * n_units <= 148) ? 2 : 1;
+    const size_t vec = (size_t)2 * nvi * a.N * 16, part = (size_t)nvi * a.N * 16;
+    if (nc > 1) {                                        // room for the partial sums: shorter chunks
+        while (a.rows_per_chunk > 1 && (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) --a.rows_per_chunk;
+        if ((size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) { nc = 1; a.rows_per_chunk = a_in.rows_per_chunk; }
+    }
+    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + (nc > 1 ? part : 0);
     if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
     static PerDevice attr_1;
     const bool raise = wp_raise(attr_1, 1);               // once per device: every instance gets the full shared-memory limit
+    cudaLaunchConfig_t lc{};
+    cudaLaunchAttribute lattr[1];
+    lc.gridDim = dim3((unsigned)(n_units * nc)); lc.blockDim = dim3(SW1_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
+    lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)nc; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
+    lc.attrs = lattr; lc.numAttrs = 1;
     wp_span_begin(B, FAM_SWEEP, s);
-#define WP_SWEEP1(NT_, NV_) do { static PerDevice at_; if (raise || wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
-        k_sweep1<NT_, NV_><<<n_units, SW1_CONSUMERS + 32, smem, s>>>(a); } while (0)
+#define WP_SWEEP1C(NT_, NV_, NC_) do { static PerDevice at_; if (raise || wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_, NC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
+        WP_CUDA(cudaLaunchKernelEx(&lc, k_sweep1<NT_, NV_, NC_>, a)); } while (0)
+#define WP_SWEEP1(NT_, NV_) WP_SWEEP1C(NT_, NV_, 1)
+#define WP_SWEEP1X(NT_, NV_) do { if (nc > 1) WP_SWEEP1C(NT_, NV_, 2); else WP_SWEEP1C(NT_, NV_, 1); } while (0)
     switch (ntile) {
         case 1: if (nvi == 1) WP_SWEEP1(1, 1); else if (nvi == 2) WP_SWEEP1(1, 2); else WP_SWEEP1(1, 4); break;
-        case 2: if (nvi == 1) WP_SWEEP1(2, 1); else if (nvi == 2) WP_SWEEP1(2, 2); else WP_SWEEP1(2, 4); break;
-        case 3: if (nvi == 1) WP_SWEEP1(3, 1); else WP_SWEEP1(3, 3); break;
-        case 4: WP_SWEEP1(4, 2); break;
+        case 2: if (nvi == 1) WP_SWEEP1X(2, 1); else if (nvi == 2) WP_SWEEP1X(2, 2); else WP_SWEEP1X(2, 4); break;
+        case 3: if (nvi == 1) WP_SWEEP1X(3, 1); else WP_SWEEP1X(3, 3); break;
+        case 4: WP_SWEEP1X(4, 2); break;
         case 6: WP_SWEEP1(6, 1); break;
         case 9: WP_SWEEP1(9, 1); break;
         case 14: WP_SWEEP1(14, 1); break;
         default: WP_SWEEP1(20, 1); break;
     }
 #undef WP_SWEEP1
+#undef WP_SWEEP1X
+#undef WP_SWEEP1C
     wp_span_end(B, s, 1);
     WP_CUDA(cudaGetLastError());
     return 0;
