@@ -245,6 +245,7 @@ extern "C" int wpccc_set_option(wpccc_basis *B, const char *key, long long value
     else if (k == "solve_route") { if (value < 0 || value > 1) WP_FAIL(WPCCC_EINVAL, "solve_route: 0 (Cholesky factor + triangular solves) or 1 (explicit inverse, Gauss-Jordan with partial pivoting)"); B->opt.solve_route = (int)value; }
     else if (k == "inverse_kernel") { if (value < 0 || value > 2) WP_FAIL(WPCCC_EINVAL, "inverse_kernel: 0 auto, 1 shared-memory, 2 global-memory blocked"); B->opt.inverse_kernel = (int)value; }
     else if (k == "inverse_chunk_cols") { if (value < 0) WP_FAIL(WPCCC_EINVAL, "inverse_chunk_cols: >= 0 (0 = automatic)"); B->opt.inverse_chunk_cols = (int)value; }
+    else if (k == "sweep_cluster") { if (value != 0 && value != 1 && value != 2 && value != 4) WP_FAIL(WPCCC_EINVAL, "sweep_cluster: 0 (automatic), 1, 2 or 4 CTAs per trajectory"); B->opt.sweep_cluster = (int)value; }
     else if (k == "timing") { B->opt.timing = value != 0; }
     else WP_FAIL(WPCCC_EINVAL, "unknown option '%s'", key);
     return 0;

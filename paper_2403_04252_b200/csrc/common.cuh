@@ -125,6 +125,7 @@ struct wpccc_basis {
         int solve_route = 0;         // 0: Cholesky factor of I - K K^H + triangular solves per RK4 stage; 1: explicit inverse (Gauss-Jordan)
         int inverse_kernel = 0;      // solve_route 1: 0 automatic, 1 shared-memory kernel, 2 global-memory blocked kernel
         int inverse_chunk_cols = 0;  // solve_route 1, register kernel: K staged in chunks of this many columns (0: automatic)
+        int sweep_cluster = 0;       // CTAs per trajectory of the two-centre sweep / per unit of the one-centre sweep: 0 automatic, 1, 2, 4 forced
         bool timing = true;          // record CUDA events per kernel family (wpccc_last_timing)
     } opt;
     std::vector<int> last_status;

@@ -683,7 +683,7 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     extern __shared__ __align__(128) unsigned char smraw[];
     const int NT = a.NT, NP = a.NP, N = NT + NP, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int t = blockIdx.x / NC;
-    const unsigned rank = NC > 1 ? cluster_ctarank() : 0u, peer = rank ^ 1u;
+    const unsigned rank = NC > 1 ? cluster_ctarank() : 0u;
     const bool track = a.drift != nullptr;
     const SweepSched S(NT, NP, chunk_bytes);
     const CholLayout CL(NP);
@@ -699,16 +699,16 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     __shared__ int redi[8];
     if (tid == 0) {
         for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], SW_CONSUMERS / 32); }
-        for (int s = 0; s < 3; ++s) mbar_init(&xbar[s], 1);
+        for (int s = 0; s < 3; ++s) mbar_init(&xbar[s], NC > 1 ? NC - 1 : 1);
         mbar_fence_init();
     }
     __syncthreads();
     if (NC > 1) cluster_sync_all();                  // the peer's mbarriers exist before anything arrives on them
     // chunk ranges of this CTA in the three split products
-    const int hH = NC > 1 ? (S.nH + 1) / 2 : S.nH, hKT = NC > 1 ? (S.nKT + 1) / 2 : S.nKT, hK = NC > 1 ? (S.nK + 1) / 2 : S.nK;
-    const int qH0 = rank ? hH : 0, qH1 = (NC > 1 && rank == 0) ? hH : S.nH;
-    const int qT0 = rank ? hKT : 0, qT1 = (NC > 1 && rank == 0) ? hKT : S.nKT;
-    const int qK0 = rank ? hK : 0, qK1 = (NC > 1 && rank == 0) ? hK : S.nK;
+    const int hH = (S.nH + NC - 1) / NC, hKT = (S.nKT + NC - 1) / NC, hK = (S.nK + NC - 1) / NC;
+    const int qH0 = min(S.nH, (int)rank * hH), qH1 = min(S.nH, qH0 + hH);
+    const int qT0 = min(S.nKT, (int)rank * hKT), qT1 = min(S.nKT, qT0 + hKT);
+    const int qK0 = min(S.nK, (int)rank * hK), qK1 = min(S.nK, qK0 + hK);
     const cplx *Hg = reinterpret_cast<const cplx *>(a.H), *Kg = reinterpret_cast<const cplx *>(a.K), *Ag = reinterpret_cast<const cplx *>(a.Ainv);
     const cplx *KTg = reinterpret_cast<const cplx *>(a.KT);
     const size_t a_stride = wp_factor_elems(NP);
@@ -793,10 +793,19 @@ __global__ void __launch_bounds__(SW_CONSUMERS + 32, 1) k_sweep2(const Sweep2Arg
     auto exchange = [&](cplx *val, int nval, int n, cplx *buf, int which) {
         for (int k = 0; k < nval; ++k) { const int j = tid + SW_CONSUMERS * k; if (j < n) buf[j] = val[k]; }
         consumer_sync();                                     // every partial sum of this CTA is in `buf` (and every read of the previous exchange is done)
-        if (tid == 0) mbar_arrive_peer(&xbar[which], peer);
+        if (tid < NC && tid != (int)rank) mbar_arrive_peer(&xbar[which], (unsigned)tid);
         mbar_wait_cluster(&xbar[which], (xphase >> which) & 1u);
         xphase ^= 1u << which;
-        for (int k = 0; k < nval; ++k) { const int j = tid + SW_CONSUMERS * k; if (j < n) { const cplx o = ld_peer(buf + j, peer); val[k].x += o.x; val[k].y += o.y; } }
+        // summed in rank order by every CTA of the cluster: bit-identical vectors everywhere
+        for (int k = 0; k < nval; ++k) {
+            const int j = tid + SW_CONSUMERS * k;
+            if (j < n) {
+                cplx sum = {0.0, 0.0};
+                #pragma unroll
+                for (int r = 0; r < NC; ++r) { const cplx o = (r == (int)rank) ? buf[j] : ld_peer(buf + j, (unsigned)r); sum.x += o.x; sum.y += o.y; }
+                val[k] = sum;
+            }
+        }
     };
 
     for (int s = 0; s < a.steps; ++s) {
@@ -1088,6 +1097,8 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a_in, cud
     const int nvi = sweep1_nv_instance(ntile, nvs, a.nv);           // a.nv: largest unit of this call
     // a cluster of two CTAs per unit when the units leave more than half of the SMs idle and a stage is bound by one SM's streams
     int nc = (a.N >= 384 && ntile >= 2 && ntile <= 4 && 2 * n_units <= 148) ? 2 : 1;
+    if (B->opt.sweep_cluster == 1) nc = 1;
+    else if (B->opt.sweep_cluster >= 2 && ntile >= 2 && ntile <= 4) nc = 2;
     const size_t vec = (size_t)2 * nvi * a.N * 16, part = (size_t)nvi * a.N * 16;
     if (nc > 1) {                                        // room for the partial sums: shorter chunks
         while (a.rows_per_chunk > 1 && (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) --a.rows_per_chunk;
@@ -1131,7 +1142,12 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     if (a.NT > SW_CONSUMERS * SW_TCOLS || a.NP > SW_CONSUMERS * SW_TCOLS) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N_T = %d or N_P = %d exceeds %d", a.NT, a.NP, SW_CONSUMERS * SW_TCOLS);
     if (N > SW_CONSUMERS * 8) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d exceeds %d", N, SW_CONSUMERS * 8);
     // a cluster of two CTAs per trajectory where the streams of one SM are what bounds a stage (wide bases)
-    const int cl = (N >= 384) ? 2 : 1;
+    const int tr = (N + SW_CONSUMERS - 1) / SW_CONSUMERS;
+    int cl = (N >= 512) ? 4 : ((N >= 384) ? 2 : 1);
+    if (B->opt.sweep_cluster) cl = B->opt.sweep_cluster;
+    // kernel instances: one CTA for TR <= 2, two CTAs for TR <= 2, four CTAs for any TR
+    if (cl == 1 && tr > 2) cl = 2;
+    if (cl == 2 && tr > 2) cl = 4;
     const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB + (cl > 1 ? 2 * (size_t)N : 0)) * 16;
     // TMA ring: one SM's bulk-copy stream delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s,
     // 32 KB 88, 48 KB 107, 64 KB 133 GB/s), so the chunks are as large as the shared memory allows: three stages of up to 64 KB,
@@ -1144,7 +1160,6 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     if (chunk < chunk_min) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
     const size_t smem = NS * chunk + vec;
     if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
-    const int tr = (N + SW_CONSUMERS - 1) / SW_CONSUMERS;
     wp_span_begin(B, FAM_SWEEP, s);
     cudaLaunchConfig_t lc{};
     cudaLaunchAttribute lattr[1];
@@ -1155,7 +1170,8 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
 #define WP_SWEEP2(SOLVE_, TR_, NC_) do { static PerDevice at_; if (wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep2<SOLVE_, TR_, NC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
         WP_CUDA(cudaLaunchKernelEx(&lc, k_sweep2<SOLVE_, TR_, NC_>, a, chunk_i, NS)); } while (0)
 #define WP_SWEEP2_TR(SOLVE_) do { if (cl == 1) { if (tr <= 1) WP_SWEEP2(SOLVE_, 1, 1); else WP_SWEEP2(SOLVE_, 2, 1); } \
-        else if (tr == 2) WP_SWEEP2(SOLVE_, 2, 2); else if (tr == 3) WP_SWEEP2(SOLVE_, 3, 2); else if (tr == 4) WP_SWEEP2(SOLVE_, 4, 2); else WP_SWEEP2(SOLVE_, 8, 2); } while (0)
+        else if (cl == 2) WP_SWEEP2(SOLVE_, 2, 2); \
+        else if (tr <= 3) WP_SWEEP2(SOLVE_, 3, 4); else if (tr == 4) WP_SWEEP2(SOLVE_, 4, 4); else WP_SWEEP2(SOLVE_, 8, 4); } while (0)
     if (a.solve) WP_SWEEP2_TR(true); else WP_SWEEP2_TR(false);
 #undef WP_SWEEP2_TR
 #undef WP_SWEEP2

@@ -253,6 +253,36 @@ def test_two_centre_mirror_pairs(lib, two_centre):
     assert np.abs(Ca[0] - co).max() < PTOL
 
 
+def test_sweep_cluster_sizes_agree(lib, two_centre):
+    """wpccc_set_option "sweep_cluster": the two-centre RK4 sweep on one CTA per trajectory and on thread-block clusters of two
+    and four CTAs (products split by rows, partial sums exchanged through distributed shared memory) -- the same amplitudes
+    to rounding, on both solve routes, with the norm tracked, over several windows; and against the oracle."""
+    prob, basis = two_centre
+    b, v = np.array([0.7, 1.9, 1.2]), np.array([1.0, 1.3, 0.8])
+    n_steps = 70
+    ref = {}
+    try:
+        for route in (0, 1):
+            basis.set_option("solve_route", route)
+            for nc in (1, 2, 4):
+                basis.set_option("sweep_cluster", nc)
+                C, drift = lib.propagate(basis, b, v, -7.0, 7.0, n_steps, track_norm=True)
+                C, drift = C.cpu().numpy(), drift.cpu().numpy()
+                assert np.isfinite(C).all()
+                if nc == 1:
+                    ref[route] = (C, drift)
+                else:
+                    assert np.abs(C - ref[route][0]).max() < 1e-13, (route, nc, np.abs(C - ref[route][0]).max())
+                    assert np.abs(drift - ref[route][1]).max() < 1e-12
+    finally:
+        basis.set_option("solve_route", 0)
+        basis.set_option("sweep_cluster", 0)
+    co = oprop.propagate(prob, b[0], v[0], -7.0, 7.0, n_steps)
+    assert np.abs(ref[0][0][0] - co).max() < PTOL
+    with pytest.raises(lib.WpcccError):
+        basis.set_option("sweep_cluster", 3)
+
+
 ROUTES = (("cholesky + triangular solves", {"solve_route": 0}),
           ("inverse, registers", {"solve_route": 1}),
           ("inverse, registers, K staged in chunks of 5 columns", {"solve_route": 1, "inverse_chunk_cols": 5}),
