@@ -147,7 +147,7 @@ size_t wpccc_workspace_bytes(const wpccc_basis *basis, int n_traj, int n_steps, 
  *   "inverse_kernel"     solve_route 1 only: 0 automatic, 1 shared-memory kernel, 2 global-memory blocked kernel.
  *   "inverse_chunk_cols" solve_route 1, register kernel: stage K in chunks of this many columns (0 automatic).
  *   "sweep_cluster"      CTAs (one thread-block cluster) per trajectory of the RK4 sweep a8: 0 (default) automatic -- one CTA for
- *                        narrow bases, two or four for wide ones, where the streams of one SM bound a stage -- or 1, 2, 4
+ *                        small bases (N < 128), two up to N = 511, four beyond, where the streams of one SM bound a stage -- or 1, 2, 4
  *                        forced (4: two-centre only; a size the basis has no kernel instance for falls back to the nearest).
  *                        The CTAs of a cluster split the matrix-vector products of a stage by rows and exchange partial sums
  *                        through distributed shared memory; results agree to rounding (the summation order differs).

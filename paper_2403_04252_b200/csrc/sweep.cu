@@ -1141,9 +1141,10 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     const int N = a.NT + a.NP;
     if (a.NT > SW_CONSUMERS * SW_TCOLS || a.NP > SW_CONSUMERS * SW_TCOLS) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N_T = %d or N_P = %d exceeds %d", a.NT, a.NP, SW_CONSUMERS * SW_TCOLS);
     if (N > SW_CONSUMERS * 8) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d exceeds %d", N, SW_CONSUMERS * 8);
-    // a cluster of two CTAs per trajectory where the streams of one SM are what bounds a stage (wide bases)
+    // a cluster of CTAs per trajectory: the streams of one SM bound a stage of a wide basis, and even at N = 172 halving them pays
     const int tr = (N + SW_CONSUMERS - 1) / SW_CONSUMERS;
-    int cl = (N >= 512) ? 4 : ((N >= 384) ? 2 : 1);
+    int cl = (N >= 512) ? 4 : ((N >= 128) ? 2 : 1);     // measured: configs[1] (N = 172) 229 -> 164 ms of sweep per job with two CTAs (154 with four, but
+                                                        // the element stream then loses more than that); configs[3] (N = 572) 1.77 -> 1.40 -> 1.06 s
     if (B->opt.sweep_cluster) cl = B->opt.sweep_cluster;
     // kernel instances: one CTA for TR <= 2, two CTAs for TR <= 2, four CTAs for any TR
     if (cl == 1 && tr > 2) cl = 2;
