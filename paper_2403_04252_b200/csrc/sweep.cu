@@ -1100,33 +1100,41 @@ int wp_sweep_one_centre(wpccc_basis *B, int n_units, const Sweep1Args &a_in, cud
     if (B->opt.sweep_cluster == 1) nc = 1;
     else if (B->opt.sweep_cluster >= 2 && ntile >= 2 && ntile <= 4) nc = 2;
     const size_t vec = (size_t)2 * nvi * a.N * 16, part = (size_t)nvi * a.N * 16;
-    if (nc > 1) {                                        // room for the partial sums: shorter chunks
-        while (a.rows_per_chunk > 1 && (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) --a.rows_per_chunk;
-        if ((size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) { nc = 1; a.rows_per_chunk = a_in.rows_per_chunk; }
-    }
-    const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + (nc > 1 ? part : 0);
-    if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
     static PerDevice attr_1;
     const bool raise = wp_raise(attr_1, 1);               // once per device: every instance gets the full shared-memory limit
-    cudaLaunchConfig_t lc{};
-    cudaLaunchAttribute lattr[1];
-    lc.gridDim = dim3((unsigned)(n_units * nc)); lc.blockDim = dim3(SW1_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
-    lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)nc; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
-    lc.attrs = lattr; lc.numAttrs = 1;
     wp_span_begin(B, FAM_SWEEP, s);
 #define WP_SWEEP1C(NT_, NV_, NC_) do { static PerDevice at_; if (raise || wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep1<NT_, NV_, NC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
-        WP_CUDA(cudaLaunchKernelEx(&lc, k_sweep1<NT_, NV_, NC_>, a)); } while (0)
+        lerr = cudaLaunchKernelEx(&lc, k_sweep1<NT_, NV_, NC_>, a); } while (0)
 #define WP_SWEEP1(NT_, NV_) WP_SWEEP1C(NT_, NV_, 1)
 #define WP_SWEEP1X(NT_, NV_) do { if (nc > 1) WP_SWEEP1C(NT_, NV_, 2); else WP_SWEEP1C(NT_, NV_, 1); } while (0)
-    switch (ntile) {
-        case 1: if (nvi == 1) WP_SWEEP1(1, 1); else if (nvi == 2) WP_SWEEP1(1, 2); else WP_SWEEP1(1, 4); break;
-        case 2: if (nvi == 1) WP_SWEEP1X(2, 1); else if (nvi == 2) WP_SWEEP1X(2, 2); else WP_SWEEP1X(2, 4); break;
-        case 3: if (nvi == 1) WP_SWEEP1X(3, 1); else WP_SWEEP1X(3, 3); break;
-        case 4: WP_SWEEP1X(4, 2); break;
-        case 6: WP_SWEEP1(6, 1); break;
-        case 9: WP_SWEEP1(9, 1); break;
-        case 14: WP_SWEEP1(14, 1); break;
-        default: WP_SWEEP1(20, 1); break;
+    for (;;) {
+        a.rows_per_chunk = a_in.rows_per_chunk;
+        if (nc > 1) {                                        // room for the partial sums: shorter chunks
+            while (a.rows_per_chunk > 1 && (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) --a.rows_per_chunk;
+            if ((size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + part > 225 * 1024) { nc = 1; a.rows_per_chunk = a_in.rows_per_chunk; }
+        }
+        const size_t smem = (size_t)a.ring_stages * a.rows_per_chunk * a.ldD * 8 + vec + (nc > 1 ? part : 0);
+        if (smem > 227 * 1024 - 1024) WP_FAIL(WPCCC_EINVAL, "one-centre sweep: N = %d too large for shared memory", a.N);
+        cudaLaunchConfig_t lc{};
+        cudaLaunchAttribute lattr[1];
+        lc.gridDim = dim3((unsigned)(n_units * nc)); lc.blockDim = dim3(SW1_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
+        lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)nc; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
+        lc.attrs = lattr; lc.numAttrs = 1;
+        cudaError_t lerr = cudaSuccess;
+        switch (ntile) {
+            case 1: if (nvi == 1) WP_SWEEP1(1, 1); else if (nvi == 2) WP_SWEEP1(1, 2); else WP_SWEEP1(1, 4); break;
+            case 2: if (nvi == 1) WP_SWEEP1X(2, 1); else if (nvi == 2) WP_SWEEP1X(2, 2); else WP_SWEEP1X(2, 4); break;
+            case 3: if (nvi == 1) WP_SWEEP1X(3, 1); else WP_SWEEP1X(3, 3); break;
+            case 4: WP_SWEEP1X(4, 2); break;
+            case 6: WP_SWEEP1(6, 1); break;
+            case 9: WP_SWEEP1(9, 1); break;
+            case 14: WP_SWEEP1(14, 1); break;
+            default: WP_SWEEP1(20, 1); break;
+        }
+        if (lerr == cudaSuccess) break;
+        (void)cudaGetLastError();
+        if (nc == 1) { wp_set_error("one-centre sweep: launch failed -> %s", cudaGetErrorString(lerr)); return WPCCC_ECUDA; }
+        nc = 1;                                          // the cluster cannot be placed on this device: one CTA per unit
     }
 #undef WP_SWEEP1
 #undef WP_SWEEP1X
@@ -1149,31 +1157,40 @@ int wp_sweep_two_centre(wpccc_basis *B, int n_traj, const Sweep2Args &a, cudaStr
     // kernel instances: one CTA for TR <= 2, two CTAs for TR <= 2, four CTAs for any TR
     if (cl == 1 && tr > 2) cl = 2;
     if (cl == 2 && tr > 2) cl = 4;
-    const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB + (cl > 1 ? 2 * (size_t)N : 0)) * 16;
-    // TMA ring: one SM's bulk-copy stream delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s,
-    // 32 KB 88, 48 KB 107, 64 KB 133 GB/s), so the chunks are as large as the shared memory allows: three stages of up to 64 KB,
-    // two stages when three would be smaller than 48 KB each
-    const size_t chunk_min = std::max((size_t)16 * N, (size_t)16 * CHOL_NB * CHOL_NB), room = (size_t)220 * 1024 - vec;
-    int NS = 3;
-    size_t chunk = std::min<size_t>(64 * 1024, room / 3);
-    if (chunk < 48 * 1024) { NS = 2; chunk = std::min<size_t>(96 * 1024, room / 2); }
-    chunk &= ~(size_t)127;
-    if (chunk < chunk_min) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
-    const size_t smem = NS * chunk + vec;
-    if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
     wp_span_begin(B, FAM_SWEEP, s);
-    cudaLaunchConfig_t lc{};
-    cudaLaunchAttribute lattr[1];
-    lc.gridDim = dim3((unsigned)(n_traj * cl)); lc.blockDim = dim3(SW_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
-    lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)cl; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
-    lc.attrs = lattr; lc.numAttrs = 1;
-    const int chunk_i = (int)chunk;
 #define WP_SWEEP2(SOLVE_, TR_, NC_) do { static PerDevice at_; if (wp_raise(at_, 1)) WP_CUDA(cudaFuncSetAttribute(k_sweep2<SOLVE_, TR_, NC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024)); \
-        WP_CUDA(cudaLaunchKernelEx(&lc, k_sweep2<SOLVE_, TR_, NC_>, a, chunk_i, NS)); } while (0)
+        lerr = cudaLaunchKernelEx(&lc, k_sweep2<SOLVE_, TR_, NC_>, a, chunk_i, NS); } while (0)
 #define WP_SWEEP2_TR(SOLVE_) do { if (cl == 1) { if (tr <= 1) WP_SWEEP2(SOLVE_, 1, 1); else WP_SWEEP2(SOLVE_, 2, 1); } \
         else if (cl == 2) WP_SWEEP2(SOLVE_, 2, 2); \
         else if (tr <= 3) WP_SWEEP2(SOLVE_, 3, 4); else if (tr == 4) WP_SWEEP2(SOLVE_, 4, 4); else WP_SWEEP2(SOLVE_, 8, 4); } while (0)
-    if (a.solve) WP_SWEEP2_TR(true); else WP_SWEEP2_TR(false);
+    for (;;) {
+        const size_t vec = ((size_t)2 * N + a.NP + CHOL_NB + CHOL_NB * SW_DLD + 8 * CHOL_NB + (cl > 1 ? 2 * (size_t)N : 0)) * 16;
+        // TMA ring: one SM's bulk-copy stream delivers about chunk / 0.36 us whatever the ring depth (measured: 16 KB chunks 46 GB/s,
+        // 32 KB 88, 48 KB 107, 64 KB 133 GB/s), so the chunks are as large as the shared memory allows: three stages of up to 64 KB,
+        // two stages when three would be smaller than 48 KB each
+        const size_t chunk_min = std::max((size_t)16 * N, (size_t)16 * CHOL_NB * CHOL_NB), room = (size_t)220 * 1024 - vec;
+        int NS = 3;
+        size_t chunk = std::min<size_t>(64 * 1024, room / 3);
+        if (chunk < 48 * 1024) { NS = 2; chunk = std::min<size_t>(96 * 1024, room / 2); }
+        chunk &= ~(size_t)127;
+        if (chunk < chunk_min) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
+        const size_t smem = NS * chunk + vec;
+        if (smem > 225 * 1024) WP_FAIL(WPCCC_EINVAL, "two-centre sweep: N = %d too large for shared memory", N);
+        cudaLaunchConfig_t lc{};
+        cudaLaunchAttribute lattr[1];
+        lc.gridDim = dim3((unsigned)(n_traj * cl)); lc.blockDim = dim3(SW_CONSUMERS + 32); lc.dynamicSmemBytes = smem; lc.stream = s;
+        lattr[0].id = cudaLaunchAttributeClusterDimension; lattr[0].val.clusterDim.x = (unsigned)cl; lattr[0].val.clusterDim.y = 1; lattr[0].val.clusterDim.z = 1;
+        lc.attrs = lattr; lc.numAttrs = 1;
+        const int chunk_i = (int)chunk;
+        cudaError_t lerr = cudaSuccess;
+        if (a.solve) WP_SWEEP2_TR(true); else WP_SWEEP2_TR(false);
+        if (lerr == cudaSuccess) break;
+        (void)cudaGetLastError();
+        // a cluster of this size cannot be placed on this device (fewer SMs per GPC, a partitioned GPU): the next smaller size
+        // that has a kernel instance for this basis, if any
+        if (cl == 1 || tr > 2) { wp_set_error("two-centre sweep: launch failed with %d CTAs per trajectory -> %s", cl, cudaGetErrorString(lerr)); return WPCCC_ECUDA; }
+        cl /= 2;
+    }
 #undef WP_SWEEP2_TR
 #undef WP_SWEEP2
     wp_span_end(B, s, 1);
